@@ -1,0 +1,365 @@
+#!/usr/bin/env python
+"""bench.py -- RBE k-space ns/atom/step and fraction of roofline (BASELINE.json metric).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config NAME] [--impl reference]
+
+One *step* = one pass of the whole hot path over one batch of synthetic input:
+rbe_set_kvectors (a fresh, pre-generated k-set) + rbe_structure_factor + rbe_forces.
+Workload at N = 1: BASELINE.json configs[2] (water + NaCl, N = 999 999, P = 200), the one the
+metric is quoted on.  With N > 1 GPUs (torchrun) the atoms are sharded, one rank per GPU, the
+k-set is replicated and the P complex structure factors are summed across ranks (weak
+scaling: every rank owns 999 999 atoms of an n-times larger box at the same density).
+
+Prints ONE JSON line (rank 0).  See DESIGN.md section 7 for every field.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import tempfile
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+METRIC = "rbe_kspace_ns_per_atom_step"
+UNIT = "ns/atom/step"
+# SFU (MUFU) issue peak: 16 lanes/SM/clk x SMs x max SM clock (checked by
+# the pipe microbenchmark in profiles/).  SURVEY.md s8(d): 2 sincos evaluations per (atom, k)
+# pair per kernel are the algorithmic work that bounds this path.
+MUFU_LANES_PER_SM = 16
+FP32_LANES_PER_SM = 128
+SFU_PER_PAIR_PER_KERNEL = 2
+FMA_PER_PAIR_STEP = 13
+BYTES_PER_ATOM_STEP = 48
+
+
+def read_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return {"hbm_gbs": float(d["hbm_gbs"]), "sm_max_mhz": float(d.get("sm_max_mhz", 1965.0)), "src": "measured"}
+    return {"hbm_gbs": 6650.0, "sm_max_mhz": 1965.0, "src": "fallback"}
+
+
+def roofline_times(n_atoms, P, num_sms, peaks):
+    clk = peaks["sm_max_mhz"] * 1e6
+    sfu_rate = num_sms * MUFU_LANES_PER_SM * clk
+    fma_rate = num_sms * FP32_LANES_PER_SM * clk
+    t_hbm = BYTES_PER_ATOM_STEP * n_atoms / (peaks["hbm_gbs"] * 1e9)
+    t_fma = FMA_PER_PAIR_STEP * n_atoms * P / fma_rate
+    t_sfu = 2 * SFU_PER_PAIR_PER_KERNEL * n_atoms * P / sfu_rate
+    return {"hbm": t_hbm, "fma": t_fma, "sfu": t_sfu}, sfu_rate
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled DURING the timed region."""
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,"
+         "clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu_index):
+        self.idx, self.proc, self.path = gpu_index, None, None
+
+    def start(self):
+        try:
+            fd, self.path = tempfile.mkstemp(suffix=".csv")
+            os.close(fd)
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", f"--id={self.idx}", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "50"],
+                stdout=open(self.path, "w"), stderr=subprocess.DEVNULL)
+        except Exception:
+            self.proc = None
+
+    def stop(self):
+        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        if self.proc is None:
+            return out
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for line in open(self.path):
+            f = [x.strip() for x in line.split(",")]
+            if len(f) < 9:
+                continue
+            try:
+                sm.append(float(f[1])); mx.append(float(f[2]))
+            except ValueError:
+                continue
+            for n, v in zip(names, f[5:9]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        os.unlink(self.path)
+        if sm:
+            out.update(sm_mhz=statistics.median(sm), sm_max_mhz=max(mx), reasons=sorted(reasons), samples=len(sm))
+        return out
+
+
+def time_oracle(cfg_name, n_sample, steps, warmup):
+    """The oracle as it stands, timed on the host cores, on the first n_sample atoms of the
+    workload (cost is linear in atoms) with the workload's full batch of P wavevectors."""
+    import oracle
+    from paper_2407_09315_b200 import inputs
+    cfg = workload_config(cfg_name, 1)
+    atoms = inputs.make_atoms(cfg)[:n_sample].copy()
+    S = oracle.S(cfg.L, cfg.alpha)
+    ts = []
+    for it in range(warmup + steps):
+        m = inputs.sample_kset(cfg.L, cfg.alpha, cfg.P, cfg.seed, it)
+        t0 = time.perf_counter()
+        rho = oracle.rho(atoms, cfg.L, m)
+        oracle.force(atoms, cfg.L, m, S, rho)
+        dt = time.perf_counter() - t0
+        if it >= warmup:
+            ts.append(dt)
+    per_step = sum(ts) / len(ts)
+    return per_step, per_step / n_sample * 1e9, oracle.max_threads(), cfg
+
+
+def workload_config(name, world):
+    from paper_2407_09315_b200 import inputs
+    if name.startswith("ions_"):
+        parts = name.split("_")
+        n = int(float(parts[1]))
+        P = int(parts[2][1:]) if len(parts) > 2 else 200
+        return inputs.ions_config(n, P)
+    return inputs.CONFIGS[name]
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    n_sample = args.ref_atoms
+    steps, warmup = max(1, args.steps), max(0, args.warmup)
+    # keep the whole run within a few minutes whatever --steps says
+    budget_s, est_per_atom = 150.0, 200 * 100e-9
+    n_sample = int(min(n_sample, max(1000, budget_s / ((steps + warmup) * est_per_atom))))
+    per_step, ns_atom, cores, cfg = time_oracle(args.config, n_sample, steps, warmup)
+    sample = f"first {n_sample} atoms of {cfg.name} (N={cfg.N}), all P={cfg.P} wavevectors, oracle.rho + oracle.force"
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": ns_atom, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": steps, "warmup": warmup, "ms_per_step": per_step * 1e3, "higher_is_better": False,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": cfg.name, "N": cfg.N, "P": cfg.P, "L": cfg.L, "alpha": cfg.alpha},
+        "cpu_baseline": {"value": ns_atom, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": ns_atom, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=200)
+    ap.add_argument("--warmup", type=int, default=20)
+    ap.add_argument("--config", default="water_nacl_1m")
+    ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
+    ap.add_argument("--ref-atoms", type=int, default=100_000)
+    ap.add_argument("--cpu-baseline-atoms", type=int, default=500_000)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--with-energy", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+    args.warmup = max(3, args.warmup)
+
+    import torch
+    import torch.distributed as dist
+    from paper_2407_09315_b200 import inputs, rbe
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the RBE path has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    if world > 1:
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+
+    base = workload_config(args.config, world)
+    # weak scaling: every rank owns base.N atoms of a box `world` times larger, same density
+    L = base.L * world ** (1.0 / 3.0)
+    n_local, n_total, P, alpha = base.N, base.N * world, base.P, base.alpha
+    cfg_r = inputs.Config(base.name, base.N, base.L, base.P, base.seed + 1000 * rank, base.kind,
+                          base.n_water, base.n_ion_pairs, base.alpha)
+    atoms = inputs.make_atoms(cfg_r)
+    if world > 1:
+        atoms[:, :3] *= np.float32(L / base.L)  # spread the shard over the larger box
+
+    ctx = rbe.Rbe(n_local, L, alpha, P)
+    info = ctx.rbe_get_launch_info()
+    # inputs larger than L2: rotate over enough {xyzq, force} buffer pairs to exceed 126 MB
+    n_rot = max(2, int(np.ceil(160e6 / max(1, 32 * n_local))))
+    n_rot = min(n_rot, 64)
+    xs = [torch.from_numpy(atoms).cuda() for _ in range(n_rot)]
+    fs = [torch.empty((n_local, 4), dtype=torch.float32, device="cuda") for _ in range(n_rot)]
+    n_k = args.warmup + args.steps
+    ksets = [inputs.sample_kset(L, alpha, P, base.seed, t) for t in range(n_k)]
+    rho_local = torch.empty((P, 2), dtype=torch.float64, device="cuda")
+    gathered = torch.empty((world, P, 2), dtype=torch.float64, device="cuda") if world > 1 else None
+
+    def step(i, ev=None):
+        x, f = xs[i % n_rot], fs[i % n_rot]
+        ctx.rbe_set_kvectors(ksets[i % n_k])
+        if ev: ev[0].record()
+        ctx.rbe_structure_factor(x, rho_local if world > 1 else None)
+        if world > 1:
+            dist.all_gather_into_tensor(gathered, rho_local)
+            ctx.rbe_set_rho(gathered.sum(0))  # fixed (rank) order
+        if ev: ev[1].record()
+        ctx.rbe_forces(x, f, args.with_energy)
+        if ev: ev[2].record()
+
+    def sync():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for i in range(args.warmup):
+        step(i)
+    sync()
+
+    # ---- timed region A: exactly K steps, device-timed, nothing else on the stream
+    sampler = ClockSampler(local_rank)
+    if rank == 0:
+        sampler.start()
+        time.sleep(0.15)
+    sync()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for i in range(args.steps):
+        step(args.warmup + i)
+    e1.record()
+    sync()
+    ms_total = e0.elapsed_time(e1)
+
+    # ---- timed region B: the same K steps with CUDA events around each call, for the
+    # per-kernel durations the roofline object needs
+    evs = [[torch.cuda.Event(enable_timing=True) for _ in range(3)] for _ in range(args.steps)]
+    sync()
+    for i in range(args.steps):
+        step(args.warmup + i, evs[i])
+    sync()
+    clocks = sampler.stop() if rank == 0 else None
+    t_sf = [e[0].elapsed_time(e[1]) for e in evs]
+    t_f = [e[1].elapsed_time(e[2]) for e in evs]
+    ms_sf, ms_f = sum(t_sf) / len(t_sf), sum(t_f) / len(t_f)
+
+    if world > 1:
+        t = torch.tensor([ms_total, ms_sf, ms_f], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms_total, ms_sf, ms_f = [float(v) for v in t.cpu()]
+    ms_step = ms_total / args.steps
+    value = ms_step * 1e6 / n_total            # whole job: all atoms of all ranks per step time
+
+    # ---- end to end through the C ABI with HOST buffers (pinned), copies inside the timed region
+    e2e = None
+    if not args.no_e2e:
+        hx = torch.from_numpy(atoms).pin_memory()
+        hf = torch.empty((n_local, 4), dtype=torch.float32).pin_memory()
+        k_e2e = max(3, min(args.steps, 20))
+        if world == 1:
+            for i in range(3):
+                ctx.rbe_step_host(hx, ksets[i % n_k], hf, with_energy=args.with_energy)
+            sync()
+            t0 = time.perf_counter()
+            e0.record()
+            for i in range(k_e2e):
+                ctx.rbe_step_host(hx, ksets[i % n_k], hf, with_energy=args.with_energy)
+            e1.record()
+            sync()
+            ms_e2e = e0.elapsed_time(e1) / k_e2e
+        else:
+            dx = torch.empty((n_local, 4), dtype=torch.float32, device="cuda")
+            df = torch.empty((n_local, 4), dtype=torch.float32, device="cuda")
+
+            def e2e_step(i):
+                dx.copy_(hx, non_blocking=True)
+                ctx.rbe_set_kvectors(ksets[i % n_k])
+                ctx.rbe_structure_factor(dx, rho_local)
+                dist.all_gather_into_tensor(gathered, rho_local)
+                ctx.rbe_set_rho(gathered.sum(0))
+                ctx.rbe_forces(dx, df, args.with_energy)
+                hf.copy_(df, non_blocking=True)
+                torch.cuda.current_stream().synchronize()
+            for i in range(3):
+                e2e_step(i)
+            sync()
+            e0.record()
+            for i in range(k_e2e):
+                e2e_step(i)
+            e1.record()
+            sync()
+            t = torch.tensor([e0.elapsed_time(e1) / k_e2e], dtype=torch.float64, device="cuda")
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            ms_e2e = float(t.cpu()[0])
+        e2e = {"value": ms_e2e * 1e6 / n_total, "unit": UNIT, "ms_per_step": ms_e2e, "steps": k_e2e,
+               "h2d_bytes_per_step": 16 * n_local + 12 * P, "d2h_bytes_per_step": 16 * n_local}
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    peaks = read_peaks()
+    tr, sfu_rate = roofline_times(n_local, P, info["num_sms"], peaks)
+    t_roof = max(tr.values())
+    pairs = n_local * P
+    sf_ops = SFU_PER_PAIR_PER_KERNEL * pairs
+    traffic = None
+    tpath = os.path.join(ROOT, "profiles", "traffic.json")
+    if os.path.exists(tpath):
+        traffic = json.load(open(tpath)).get(f"sf_kernel:{args.config}")
+    out = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": False, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+        "config": {"workload": base.name, "N_per_gpu": n_local, "N_total": n_total, "P": P, "L": L, "alpha": alpha,
+                   "l2": f"inputs rotate over {n_rot} buffer sets ({32 * n_local * n_rot / 1e6:.0f} MB > 126 MB L2)",
+                   "parallelism": f"atoms sharded over {world} GPU(s), k-set replicated",
+                   "launch": info, "with_energy": bool(args.with_energy)},
+        "kernels_ms": {"structure_factor_call": ms_sf, "forces_call": ms_f,
+                       "note": "region B (CUDA events around each C-ABI call); structure_factor_call = sf_kernel + fin_kernel"},
+        "roofline": {
+            "bound": "alu", "kernel": "sf_kernel (+fin_kernel, timed together)",
+            "achieved": sf_ops / (ms_sf * 1e-3) / 1e9, "peak": sfu_rate / 1e9, "unit": "G sincos-op/s (MUFU)",
+            "frac": (sf_ops / (ms_sf * 1e-3)) / sfu_rate, "traffic": traffic,
+            "peak_source": f"derived: {MUFU_LANES_PER_SM} MUFU lanes/SM/clk x {info['num_sms']} SMs x {peaks['sm_max_mhz']:.0f} MHz",
+        },
+        "roofline_step": {
+            "t_roof_us": t_roof * 1e6, "t_hbm_us": tr["hbm"] * 1e6, "t_fma_us": tr["fma"] * 1e6, "t_sfu_us": tr["sfu"] * 1e6,
+            "frac": t_roof / (ms_step * 1e-3), "ns_per_atom_at_roofline": t_roof * 1e9 / n_local,
+            "hbm_peak_gbs": peaks["hbm_gbs"], "peaks": peaks["src"],
+            "note": "SURVEY.md s8(d): 4 sincos + 13 FMA per (atom,k) pair per step, 48 B per atom",
+        },
+        "clocks": clocks,
+        "gpu_launches": 3 * args.steps,
+        "paper_context": "8.20 ms/step, 1e6 atoms, A100, RBL+RBE nonbonded total, P=100 (PAPER.md P:284); 2.89 ms k-space at 1e5 atoms, P=200 (P:266)",
+    }
+    if e2e:
+        out["e2e"] = e2e
+    if not args.no_cpu_baseline and world == 1:
+        n_s = min(args.cpu_baseline_atoms, base.N)
+        per_step, ns_cpu, cores, _ = time_oracle(args.config, n_s, 1, 0)
+        out["cpu_baseline"] = {"value": ns_cpu, "unit": UNIT, "cores": cores, "kind": "oracle",
+                               "sample": f"first {n_s} atoms of {base.name}, all P={P} wavevectors, oracle.rho + oracle.force, 1 step ({per_step:.1f} s)"}
+    print(json.dumps(out))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

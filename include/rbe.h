@@ -1,0 +1,161 @@
+/*
+ * rbe.h -- C ABI of librbe: the random batch Ewald (RBE) Fourier-space Coulomb force of
+ * arxiv 2407.09315 (RBMD) on one NVIDIA B200 (sm_100a).
+ *
+ * "P:nnn" below = line nnn of the paper text (/root/reference/PAPER.md at build time).
+ *
+ * What the library computes, for N atoms {r_i, q_i} in a cubic periodic box of side L
+ * (V = L^3) and a batch of P integer wavevectors m_l in Z^3 \ {0}, k_l = 2 pi m_l / L
+ * (P:115):
+ *
+ *   rho(k_l) = sum_j q_j exp(i k_l . r_j)                                  Eq. (2.9),
+ *   F_i      = - sum_l w_l (4 pi q_i k_l / (V k_l^2)) Im(exp(-i k_l . r_i) rho(k_l))
+ *                                                                           Eq. (2.12)
+ *   U        = (2 pi / V) sum_l w_l |rho(k_l)|^2 / k_l^2      (2nd term of Eq. (2.8),  P:112)
+ *
+ * with w_l = S / P by default, S = sum_{m != 0} exp(-|k_m|^2 / 4 alpha) the paper's
+ * normalisation constant Q.  The k-set is drawn by the caller (Algorithm 1 step 1,
+ * P:202) and handed over as integers; steps 2-4 of Algorithm 1 run on the GPU.
+ *
+ * Units are Gaussian (Eq. 2.5): charges in e, lengths in A, forces in e^2/A^2, energy
+ * in e^2/A; alpha in A^-2 (erfc(sqrt(alpha) r)).  No Coulomb constant is applied.
+ *
+ * Conventions
+ *  - `d_*` pointers are DEVICE memory owned by the caller, 16-byte aligned, never retained
+ *    after the call returns (except the workspace, retained until rbe_destroy or the next
+ *    rbe_set_workspace).  `h_*` pointers are HOST memory owned by the caller.
+ *  - `stream` is a cudaStream_t passed as void* (0 = the legacy default stream).  Every call
+ *    that takes a stream only enqueues work on it and returns; the exceptions are
+ *    rbe_kspace_energy and rbe_step_host, which synchronise that stream before returning.
+ *  - The library allocates no device memory.  Host memory: the context and a small pinned
+ *    staging ring for the k-vectors, both freed by rbe_destroy.
+ *  - Every function returns an rbe_status (or a value documented below); nothing aborts,
+ *    throws across the boundary, or prints.  rbe_last_error gives the text of the last failure.
+ *  - Results are bitwise reproducible run to run on the same device: no floating-point atomics,
+ *    every reduction in a fixed order.
+ *  - Positions may lie outside [0, L): exp(i k . r) is exactly periodic because k . nL = 2 pi m . n.
+ *    Non-finite positions or charges are undefined behaviour (not checked on the hot path).
+ *  - A context is not thread-safe; use one per host thread / stream.
+ */
+#ifndef RBE_H_
+#define RBE_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct rbe_ctx rbe_ctx; /* opaque; created by rbe_create, freed by rbe_destroy */
+
+typedef enum {
+    RBE_OK = 0,
+    RBE_ERR_INVALID_ARG = 1,  /* null pointer, N < 0, L <= 0, alpha <= 0, P < 1, misaligned pointer */
+    RBE_ERR_BAD_KVECTOR = 2,  /* some m_l == (0,0,0) or |m_l,d| >= 2^15; or a weight is not finite */
+    RBE_ERR_NOT_READY = 3,    /* call order: workspace / k-vectors / structure factor missing */
+    RBE_ERR_WORKSPACE = 4,    /* workspace too small or misaligned */
+    RBE_ERR_CUDA = 5,         /* a CUDA runtime call failed (text in rbe_last_error) */
+    RBE_ERR_NO_DEVICE = 6     /* no usable sm_100 device: there is no CPU fallback */
+} rbe_status;
+
+/* Launch geometry of the three kernels, for benchmarks and profiles (read-only information). */
+typedef struct {
+    int32_t num_sms;
+    int32_t sf_grid_x, sf_grid_y, sf_threads, sf_smem_bytes; /* structure-factor kernel */
+    int32_t sf_k_per_thread, sf_atom_groups, sf_tile_atoms;
+    int32_t fin_grid, fin_threads;                           /* fixed-order finalise kernel */
+    int32_t f_grid, f_threads, f_smem_bytes, f_atoms_per_thread; /* force kernel */
+} rbe_launch_info;
+
+/* Create a context for N atoms (on this GPU), box side L [A], splitting parameter alpha [A^-2]
+ * (Eq. 2.6) and batch size P.  Computes S(L, alpha) in fp64 on the host
+ * (S = H^3 - 1, H = sum_m exp(-pi^2 m^2 / (alpha L^2))).  Makes no CUDA call, so it works
+ * on a machine without a GPU.  N = 0 is allowed (all outputs are then zero / empty).
+ * Errors: RBE_ERR_INVALID_ARG. */
+rbe_status rbe_create(rbe_ctx** out, int64_t N, double L, double alpha, int32_t P);
+
+/* Free the context, its pinned staging buffers and events.  NULL is accepted. */
+rbe_status rbe_destroy(rbe_ctx* ctx);
+
+/* The paper's normalisation constant Q == S for this context's L and alpha. */
+double rbe_normaliser_S(const rbe_ctx* ctx);
+
+/* Bytes of device scratch the context needs (per-CTA fp64 partials, rho, per-k tables).
+ * Queries the current CUDA device on first use.  Returns 0 on error (see rbe_last_error). */
+size_t rbe_workspace_bytes(rbe_ctx* ctx);
+
+/* Hand the context a device buffer of at least rbe_workspace_bytes bytes, 256-byte aligned,
+ * allocated on the current CUDA device.  Caller keeps ownership and must keep it alive.
+ * Errors: RBE_ERR_WORKSPACE, RBE_ERR_NO_DEVICE, RBE_ERR_CUDA. */
+rbe_status rbe_set_workspace(rbe_ctx* ctx, void* d_ws, size_t bytes);
+
+/* Fill *out with the launch geometry chosen for this context (valid after rbe_set_workspace). */
+rbe_status rbe_get_launch_info(const rbe_ctx* ctx, rbe_launch_info* out);
+
+/* Algorithm 1 step 1 hand-over: upload the batch of wavevectors.
+ *   h_m  int32 [P][3], host: integer triples m_l, k_l = 2 pi m_l / L.  Duplicates allowed.
+ *   h_w  double [P], host, or NULL.  NULL: w_l = S / P (Eq. 2.12).  Otherwise w_l = h_w[l];
+ *        with w_l = exp(-k_l^2 / 4 alpha) and the k-set = every grid vector the same kernels
+ *        evaluate the deterministic sum of Eq. (2.11).
+ * The arrays are copied before the call returns (they may be reused immediately); the
+ * host-to-device copy is enqueued on `stream`.  Invalidates any previous structure factor.
+ * Errors: RBE_ERR_BAD_KVECTOR, RBE_ERR_NOT_READY (no workspace), RBE_ERR_CUDA. */
+rbe_status rbe_set_kvectors(rbe_ctx* ctx, const int32_t* h_m, const double* h_w, void* stream);
+
+/* Algorithm 1 steps 2-3, Eq. (2.9): rho(k_l) for l = 0..P-1 over this context's
+ * N atoms, then the per-k force coefficients for rbe_forces.
+ *   d_xyzq  float4 [N] = {x, y, z, q} (AoS), device.
+ *   d_rho   double2 [P] = {Re, Im}, device, or NULL if the caller does not want a copy.
+ * fp32 phases from 32-bit fixed-point fractional coordinates (m . s mod 1 is exact), fp32
+ * sincos, fp32 partial sums over at most 64 atoms, fp64 above that; per-CTA fp64 partials
+ * summed in a fixed order by a second kernel.
+ * Errors: RBE_ERR_NOT_READY, RBE_ERR_INVALID_ARG, RBE_ERR_CUDA. */
+rbe_status rbe_structure_factor(rbe_ctx* ctx, const void* d_xyzq, void* d_rho, void* stream);
+
+/* Replace the context's structure factors by d_rho (double2 [P], device) and rebuild the
+ * force coefficients.  This is the multi-GPU exchange point: each rank computes rho over its
+ * own atoms, the ranks sum the P complex numbers (rank order), and each rank injects the
+ * global sum here before rbe_forces.  Requires rbe_set_kvectors.
+ * Errors: RBE_ERR_NOT_READY, RBE_ERR_INVALID_ARG, RBE_ERR_CUDA. */
+rbe_status rbe_set_rho(rbe_ctx* ctx, const void* d_rho, void* stream);
+
+/* Algorithm 1 step 4, Eq. (2.12): forces on this context's N atoms from the
+ * current k-set and structure factors.
+ *   d_xyzq   float4 [N], device: the same positions the structure factor was computed from.
+ *   d_force  float4 [N], device: {F_x, F_y, F_z, e_i}; e_i = 0 unless with_energy != 0, then
+ *            e_i = (2 pi q_i / V) sum_l w_l Re(exp(-i k_l . r_i) rho(k_l)) / k_l^2 (sum_i e_i = U).
+ * Errors: RBE_ERR_NOT_READY (no structure factor since the last rbe_set_kvectors),
+ *         RBE_ERR_INVALID_ARG, RBE_ERR_CUDA. */
+rbe_status rbe_forces(rbe_ctx* ctx, const void* d_xyzq, void* d_force, int32_t with_energy,
+                      void* stream);
+
+/* U = (2 pi / V) sum_l w_l |rho(k_l)|^2 / k_l^2 for the current k-set and structure factors,
+ * summed in fp64 in a fixed order; written to *h_U (host).  Synchronises `stream`.
+ * Errors: RBE_ERR_NOT_READY, RBE_ERR_INVALID_ARG, RBE_ERR_CUDA. */
+rbe_status rbe_kspace_energy(rbe_ctx* ctx, double* h_U, void* stream);
+
+/* One whole step from HOST buffers (the end-to-end path): copies h_xyzq (float [N][4]) to the
+ * device, uploads the k-set, runs rbe_structure_factor and rbe_forces, copies the forces back
+ * into h_force (float [N][4]) and, if h_U != NULL, the energy into *h_U; synchronises `stream`.
+ * d_scratch: caller-owned device buffer of at least 32 * N bytes (positions + forces).
+ * Pinned host buffers make the copies asynchronous; pageable ones work but are slower.
+ * Errors: as the calls it is made of, plus RBE_ERR_WORKSPACE if d_scratch is too small. */
+rbe_status rbe_step_host(rbe_ctx* ctx, const float* h_xyzq, const int32_t* h_m, const double* h_w,
+                         float* h_force, int32_t with_energy, double* h_U, void* d_scratch,
+                         size_t scratch_bytes, void* stream);
+
+/* Text of the last error on this context (owned by the context; "" if none).  For ctx == NULL
+ * returns a static string. */
+const char* rbe_last_error(const rbe_ctx* ctx);
+
+/* Static name of a status code. */
+const char* rbe_status_string(rbe_status s);
+
+/* Library version: major * 10000 + minor * 100 + patch. */
+int32_t rbe_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* RBE_H_ */

@@ -1,0 +1,380 @@
+// rbe_api.cu -- the C ABI of librbe (include/rbe.h): context, workspace carving, k-vector
+// upload and kernel launches.  No torch types, no device allocation, no CPU fallback.
+#include "rbe.h"
+
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+
+#include "rbe_kernels.cuh"
+
+namespace {
+
+constexpr int NSTAGE = 8;  // pinned staging slots for k-vector uploads in flight
+
+inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+
+}  // namespace
+
+struct rbe_ctx {
+    int64_t N = 0;
+    double L = 0, alpha = 0, S = 0;
+    int32_t P = 0;
+
+    // device / launch geometry (filled by init_device)
+    bool dev_ready = false;
+    int device = -1;
+    rbe_launch_info li{};
+    int sf_gs = 0, sf_ng = 0, sf_ai = 0;
+    size_t ws_bytes = 0;
+    size_t off_kvec = 0, off_w = 0, off_part = 0, off_rho = 0, off_ka = 0, off_kb = 0, off_uk = 0, off_U = 0;
+
+    // workspace
+    unsigned char* ws = nullptr;
+    bool have_k = false, have_w = false, have_rho = false;
+
+    // pinned staging ring
+    void* stage[NSTAGE] = {};
+    cudaEvent_t stage_ev[NSTAGE] = {};
+    bool stage_used[NSTAGE] = {};
+    size_t stage_bytes = 0;
+    int stage_next = 0;
+    double* h_U_pinned = nullptr;
+
+    std::string err;
+};
+
+namespace {
+
+rbe_status fail(rbe_ctx* c, rbe_status s, const std::string& msg) {
+    if (c) c->err = msg;
+    return s;
+}
+
+rbe_status cuda_fail(rbe_ctx* c, const char* what, cudaError_t e) {
+    return fail(c, RBE_ERR_CUDA, std::string(what) + ": " + cudaGetErrorString(e));
+}
+
+#define RBE_CUDA(ctx, call)                                   \
+    do {                                                      \
+        cudaError_t e__ = (call);                             \
+        if (e__ != cudaSuccess) return cuda_fail(ctx, #call, e__); \
+    } while (0)
+
+double normaliser_S(double L, double alpha) {
+    // S = H^3 - 1, H = sum_{m in Z} exp(-pi^2 m^2 / (alpha L^2))   (k = 2 pi m / L P:115)
+    const double c = rbe::PI_D * rbe::PI_D / (alpha * L * L);
+    double H = 1.0;
+    for (int64_t m = 1; m < (int64_t)1 << 40; ++m) {
+        const double t = std::exp(-c * (double)m * (double)m);
+        if (!(t > 1e-300)) break;
+        H += 2.0 * t;
+    }
+    return H * H * H - 1.0;
+}
+
+// Choose the launch geometry for this context on the current device.
+rbe_status init_device(rbe_ctx* c) {
+    if (c->dev_ready) return RBE_OK;
+    int ndev = 0;
+    cudaError_t e = cudaGetDeviceCount(&ndev);
+    if (e != cudaSuccess || ndev == 0) {
+        cudaGetLastError();
+        return fail(c, RBE_ERR_NO_DEVICE, "no CUDA device (librbe has no CPU fallback)");
+    }
+    RBE_CUDA(c, cudaGetDevice(&c->device));
+    cudaDeviceProp prop;
+    RBE_CUDA(c, cudaGetDeviceProperties(&prop, c->device));
+    if (prop.major != 10)
+        return fail(c, RBE_ERR_NO_DEVICE, "librbe is built for sm_100a only; device is sm_" +
+                                              std::to_string(prop.major) + std::to_string(prop.minor));
+    rbe_launch_info& li = c->li;
+    li.num_sms = prop.multiProcessorCount;
+
+    // ---- SF kernel: a thread owns SF_KPT wavevectors; gs threads cover one k-chunk.
+    const int slots = (c->P + rbe::SF_KPT - 1) / rbe::SF_KPT;
+    int gy = (slots + rbe::SF_TMAX - 1) / rbe::SF_TMAX;
+    int gs = (slots + gy - 1) / gy;
+    int ng = rbe::SF_TMAX / gs;
+    if (ng < 1) ng = 1;
+    int threads = (int)align_up((size_t)gs * ng, 32);
+    int ai = rbe::SF_AI;
+    if (ng * ai > 2 * threads) ai = (2 * threads) / ng;
+    if (ai < 1) ai = 1;
+    int gx = li.num_sms / gy;
+    if (gx < 1) gx = 1;
+    // never more CTAs than groups of atoms to feed them
+    const int64_t max_gx = c->N > 0 ? (c->N + ng - 1) / ng : 1;
+    if ((int64_t)gx > max_gx) gx = (int)max_gx;
+    c->sf_gs = gs; c->sf_ng = ng; c->sf_ai = ai;
+    li.sf_grid_x = gx; li.sf_grid_y = gy; li.sf_threads = threads;
+    li.sf_k_per_thread = rbe::SF_KPT; li.sf_atom_groups = ng; li.sf_tile_atoms = ng * ai;
+    size_t sm_tiles = (size_t)2 * ng * ai * sizeof(uint4);
+    size_t sm_red = (size_t)ng * gs * rbe::SF_KPT * sizeof(double2);
+    li.sf_smem_bytes = (int32_t)(sm_tiles > sm_red ? sm_tiles : sm_red);
+
+    li.fin_grid = (c->P + rbe::FIN_KB - 1) / rbe::FIN_KB;
+    li.fin_threads = rbe::FIN_KB * rbe::FIN_SL;
+
+    // ---- F kernel: warps take balanced runs of 32-atom units; one wave of CTAs.
+    li.f_threads = rbe::F_THREADS;
+    li.f_atoms_per_thread = 4;
+    const int nk = c->P < rbe::F_KCHUNK ? c->P : rbe::F_KCHUNK;
+    li.f_smem_bytes = (int32_t)((size_t)nk * (sizeof(int4) + sizeof(float4)));
+    RBE_CUDA(c, cudaFuncSetAttribute(rbe::f_kernel<4, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, li.f_smem_bytes));
+    RBE_CUDA(c, cudaFuncSetAttribute(rbe::f_kernel<4, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, li.f_smem_bytes));
+    int occ0 = 0, occ1 = 0;  // resident CTAs per SM: the grid is exactly one wave
+    RBE_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ0, rbe::f_kernel<4, false>, rbe::F_THREADS, li.f_smem_bytes));
+    RBE_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ1, rbe::f_kernel<4, true>, rbe::F_THREADS, li.f_smem_bytes));
+    int f_ctas_per_sm = occ0 < occ1 ? occ0 : occ1;
+    if (f_ctas_per_sm < 1) f_ctas_per_sm = 1;
+    if (f_ctas_per_sm > 4) f_ctas_per_sm = 4;
+    int64_t f_grid = (int64_t)li.num_sms * f_ctas_per_sm;
+    const int64_t units = (c->N + 31) / 32;
+    const int64_t max_f = units > 0 ? (units + (rbe::F_THREADS / 32) - 1) / (rbe::F_THREADS / 32) : 1;
+    if (f_grid > max_f) f_grid = max_f;
+    li.f_grid = (int32_t)f_grid;
+
+    RBE_CUDA(c, cudaFuncSetAttribute(rbe::sf_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, li.sf_smem_bytes));
+
+    // ---- workspace layout
+    size_t off = 0;
+    const size_t P = (size_t)c->P;
+    c->off_kvec = off; off = align_up(off + P * sizeof(int4), 256);
+    c->off_w = off;    off = align_up(off + P * sizeof(double), 256);
+    c->off_part = off; off = align_up(off + (size_t)gx * P * sizeof(double2), 256);
+    c->off_rho = off;  off = align_up(off + P * sizeof(double2), 256);
+    c->off_ka = off;   off = align_up(off + P * sizeof(int4), 256);
+    c->off_kb = off;   off = align_up(off + P * sizeof(float4), 256);
+    c->off_uk = off;   off = align_up(off + P * sizeof(double), 256);
+    c->off_U = off;    off = align_up(off + sizeof(double), 256);
+    c->ws_bytes = off;
+
+    c->stage_bytes = P * (sizeof(int4) + sizeof(double));
+    c->dev_ready = true;
+    return RBE_OK;
+}
+
+template <typename T>
+T* ws_ptr(rbe_ctx* c, size_t off) { return reinterpret_cast<T*>(c->ws + off); }
+
+rbe_status launch_fin(rbe_ctx* c, const double2* part, int nrows, double2* rho_user, cudaStream_t st) {
+    rbe::FinParams fp;
+    fp.part = part; fp.nrows = nrows; fp.P = c->P;
+    fp.kvec = ws_ptr<int4>(c, c->off_kvec);
+    fp.w = c->have_w ? ws_ptr<double>(c, c->off_w) : nullptr;
+    fp.w_uniform = c->S / (double)c->P;
+    fp.L = c->L;
+    fp.rho = ws_ptr<double2>(c, c->off_rho);
+    fp.rho_user = rho_user;
+    fp.ka = ws_ptr<int4>(c, c->off_ka);
+    fp.kb = ws_ptr<float4>(c, c->off_kb);
+    fp.uk = ws_ptr<double>(c, c->off_uk);
+    rbe::fin_kernel<<<c->li.fin_grid, c->li.fin_threads, 0, st>>>(fp);
+    RBE_CUDA(c, cudaGetLastError());
+    c->have_rho = true;
+    return RBE_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+rbe_status rbe_create(rbe_ctx** out, int64_t N, double L, double alpha, int32_t P) {
+    if (!out) return RBE_ERR_INVALID_ARG;
+    *out = nullptr;
+    if (N < 0 || !(L > 0.0) || !(alpha > 0.0) || P < 1 || !std::isfinite(L) || !std::isfinite(alpha) ||
+        P > (1 << 20))
+        return RBE_ERR_INVALID_ARG;
+    rbe_ctx* c = new (std::nothrow) rbe_ctx();
+    if (!c) return RBE_ERR_INVALID_ARG;
+    c->N = N; c->L = L; c->alpha = alpha; c->P = P;
+    c->S = normaliser_S(L, alpha);
+    *out = c;
+    return RBE_OK;
+}
+
+rbe_status rbe_destroy(rbe_ctx* c) {
+    if (!c) return RBE_OK;
+    for (int i = 0; i < NSTAGE; ++i) {
+        if (c->stage_ev[i]) cudaEventDestroy(c->stage_ev[i]);
+        if (c->stage[i]) cudaFreeHost(c->stage[i]);
+    }
+    if (c->h_U_pinned) cudaFreeHost(c->h_U_pinned);
+    delete c;
+    return RBE_OK;
+}
+
+double rbe_normaliser_S(const rbe_ctx* c) { return c ? c->S : 0.0; }
+
+size_t rbe_workspace_bytes(rbe_ctx* c) {
+    if (!c) return 0;
+    if (init_device(c) != RBE_OK) return 0;
+    return c->ws_bytes;
+}
+
+rbe_status rbe_set_workspace(rbe_ctx* c, void* d_ws, size_t bytes) {
+    if (!c) return RBE_ERR_INVALID_ARG;
+    rbe_status s = init_device(c);
+    if (s != RBE_OK) return s;
+    if (!d_ws || bytes < c->ws_bytes || (reinterpret_cast<uintptr_t>(d_ws) & 255u))
+        return fail(c, RBE_ERR_WORKSPACE, "workspace must be non-null, 256-byte aligned and >= rbe_workspace_bytes");
+    c->ws = static_cast<unsigned char*>(d_ws);
+    c->have_k = c->have_w = c->have_rho = false;
+    return RBE_OK;
+}
+
+rbe_status rbe_get_launch_info(const rbe_ctx* c, rbe_launch_info* out) {
+    if (!c || !out) return RBE_ERR_INVALID_ARG;
+    if (!c->dev_ready) return RBE_ERR_NOT_READY;
+    *out = c->li;
+    return RBE_OK;
+}
+
+rbe_status rbe_set_kvectors(rbe_ctx* c, const int32_t* h_m, const double* h_w, void* stream) {
+    if (!c || !h_m) return fail(c, RBE_ERR_INVALID_ARG, "rbe_set_kvectors: null argument");
+    // validate first: independent of the device state
+    for (int32_t l = 0; l < c->P; ++l) {
+        const int32_t a = h_m[3 * l], b = h_m[3 * l + 1], d = h_m[3 * l + 2];
+        if ((a == 0 && b == 0 && d == 0) || a <= -32768 || a >= 32768 || b <= -32768 || b >= 32768 ||
+            d <= -32768 || d >= 32768)
+            return fail(c, RBE_ERR_BAD_KVECTOR, "k-vector " + std::to_string(l) + " is zero or out of range (|m_d| < 2^15)");
+        if (h_w && !std::isfinite(h_w[l]))
+            return fail(c, RBE_ERR_BAD_KVECTOR, "weight " + std::to_string(l) + " is not finite");
+    }
+    if (!c->ws) return fail(c, RBE_ERR_NOT_READY, "rbe_set_kvectors before rbe_set_workspace");
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    const int slot = c->stage_next;
+    c->stage_next = (slot + 1) % NSTAGE;
+    if (!c->stage[slot]) {
+        RBE_CUDA(c, cudaMallocHost(&c->stage[slot], c->stage_bytes));
+        RBE_CUDA(c, cudaEventCreateWithFlags(&c->stage_ev[slot], cudaEventDisableTiming));
+    } else if (c->stage_used[slot]) {
+        RBE_CUDA(c, cudaEventSynchronize(c->stage_ev[slot]));
+    }
+    int4* hm = static_cast<int4*>(c->stage[slot]);
+    for (int32_t l = 0; l < c->P; ++l) hm[l] = make_int4(h_m[3 * l], h_m[3 * l + 1], h_m[3 * l + 2], 0);
+    size_t bytes = (size_t)c->P * sizeof(int4);
+    RBE_CUDA(c, cudaMemcpyAsync(c->ws + c->off_kvec, hm, bytes, cudaMemcpyHostToDevice, st));
+    if (h_w) {
+        double* hw = reinterpret_cast<double*>(hm + c->P);
+        std::memcpy(hw, h_w, (size_t)c->P * sizeof(double));
+        RBE_CUDA(c, cudaMemcpyAsync(c->ws + c->off_w, hw, (size_t)c->P * sizeof(double), cudaMemcpyHostToDevice, st));
+    }
+    RBE_CUDA(c, cudaEventRecord(c->stage_ev[slot], st));
+    c->stage_used[slot] = true;
+    c->have_k = true;
+    c->have_w = (h_w != nullptr);
+    c->have_rho = false;
+    return RBE_OK;
+}
+
+rbe_status rbe_structure_factor(rbe_ctx* c, const void* d_xyzq, void* d_rho, void* stream) {
+    if (!c) return RBE_ERR_INVALID_ARG;
+    if (!c->ws || !c->have_k) return fail(c, RBE_ERR_NOT_READY, "rbe_structure_factor needs a workspace and k-vectors");
+    if ((c->N > 0 && !d_xyzq) || (reinterpret_cast<uintptr_t>(d_xyzq) & 15u) || (reinterpret_cast<uintptr_t>(d_rho) & 15u))
+        return fail(c, RBE_ERR_INVALID_ARG, "rbe_structure_factor: null or misaligned pointer");
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    rbe::SfParams sp;
+    sp.xyzq = static_cast<const float4*>(d_xyzq);
+    sp.N = c->N;
+    sp.kvec = ws_ptr<int4>(c, c->off_kvec);
+    sp.part = ws_ptr<double2>(c, c->off_part);
+    sp.two32_over_L = rbe::TWO32 / c->L;
+    sp.P = c->P; sp.gs = c->sf_gs; sp.ng = c->sf_ng; sp.ai = c->sf_ai;
+    dim3 grid(c->li.sf_grid_x, c->li.sf_grid_y);
+    rbe::sf_kernel<<<grid, c->li.sf_threads, c->li.sf_smem_bytes, st>>>(sp);
+    RBE_CUDA(c, cudaGetLastError());
+    return launch_fin(c, sp.part, c->li.sf_grid_x, static_cast<double2*>(d_rho), st);
+}
+
+rbe_status rbe_set_rho(rbe_ctx* c, const void* d_rho, void* stream) {
+    if (!c) return RBE_ERR_INVALID_ARG;
+    if (!c->ws || !c->have_k) return fail(c, RBE_ERR_NOT_READY, "rbe_set_rho needs a workspace and k-vectors");
+    if (!d_rho || (reinterpret_cast<uintptr_t>(d_rho) & 15u))
+        return fail(c, RBE_ERR_INVALID_ARG, "rbe_set_rho: null or misaligned pointer");
+    return launch_fin(c, static_cast<const double2*>(d_rho), 1, nullptr, static_cast<cudaStream_t>(stream));
+}
+
+rbe_status rbe_forces(rbe_ctx* c, const void* d_xyzq, void* d_force, int32_t with_energy, void* stream) {
+    if (!c) return RBE_ERR_INVALID_ARG;
+    if (!c->ws || !c->have_k || !c->have_rho)
+        return fail(c, RBE_ERR_NOT_READY, "rbe_forces needs rbe_structure_factor (or rbe_set_rho) after rbe_set_kvectors");
+    if (c->N == 0) return RBE_OK;
+    if (!d_xyzq || !d_force || (reinterpret_cast<uintptr_t>(d_xyzq) & 15u) || (reinterpret_cast<uintptr_t>(d_force) & 15u))
+        return fail(c, RBE_ERR_INVALID_ARG, "rbe_forces: null or misaligned pointer");
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    rbe::FParams fp;
+    fp.xyzq = static_cast<const float4*>(d_xyzq);
+    fp.force = static_cast<float4*>(d_force);
+    fp.N = c->N;
+    fp.ka = ws_ptr<int4>(c, c->off_ka);
+    fp.kb = ws_ptr<float4>(c, c->off_kb);
+    fp.two32_over_L = rbe::TWO32 / c->L;
+    fp.P = c->P;
+    if (with_energy)
+        rbe::f_kernel<4, true><<<c->li.f_grid, c->li.f_threads, c->li.f_smem_bytes, st>>>(fp);
+    else
+        rbe::f_kernel<4, false><<<c->li.f_grid, c->li.f_threads, c->li.f_smem_bytes, st>>>(fp);
+    RBE_CUDA(c, cudaGetLastError());
+    return RBE_OK;
+}
+
+rbe_status rbe_kspace_energy(rbe_ctx* c, double* h_U, void* stream) {
+    if (!c || !h_U) return fail(c, RBE_ERR_INVALID_ARG, "rbe_kspace_energy: null argument");
+    if (!c->ws || !c->have_k || !c->have_rho) return fail(c, RBE_ERR_NOT_READY, "rbe_kspace_energy needs a structure factor");
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    if (!c->h_U_pinned) RBE_CUDA(c, cudaMallocHost(reinterpret_cast<void**>(&c->h_U_pinned), sizeof(double)));
+    rbe::energy_kernel<<<1, 256, 0, st>>>(ws_ptr<double>(c, c->off_uk), c->P, ws_ptr<double>(c, c->off_U));
+    RBE_CUDA(c, cudaGetLastError());
+    RBE_CUDA(c, cudaMemcpyAsync(c->h_U_pinned, c->ws + c->off_U, sizeof(double), cudaMemcpyDeviceToHost, st));
+    RBE_CUDA(c, cudaStreamSynchronize(st));
+    *h_U = *c->h_U_pinned;
+    return RBE_OK;
+}
+
+rbe_status rbe_step_host(rbe_ctx* c, const float* h_xyzq, const int32_t* h_m, const double* h_w, float* h_force,
+                         int32_t with_energy, double* h_U, void* d_scratch, size_t scratch_bytes, void* stream) {
+    if (!c) return RBE_ERR_INVALID_ARG;
+    if ((c->N > 0 && (!h_xyzq || !h_force)) || !h_m) return fail(c, RBE_ERR_INVALID_ARG, "rbe_step_host: null argument");
+    const size_t nb = (size_t)c->N * sizeof(float4);
+    if (c->N > 0 && (!d_scratch || scratch_bytes < 2 * nb || (reinterpret_cast<uintptr_t>(d_scratch) & 255u)))
+        return fail(c, RBE_ERR_WORKSPACE, "rbe_step_host: d_scratch must hold 32*N bytes, 256-byte aligned");
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    unsigned char* d_x = static_cast<unsigned char*>(d_scratch);
+    unsigned char* d_f = d_x + align_up(nb, 256);
+    if (c->N > 0 && scratch_bytes < align_up(nb, 256) + nb)
+        return fail(c, RBE_ERR_WORKSPACE, "rbe_step_host: d_scratch too small");
+    rbe_status s = rbe_set_kvectors(c, h_m, h_w, stream);
+    if (s != RBE_OK) return s;
+    if (c->N > 0) RBE_CUDA(c, cudaMemcpyAsync(d_x, h_xyzq, nb, cudaMemcpyHostToDevice, st));
+    s = rbe_structure_factor(c, d_x, nullptr, stream);
+    if (s != RBE_OK) return s;
+    s = rbe_forces(c, d_x, d_f, with_energy, stream);
+    if (s != RBE_OK) return s;
+    if (c->N > 0) RBE_CUDA(c, cudaMemcpyAsync(h_force, d_f, nb, cudaMemcpyDeviceToHost, st));
+    if (h_U) return rbe_kspace_energy(c, h_U, stream);
+    RBE_CUDA(c, cudaStreamSynchronize(st));
+    return RBE_OK;
+}
+
+const char* rbe_last_error(const rbe_ctx* c) { return c ? c->err.c_str() : "null context"; }
+
+const char* rbe_status_string(rbe_status s) {
+    switch (s) {
+        case RBE_OK: return "RBE_OK";
+        case RBE_ERR_INVALID_ARG: return "RBE_ERR_INVALID_ARG";
+        case RBE_ERR_BAD_KVECTOR: return "RBE_ERR_BAD_KVECTOR";
+        case RBE_ERR_NOT_READY: return "RBE_ERR_NOT_READY";
+        case RBE_ERR_WORKSPACE: return "RBE_ERR_WORKSPACE";
+        case RBE_ERR_CUDA: return "RBE_ERR_CUDA";
+        case RBE_ERR_NO_DEVICE: return "RBE_ERR_NO_DEVICE";
+    }
+    return "RBE_ERR_UNKNOWN";
+}
+
+int32_t rbe_version(void) { return 100; }
+
+}  // extern "C"

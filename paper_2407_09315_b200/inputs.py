@@ -139,13 +139,13 @@ def sample_kset(L: float, alpha: float, P: int, seed: int, step: int = 0) -> np.
     cdf[-1] = 1.0
     out = np.empty((P, 3), dtype=np.int32)
     filled = 0
+    p_accept = 1.0 - float(p[ms == 0][0]) ** 3
     while filled < P:
-        n = P - filled
+        n = int(min(4_000_000, max(16, (P - filled) / max(p_accept, 1e-12) * 1.1)))
         u = rng.random((n, 3))
         idx = np.minimum(np.searchsorted(cdf, u, side="right"), len(ms) - 1)
         cand = ms[idx]
-        keep = np.any(cand != 0, axis=1)
-        cand = cand[keep]
+        cand = cand[np.any(cand != 0, axis=1)][: P - filled]
         out[filled:filled + cand.shape[0]] = cand
         filled += cand.shape[0]
     return out

@@ -1,0 +1,210 @@
+"""ctypes binding of librbe (include/rbe.h): argument marshalling only.
+
+Same names as the C ABI.  torch supplies device memory and the CUDA stream; every step of
+the path runs in the library's own kernels.  There is no CPU fallback: if librbe.so is
+missing, or there is no sm_100 device, the calls raise.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+SO_PATH = os.path.join(HERE, "librbe.so")
+
+RBE_OK = 0
+STATUS_NAMES = {
+    0: "RBE_OK", 1: "RBE_ERR_INVALID_ARG", 2: "RBE_ERR_BAD_KVECTOR", 3: "RBE_ERR_NOT_READY",
+    4: "RBE_ERR_WORKSPACE", 5: "RBE_ERR_CUDA", 6: "RBE_ERR_NO_DEVICE",
+}
+
+
+class RbeError(RuntimeError):
+    def __init__(self, status: int, msg: str):
+        super().__init__(f"{STATUS_NAMES.get(status, status)}: {msg}")
+        self.status = status
+
+
+class LaunchInfo(ctypes.Structure):
+    _fields_ = [(n, ctypes.c_int32) for n in (
+        "num_sms", "sf_grid_x", "sf_grid_y", "sf_threads", "sf_smem_bytes", "sf_k_per_thread",
+        "sf_atom_groups", "sf_tile_atoms", "fin_grid", "fin_threads", "f_grid", "f_threads",
+        "f_smem_bytes", "f_atoms_per_thread")]
+
+    def as_dict(self):
+        return {n: int(getattr(self, n)) for n, _ in self._fields_}
+
+
+_lib = None
+
+
+def lib():
+    """Load librbe.so (built in-tree by build.py).  Fails loudly if it is not there."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(SO_PATH):
+            raise ImportError(
+                f"{SO_PATH} not found: build it with `python -m paper_2407_09315_b200.build` "
+                "(or __graft_entry__.build()); there is no fallback path")
+        L = ctypes.CDLL(SO_PATH)
+        vp, i32, i64, dbl, sz = ctypes.c_void_p, ctypes.c_int32, ctypes.c_int64, ctypes.c_double, ctypes.c_size_t
+        L.rbe_create.restype = ctypes.c_int
+        L.rbe_create.argtypes = [ctypes.POINTER(vp), i64, dbl, dbl, i32]
+        L.rbe_destroy.restype = ctypes.c_int
+        L.rbe_destroy.argtypes = [vp]
+        L.rbe_normaliser_S.restype = dbl
+        L.rbe_normaliser_S.argtypes = [vp]
+        L.rbe_workspace_bytes.restype = sz
+        L.rbe_workspace_bytes.argtypes = [vp]
+        L.rbe_set_workspace.restype = ctypes.c_int
+        L.rbe_set_workspace.argtypes = [vp, vp, sz]
+        L.rbe_get_launch_info.restype = ctypes.c_int
+        L.rbe_get_launch_info.argtypes = [vp, ctypes.POINTER(LaunchInfo)]
+        L.rbe_set_kvectors.restype = ctypes.c_int
+        L.rbe_set_kvectors.argtypes = [vp, vp, vp, vp]
+        L.rbe_structure_factor.restype = ctypes.c_int
+        L.rbe_structure_factor.argtypes = [vp, vp, vp, vp]
+        L.rbe_set_rho.restype = ctypes.c_int
+        L.rbe_set_rho.argtypes = [vp, vp, vp]
+        L.rbe_forces.restype = ctypes.c_int
+        L.rbe_forces.argtypes = [vp, vp, vp, i32, vp]
+        L.rbe_kspace_energy.restype = ctypes.c_int
+        L.rbe_kspace_energy.argtypes = [vp, ctypes.POINTER(dbl), vp]
+        L.rbe_step_host.restype = ctypes.c_int
+        L.rbe_step_host.argtypes = [vp, vp, vp, vp, vp, i32, ctypes.POINTER(dbl), vp, sz, vp]
+        L.rbe_last_error.restype = ctypes.c_char_p
+        L.rbe_last_error.argtypes = [vp]
+        L.rbe_status_string.restype = ctypes.c_char_p
+        L.rbe_status_string.argtypes = [ctypes.c_int]
+        L.rbe_version.restype = i32
+        _lib = L
+    return _lib
+
+
+def _stream_ptr(stream):
+    if stream is None:
+        import torch
+        stream = torch.cuda.current_stream()
+    return ctypes.c_void_p(int(getattr(stream, "cuda_stream", stream)))
+
+
+def _np_ptr(a):
+    return None if a is None else ctypes.c_void_p(a.ctypes.data)
+
+
+class Rbe:
+    """One RBE context: N atoms on the current device, box L, alpha, batch size P."""
+
+    def __init__(self, N: int, L: float, alpha: float, P: int, *, allocate: bool = True):
+        self._h = ctypes.c_void_p()
+        self.N, self.L, self.alpha, self.P = int(N), float(L), float(alpha), int(P)
+        st = lib().rbe_create(ctypes.byref(self._h), self.N, self.L, self.alpha, self.P)
+        if st != RBE_OK:
+            self._h = ctypes.c_void_p()
+            raise RbeError(st, "rbe_create: invalid argument")
+        self._ws = None
+        self._scratch = None
+        if allocate:
+            self.rbe_set_workspace()
+
+    # ---- plumbing
+    def _check(self, st):
+        if st != RBE_OK:
+            raise RbeError(st, lib().rbe_last_error(self._h).decode())
+
+    def close(self):
+        if getattr(self, "_h", None) is not None and self._h.value:
+            lib().rbe_destroy(self._h)
+            self._h = ctypes.c_void_p()
+
+    __del__ = close
+
+    # ---- the C ABI, same names
+    def rbe_normaliser_S(self) -> float:
+        return float(lib().rbe_normaliser_S(self._h))
+
+    def rbe_workspace_bytes(self) -> int:
+        n = int(lib().rbe_workspace_bytes(self._h))
+        if n == 0:
+            raise RbeError(6, lib().rbe_last_error(self._h).decode())
+        return n
+
+    def rbe_set_workspace(self, ws=None):
+        import torch
+        if ws is None:
+            ws = torch.empty(self.rbe_workspace_bytes(), dtype=torch.uint8, device="cuda")
+        self._check(lib().rbe_set_workspace(self._h, ctypes.c_void_p(ws.data_ptr()), ws.numel() * ws.element_size()))
+        self._ws = ws  # keep alive
+
+    def rbe_get_launch_info(self) -> dict:
+        li = LaunchInfo()
+        self._check(lib().rbe_get_launch_info(self._h, ctypes.byref(li)))
+        return li.as_dict()
+
+    def rbe_set_kvectors(self, m, w=None, stream=None):
+        """m: numpy int32 [P,3] (host); w: numpy float64 [P] (host) or None."""
+        import numpy as np
+        mm = np.ascontiguousarray(m, dtype=np.int32)
+        assert mm.shape == (self.P, 3), mm.shape
+        ww = None if w is None else np.ascontiguousarray(w, dtype=np.float64)
+        assert ww is None or ww.shape == (self.P,)
+        self._check(lib().rbe_set_kvectors(self._h, _np_ptr(mm), _np_ptr(ww), _stream_ptr(stream)))
+
+    def rbe_structure_factor(self, xyzq, rho=None, stream=None):
+        """xyzq: cuda float32 [N,4]; rho: cuda float64 [P,2] or None."""
+        _check_tensor(xyzq, (self.N, 4), "float32")
+        if rho is not None:
+            _check_tensor(rho, (self.P, 2), "float64")
+        self._check(lib().rbe_structure_factor(
+            self._h, ctypes.c_void_p(xyzq.data_ptr()),
+            None if rho is None else ctypes.c_void_p(rho.data_ptr()), _stream_ptr(stream)))
+
+    def rbe_set_rho(self, rho, stream=None):
+        _check_tensor(rho, (self.P, 2), "float64")
+        self._check(lib().rbe_set_rho(self._h, ctypes.c_void_p(rho.data_ptr()), _stream_ptr(stream)))
+
+    def rbe_forces(self, xyzq, force, with_energy: bool = False, stream=None):
+        """xyzq, force: cuda float32 [N,4]."""
+        _check_tensor(xyzq, (self.N, 4), "float32")
+        _check_tensor(force, (self.N, 4), "float32")
+        self._check(lib().rbe_forces(self._h, ctypes.c_void_p(xyzq.data_ptr()),
+                                     ctypes.c_void_p(force.data_ptr()), int(bool(with_energy)),
+                                     _stream_ptr(stream)))
+
+    def rbe_kspace_energy(self, stream=None) -> float:
+        u = ctypes.c_double(0.0)
+        self._check(lib().rbe_kspace_energy(self._h, ctypes.byref(u), _stream_ptr(stream)))
+        return float(u.value)
+
+    def rbe_step_host(self, h_xyzq, m, h_force, w=None, with_energy=False, want_energy=False, stream=None):
+        """End-to-end step from HOST buffers: h_xyzq / h_force are CPU float32 [N,4] torch tensors
+        (pinned for asynchronous copies) or numpy arrays; m numpy int32 [P,3]."""
+        import numpy as np
+        import torch
+        if self._scratch is None:
+            self._scratch = torch.empty(max(1, 32 * self.N + 512), dtype=torch.uint8, device="cuda")
+        mm = np.ascontiguousarray(m, dtype=np.int32)
+        assert mm.shape == (self.P, 3)
+        ww = None if w is None else np.ascontiguousarray(w, dtype=np.float64)
+        u = ctypes.c_double(0.0)
+        self._check(lib().rbe_step_host(
+            self._h, ctypes.c_void_p(_host_ptr(h_xyzq, self.N)), _np_ptr(mm), _np_ptr(ww),
+            ctypes.c_void_p(_host_ptr(h_force, self.N)), int(bool(with_energy)),
+            ctypes.byref(u) if want_energy else None,
+            ctypes.c_void_p(self._scratch.data_ptr()), self._scratch.numel(), _stream_ptr(stream)))
+        return float(u.value) if want_energy else None
+
+
+def _check_tensor(t, shape, dtype):
+    import torch
+    if not (t.is_cuda and t.is_contiguous() and tuple(t.shape) == tuple(shape) and t.dtype == getattr(torch, dtype)):
+        raise ValueError(f"expected contiguous cuda {dtype} tensor of shape {shape}, got {t.dtype} {tuple(t.shape)} on {t.device}")
+
+
+def _host_ptr(a, N):
+    import numpy as np
+    if isinstance(a, np.ndarray):
+        assert a.dtype == np.float32 and a.flags["C_CONTIGUOUS"] and a.shape == (N, 4)
+        return a.ctypes.data
+    assert (not a.is_cuda) and a.is_contiguous() and tuple(a.shape) == (N, 4)
+    return a.data_ptr()

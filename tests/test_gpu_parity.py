@@ -1,0 +1,241 @@
+"""Parity of the CUDA path (through the C ABI) against the fp64 oracle, element by element on
+the same seeded inputs and the same k-set.  Tolerances are BASELINE.json north_star's
+(reading Q15):
+
+  rho : max_l |rho_gpu,l - rho_or,l|            <= 1e-6 * sum_j |q_j|
+  F   : ||F_gpu - F_or||_2 / ||F_or||_2          <= 2e-5   (all 3N components, or the sample)
+  U   : |U_gpu - U_or| / |U_or|                  <= 1e-5
+"""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+from paper_2407_09315_b200 import inputs, rbe
+
+pytestmark = pytest.mark.gpu
+
+RHO_TOL, F_TOL, U_TOL = 1e-6, 2e-5, 1e-5
+
+
+def gpu_step(atoms, L, alpha, m, w=None, with_energy=False):
+    N, P = atoms.shape[0], m.shape[0]
+    ctx = rbe.Rbe(N, L, alpha, P)
+    xyzq = torch.from_numpy(atoms).cuda()
+    rho = torch.empty((P, 2), dtype=torch.float64, device="cuda")
+    force = torch.full((N, 4), float("nan"), dtype=torch.float32, device="cuda")
+    ctx.rbe_set_kvectors(m, w)
+    ctx.rbe_structure_factor(xyzq, rho)
+    ctx.rbe_forces(xyzq, force, with_energy)
+    U = ctx.rbe_kspace_energy()
+    torch.cuda.synchronize()
+    return ctx, rho.cpu().numpy(), force.cpu().numpy(), U
+
+
+def check(atoms, L, alpha, m, w=None, with_energy=False, sel=None, f_tol=F_TOL):
+    ctx, rho_g, F_g, U_g = gpu_step(atoms, L, alpha, m, w, with_energy)
+    S = oracle.S(L, alpha)
+    assert abs(ctx.rbe_normaliser_S() - S) <= 1e-13 * S
+    rho_o = oracle.rho(atoms, L, m)
+    qsum = np.abs(atoms[:, 3].astype(np.float64)).sum()
+    err_rho = np.abs(rho_g - rho_o).max() if len(m) else 0.0
+    assert err_rho <= RHO_TOL * max(qsum, 1e-300), (err_rho, qsum)
+    out = oracle.force(atoms, L, m, S, rho_o, w=w, sel=sel, with_energy=with_energy)
+    F_o, e_o = out if with_energy else (out, None)
+    Fg = F_g[:, :3].astype(np.float64)
+    if sel is not None:
+        Fg = Fg[sel]
+    nrm = np.linalg.norm(F_o)
+    err_F = np.linalg.norm(Fg - F_o) / nrm if nrm > 0 else np.abs(Fg).max()
+    assert err_F <= f_tol, err_F
+    U_o = oracle.energy(L, m, S, rho_o, w=w)
+    assert abs(U_g - U_o) <= U_TOL * abs(U_o) + 1e-300, (U_g, U_o)
+    eg = F_g[:, 3].astype(np.float64)
+    if with_energy:
+        egs = eg if sel is None else eg[sel]
+        assert np.linalg.norm(egs - e_o) <= 2e-5 * np.linalg.norm(e_o) + 1e-12
+    else:
+        assert np.all(eg == 0.0)
+    assert np.isfinite(F_g).all()
+    return dict(rho=err_rho / max(qsum, 1e-300), F=err_F, U=abs(U_g - U_o) / max(abs(U_o), 1e-300),
+                F_gpu=F_g, rho_gpu=rho_g)
+
+
+# ------------------------------------------------------------------ BASELINE.json configs
+@pytest.mark.parametrize("name", ["water_3k", "water_96k"])
+@pytest.mark.parametrize("with_energy", [False, True])
+def test_config_small(name, with_energy):
+    cfg = inputs.CONFIGS[name]
+    atoms = inputs.make_atoms(cfg)
+    m = inputs.sample_kset(cfg.L, cfg.alpha, cfg.P, cfg.seed, 0)
+    r = check(atoms, cfg.L, cfg.alpha, m, with_energy=with_energy)
+    # momentum conservation on the GPU result: |sum_i F_i|_inf <= 1e-6 * sum_i |F_i|_inf
+    F = r["F_gpu"][:, :3].astype(np.float64)
+    assert np.abs(F.sum(0)).max() <= 1e-6 * np.abs(F).max(1).sum()
+
+
+def test_config_1m_full_size_bench_configuration():
+    """Config 3 (N = 999 999, P = 200) in the launch configuration bench.py times: rho against
+    the full oracle, forces on 20 000 sampled atoms, sum F = 0 over all atoms."""
+    cfg = inputs.CONFIGS["water_nacl_1m"]
+    atoms = inputs.make_atoms(cfg)
+    m = inputs.sample_kset(cfg.L, cfg.alpha, cfg.P, cfg.seed, 0)
+    sel = np.sort(np.random.default_rng(0).choice(cfg.N, 20_000, replace=False)).astype(np.int64)
+    sel[-3:] = [cfg.N - 3, cfg.N - 2, cfg.N - 1]  # the ragged tail and the ions
+    r = check(atoms, cfg.L, cfg.alpha, m, with_energy=False, sel=sel)
+    F = r["F_gpu"][:, :3].astype(np.float64)
+    assert np.abs(F.sum(0)).max() <= 1e-6 * np.abs(F).max(1).sum()
+
+
+def test_config_10m_sampled():
+    cfg = inputs.CONFIGS["water_10m"]
+    atoms = inputs.make_atoms(cfg)
+    m = inputs.sample_kset(cfg.L, cfg.alpha, cfg.P, cfg.seed, 0)
+    sel = np.sort(np.random.default_rng(1).choice(cfg.N, 5_000, replace=False)).astype(np.int64)
+    check(atoms, cfg.L, cfg.alpha, m, sel=sel)
+
+
+def test_ions_1e8_max_size_small_batch():
+    """The largest sweep point (N = 1e8, L = 1000 A: the hardest case for fp32 phases).  The
+    oracle cannot do P = 200 here in minutes, so the batch is P = 8 and forces are sampled."""
+    cfg = inputs.ions_config(10 ** 8, P=8)
+    atoms = inputs.make_atoms(cfg)
+    m = inputs.sample_kset(cfg.L, cfg.alpha, cfg.P, cfg.seed, 0)
+    sel = np.sort(np.random.default_rng(2).choice(cfg.N, 2_000, replace=False)).astype(np.int64)
+    check(atoms, cfg.L, cfg.alpha, m, sel=sel)
+
+
+# ------------------------------------------------------------------------ ragged / edge
+@pytest.mark.parametrize("N", [1, 2, 31, 32, 33, 1000, 4097, 20011])
+def test_ragged_atom_counts(N):
+    cfg = inputs.ions_config(20_012)
+    atoms = inputs.make_atoms(cfg)[:N].copy()
+    m = inputs.sample_kset(cfg.L, cfg.alpha, 100, 11, N)
+    check(atoms, cfg.L, cfg.alpha, m, with_energy=True)
+
+
+@pytest.mark.parametrize("P", [1, 3, 4, 5, 50, 127, 200, 257, 400, 800, 1600, 2049, 4500])
+def test_ragged_batch_sizes(P):
+    cfg = inputs.ions_config(10_000)
+    atoms = inputs.make_atoms(cfg)
+    m = inputs.sample_kset(cfg.L, cfg.alpha, P, 12, P)
+    check(atoms, cfg.L, cfg.alpha, m, with_energy=(P % 2 == 1))
+
+
+def test_empty_system():
+    m = inputs.sample_kset(20.0, 0.09, 16, 1)
+    ctx, rho, F, U = gpu_step(np.zeros((0, 4), dtype=np.float32), 20.0, 0.09, m)
+    assert np.all(rho == 0.0) and F.shape == (0, 4) and U == 0.0
+
+
+def test_positions_far_outside_the_box_and_extreme_m():
+    """Periodic wrap is implicit (reading Q6); |m_d| up to 2^15 - 1 is accepted (reading Q10)."""
+    L, alpha = 64.0, 0.09
+    rng = np.random.default_rng(3)
+    n = 50_000  # the fixed-point phase error |m| 2^-33 turns adds up like sqrt(N); the bar like N
+    atoms = np.empty((n, 4), dtype=np.float32)
+    atoms[:, :3] = (rng.random((n, 3)) * 40 - 20) * L  # up to 20 boxes away
+    atoms[:, 3] = np.where(np.arange(n) % 2 == 0, 1.0, -1.0)
+    m = inputs.sample_kset(L, alpha, 64, 5)
+    m[0] = [32767, -32767, 32767]
+    m[1] = [-32767, 0, 1]
+    # |x| ~ 1280 A carries an fp32 ulp of 1.2e-4 A; the oracle sees the same fp32 values
+    check(atoms, L, alpha, m, with_energy=True)
+
+
+def test_weighted_full_grid_reproduces_deterministic_ewald():
+    """w_l = exp(-k_l^2/4alpha) over every grid vector: the GPU kernels evaluate Eq. (2.11) and
+    the second term of Eq. (2.8) -- compared with oracle.ewald_full, not with the RBE oracle."""
+    L, alpha, mmax = 12.0, 0.3, 7
+    cfg = inputs.ions_config(400)
+    atoms = inputs.make_atoms(cfg)
+    atoms[:, :3] *= np.float32(L / cfg.L)
+    m = inputs.full_kgrid(mmax)
+    k2 = (2 * np.pi / L) ** 2 * (m.astype(np.float64) ** 2).sum(1)
+    w = np.exp(-k2 / (4 * alpha))
+    ctx, rho, F, U = gpu_step(atoms, L, alpha, m, w=w, with_energy=True)
+    Uref, _, Fl = oracle.ewald_full(atoms[:, :3].astype(np.float64), atoms[:, 3].astype(np.float64),
+                                    L, alpha, nreal=0, mmax=mmax)
+    assert np.linalg.norm(F[:, :3] - Fl) / np.linalg.norm(Fl) <= F_TOL
+    assert abs(U - Uref[1]) <= U_TOL * abs(Uref[1])
+    assert abs(F[:, 3].astype(np.float64).sum() - Uref[1]) <= 1e-4 * abs(Uref[1])
+
+
+def test_bitwise_reproducible_and_k_resubmission():
+    cfg = inputs.CONFIGS["water_96k"]
+    atoms = inputs.make_atoms(cfg)
+    xyzq = torch.from_numpy(atoms).cuda()
+    ctx = rbe.Rbe(cfg.N, cfg.L, cfg.alpha, cfg.P)
+    outs = []
+    for step in (0, 1, 0):
+        m = inputs.sample_kset(cfg.L, cfg.alpha, cfg.P, cfg.seed, step)
+        rho = torch.empty((cfg.P, 2), dtype=torch.float64, device="cuda")
+        F = torch.empty((cfg.N, 4), dtype=torch.float32, device="cuda")
+        ctx.rbe_set_kvectors(m)
+        ctx.rbe_structure_factor(xyzq, rho)
+        ctx.rbe_forces(xyzq, F)
+        outs.append((rho.cpu().numpy().copy(), F.cpu().numpy().copy(), ctx.rbe_kspace_energy()))
+    assert np.array_equal(outs[0][0], outs[2][0]) and np.array_equal(outs[0][1], outs[2][1])
+    assert outs[0][2] == outs[2][2]
+    assert not np.array_equal(outs[0][0], outs[1][0])
+
+
+def test_call_order_errors_on_device():
+    ctx = rbe.Rbe(64, 10.0, 0.3, 4)
+    xyzq = torch.zeros((64, 4), dtype=torch.float32, device="cuda")
+    F = torch.zeros((64, 4), dtype=torch.float32, device="cuda")
+    with pytest.raises(rbe.RbeError) as e:
+        ctx.rbe_structure_factor(xyzq)
+    assert e.value.status == 3
+    ctx.rbe_set_kvectors(np.array([[1, 0, 0], [0, 1, 0], [0, 0, 1], [1, 1, 1]], dtype=np.int32))
+    with pytest.raises(rbe.RbeError) as e:
+        ctx.rbe_forces(xyzq, F)
+    assert e.value.status == 3
+    ctx.rbe_structure_factor(xyzq)
+    ctx.rbe_forces(xyzq, F)
+    ctx.rbe_set_kvectors(np.array([[2, 0, 0], [0, 1, 0], [0, 0, 1], [1, 1, 1]], dtype=np.int32))
+    with pytest.raises(rbe.RbeError):  # a new k-set invalidates the structure factor
+        ctx.rbe_forces(xyzq, F)
+    info = ctx.rbe_get_launch_info()
+    assert info["num_sms"] >= 100 and info["sf_grid_x"] >= 1
+
+
+def test_two_shards_with_rank_ordered_sum_match_single_context():
+    """Multi-GPU data path on one device: two contexts own half the atoms each; the partial
+    structure factors are summed in rank order and injected with rbe_set_rho."""
+    cfg = inputs.CONFIGS["water_96k"]
+    atoms = inputs.make_atoms(cfg)
+    m = inputs.sample_kset(cfg.L, cfg.alpha, cfg.P, cfg.seed, 0)
+    parts, ctxs, xs = [], [], []
+    for rank in range(2):
+        lo, hi = inputs.shard_bounds(cfg.N, 2, rank, align=32)
+        x = torch.from_numpy(atoms[lo:hi].copy()).cuda()
+        c = rbe.Rbe(hi - lo, cfg.L, cfg.alpha, cfg.P)
+        rho = torch.empty((cfg.P, 2), dtype=torch.float64, device="cuda")
+        c.rbe_set_kvectors(m)
+        c.rbe_structure_factor(x, rho)
+        parts.append(rho); ctxs.append(c); xs.append(x)
+    total = parts[0] + parts[1]
+    Fs = []
+    for c, x in zip(ctxs, xs):
+        F = torch.empty((x.shape[0], 4), dtype=torch.float32, device="cuda")
+        c.rbe_set_rho(total)
+        c.rbe_forces(x, F)
+        Fs.append(F.cpu().numpy())
+    F_g = np.concatenate(Fs)[:, :3].astype(np.float64)
+    S = oracle.S(cfg.L, cfg.alpha)
+    rho_o = oracle.rho(atoms, cfg.L, m)
+    F_o = oracle.force(atoms, cfg.L, m, S, rho_o)
+    assert np.abs(total.cpu().numpy() - rho_o).max() <= RHO_TOL * np.abs(atoms[:, 3]).sum()
+    assert np.linalg.norm(F_g - F_o) / np.linalg.norm(F_o) <= F_TOL
+
+
+def test_host_buffer_step_matches_device_path():
+    cfg = inputs.CONFIGS["water_3k"]
+    atoms = inputs.make_atoms(cfg)
+    m = inputs.sample_kset(cfg.L, cfg.alpha, cfg.P, cfg.seed, 0)
+    ctx, rho_g, F_g, U_g = gpu_step(atoms, cfg.L, cfg.alpha, m, with_energy=True)
+    h_x = torch.from_numpy(atoms).pin_memory()
+    h_f = torch.empty((cfg.N, 4), dtype=torch.float32).pin_memory()
+    U = ctx.rbe_step_host(h_x, m, h_f, with_energy=True, want_energy=True)
+    assert np.array_equal(h_f.numpy(), F_g) and U == U_g
