@@ -4,6 +4,7 @@
 
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <string>
@@ -27,9 +28,11 @@ struct rbe_ctx {
     bool dev_ready = false;
     int device = -1;
     rbe_launch_info li{};
-    int sf_gs = 0, sf_ng = 0, sf_ai = 0;
+    int sf_gs = 0, sf_ng = 0, sf_flush_every = 1;
+    int sf_pairing = 3;
+    bool sf_deep = false;   // a group takes more than SF_DEPTH atoms from one tile: flush inside the loops
     size_t ws_bytes = 0;
-    size_t off_kvec = 0, off_w = 0, off_part = 0, off_rho = 0, off_ka = 0, off_kb = 0, off_uk = 0, off_U = 0;
+    size_t off_kvec = 0, off_w = 0, off_part = 0, off_rho = 0, off_ka = 0, off_kb = 0, off_uk = 0, off_U = 0, off_ticket = 0;
 
     // workspace
     unsigned char* ws = nullptr;
@@ -93,41 +96,41 @@ rbe_status init_device(rbe_ctx* c) {
     rbe_launch_info& li = c->li;
     li.num_sms = prop.multiProcessorCount;
 
-    // ---- SF kernel: a thread owns SF_KPT wavevectors; gs threads cover one k-chunk.
+    // ---- SF kernel: a thread owns SF_KPT wavevectors; gs threads cover one k-chunk, ng atom
+    // groups share a CTA of up to SF_TMAX threads (one CTA per SM); tile = blockDim.x atoms.
     const int slots = (c->P + rbe::SF_KPT - 1) / rbe::SF_KPT;
     int gy = (slots + rbe::SF_TMAX - 1) / rbe::SF_TMAX;
     int gs = (slots + gy - 1) / gy;
     int ng = rbe::SF_TMAX / gs;
     if (ng < 1) ng = 1;
     int threads = (int)align_up((size_t)gs * ng, 32);
-    int ai = rbe::SF_AI;
-    if (ng * ai > 2 * threads) ai = (2 * threads) / ng;
-    if (ai < 1) ai = 1;
     int gx = li.num_sms / gy;
     if (gx < 1) gx = 1;
-    // never more CTAs than groups of atoms to feed them
-    const int64_t max_gx = c->N > 0 ? (c->N + ng - 1) / ng : 1;
+    // never more CTAs than 32-atom windows to feed them
+    const int64_t max_gx = c->N > 0 ? (c->N + 31) / 32 : 1;
     if ((int64_t)gx > max_gx) gx = (int)max_gx;
-    c->sf_gs = gs; c->sf_ng = ng; c->sf_ai = ai;
+    const int per_group = (threads + ng - 1) / ng;   // atoms a group takes from one tile
+    c->sf_gs = gs; c->sf_ng = ng;
+    c->sf_flush_every = per_group >= rbe::SF_DEPTH ? 1 : rbe::SF_DEPTH / per_group;
+    c->sf_deep = per_group + 1 > rbe::SF_DEPTH;
     li.sf_grid_x = gx; li.sf_grid_y = gy; li.sf_threads = threads;
-    li.sf_k_per_thread = rbe::SF_KPT; li.sf_atom_groups = ng; li.sf_tile_atoms = ng * ai;
-    size_t sm_tiles = (size_t)2 * ng * ai * sizeof(uint4);
-    size_t sm_red = (size_t)ng * gs * rbe::SF_KPT * sizeof(double2);
-    li.sf_smem_bytes = (int32_t)(sm_tiles > sm_red ? sm_tiles : sm_red);
+    li.sf_k_per_thread = rbe::SF_KPT; li.sf_atom_groups = ng; li.sf_tile_atoms = threads;
+    // raw tile + record arena (16 B per atom each) + fp64 accumulators [SF_KPT][threads]
+    li.sf_smem_bytes = (int32_t)((size_t)threads * (2 * sizeof(uint4) + rbe::SF_KPT * sizeof(double2)));
 
     li.fin_grid = (c->P + rbe::FIN_KB - 1) / rbe::FIN_KB;
     li.fin_threads = rbe::FIN_KB * rbe::FIN_SL;
 
     // ---- F kernel: warps take balanced runs of 32-atom units; one wave of CTAs.
     li.f_threads = rbe::F_THREADS;
-    li.f_atoms_per_thread = 4;
+    li.f_atoms_per_thread = rbe::F_RMAX;
     const int nk = c->P < rbe::F_KCHUNK ? c->P : rbe::F_KCHUNK;
     li.f_smem_bytes = (int32_t)((size_t)nk * (sizeof(int4) + sizeof(float4)));
-    RBE_CUDA(c, cudaFuncSetAttribute(rbe::f_kernel<4, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, li.f_smem_bytes));
-    RBE_CUDA(c, cudaFuncSetAttribute(rbe::f_kernel<4, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, li.f_smem_bytes));
+    RBE_CUDA(c, cudaFuncSetAttribute(rbe::f_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, li.f_smem_bytes));
+    RBE_CUDA(c, cudaFuncSetAttribute(rbe::f_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, li.f_smem_bytes));
     int occ0 = 0, occ1 = 0;  // resident CTAs per SM: the grid is exactly one wave
-    RBE_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ0, rbe::f_kernel<4, false>, rbe::F_THREADS, li.f_smem_bytes));
-    RBE_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ1, rbe::f_kernel<4, true>, rbe::F_THREADS, li.f_smem_bytes));
+    RBE_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ0, rbe::f_kernel<false>, rbe::F_THREADS, li.f_smem_bytes));
+    RBE_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ1, rbe::f_kernel<true>, rbe::F_THREADS, li.f_smem_bytes));
     int f_ctas_per_sm = occ0 < occ1 ? occ0 : occ1;
     if (f_ctas_per_sm < 1) f_ctas_per_sm = 1;
     if (f_ctas_per_sm > 4) f_ctas_per_sm = 4;
@@ -137,7 +140,8 @@ rbe_status init_device(rbe_ctx* c) {
     if (f_grid > max_f) f_grid = max_f;
     li.f_grid = (int32_t)f_grid;
 
-    RBE_CUDA(c, cudaFuncSetAttribute(rbe::sf_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, li.sf_smem_bytes));
+    RBE_CUDA(c, cudaFuncSetAttribute(rbe::sf_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, li.sf_smem_bytes));
+    RBE_CUDA(c, cudaFuncSetAttribute(rbe::sf_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, li.sf_smem_bytes));
 
     // ---- workspace layout
     size_t off = 0;
@@ -150,6 +154,7 @@ rbe_status init_device(rbe_ctx* c) {
     c->off_kb = off;   off = align_up(off + P * sizeof(float4), 256);
     c->off_uk = off;   off = align_up(off + P * sizeof(double), 256);
     c->off_U = off;    off = align_up(off + sizeof(double), 256);
+    c->off_ticket = off; off = align_up(off + sizeof(unsigned int), 256);
     c->ws_bytes = off;
 
     c->stage_bytes = P * (sizeof(int4) + sizeof(double));
@@ -160,7 +165,7 @@ rbe_status init_device(rbe_ctx* c) {
 template <typename T>
 T* ws_ptr(rbe_ctx* c, size_t off) { return reinterpret_cast<T*>(c->ws + off); }
 
-rbe_status launch_fin(rbe_ctx* c, const double2* part, int nrows, double2* rho_user, cudaStream_t st) {
+rbe::FinParams fin_params(rbe_ctx* c, const double2* part, int nrows, double2* rho_user) {
     rbe::FinParams fp;
     fp.part = part; fp.nrows = nrows; fp.P = c->P;
     fp.kvec = ws_ptr<int4>(c, c->off_kvec);
@@ -172,6 +177,11 @@ rbe_status launch_fin(rbe_ctx* c, const double2* part, int nrows, double2* rho_u
     fp.ka = ws_ptr<int4>(c, c->off_ka);
     fp.kb = ws_ptr<float4>(c, c->off_kb);
     fp.uk = ws_ptr<double>(c, c->off_uk);
+    return fp;
+}
+
+rbe_status launch_fin(rbe_ctx* c, const double2* part, int nrows, double2* rho_user, cudaStream_t st) {
+    const rbe::FinParams fp = fin_params(c, part, nrows, rho_user);
     rbe::fin_kernel<<<c->li.fin_grid, c->li.fin_threads, 0, st>>>(fp);
     RBE_CUDA(c, cudaGetLastError());
     c->have_rho = true;
@@ -192,6 +202,7 @@ rbe_status rbe_create(rbe_ctx** out, int64_t N, double L, double alpha, int32_t 
     if (!c) return RBE_ERR_INVALID_ARG;
     c->N = N; c->L = L; c->alpha = alpha; c->P = P;
     c->S = normaliser_S(L, alpha);
+    if (const char* e = std::getenv("RBE_SF_PAIRING")) c->sf_pairing = std::atoi(e);
     *out = c;
     return RBE_OK;
 }
@@ -223,6 +234,9 @@ rbe_status rbe_set_workspace(rbe_ctx* c, void* d_ws, size_t bytes) {
         return fail(c, RBE_ERR_WORKSPACE, "workspace must be non-null, 256-byte aligned and >= rbe_workspace_bytes");
     c->ws = static_cast<unsigned char*>(d_ws);
     c->have_k = c->have_w = c->have_rho = false;
+    // the structure-factor kernel's completion ticket starts at zero and resets itself
+    RBE_CUDA(c, cudaMemset(c->ws + c->off_ticket, 0, sizeof(unsigned int)));
+    RBE_CUDA(c, cudaDeviceSynchronize());
     return RBE_OK;
 }
 
@@ -283,11 +297,17 @@ rbe_status rbe_structure_factor(rbe_ctx* c, const void* d_xyzq, void* d_rho, voi
     sp.kvec = ws_ptr<int4>(c, c->off_kvec);
     sp.part = ws_ptr<double2>(c, c->off_part);
     sp.two32_over_L = rbe::TWO32 / c->L;
-    sp.P = c->P; sp.gs = c->sf_gs; sp.ng = c->sf_ng; sp.ai = c->sf_ai;
+    sp.P = c->P; sp.gs = c->sf_gs; sp.ng = c->sf_ng; sp.flush_every = c->sf_flush_every;
+    sp.pairing = c->sf_pairing;
+    sp.ticket = ws_ptr<unsigned int>(c, c->off_ticket);
+    // the last CTA to finish runs the fixed-order finalise: no second launch on the hot path
+    sp.fin = fin_params(c, sp.part, c->li.sf_grid_x, static_cast<double2*>(d_rho));
     dim3 grid(c->li.sf_grid_x, c->li.sf_grid_y);
-    rbe::sf_kernel<<<grid, c->li.sf_threads, c->li.sf_smem_bytes, st>>>(sp);
+    if (c->sf_deep) rbe::sf_kernel<true><<<grid, c->li.sf_threads, c->li.sf_smem_bytes, st>>>(sp);
+    else rbe::sf_kernel<false><<<grid, c->li.sf_threads, c->li.sf_smem_bytes, st>>>(sp);
     RBE_CUDA(c, cudaGetLastError());
-    return launch_fin(c, sp.part, c->li.sf_grid_x, static_cast<double2*>(d_rho), st);
+    c->have_rho = true;
+    return RBE_OK;
 }
 
 rbe_status rbe_set_rho(rbe_ctx* c, const void* d_rho, void* stream) {
@@ -314,10 +334,21 @@ rbe_status rbe_forces(rbe_ctx* c, const void* d_xyzq, void* d_force, int32_t wit
     fp.kb = ws_ptr<float4>(c, c->off_kb);
     fp.two32_over_L = rbe::TWO32 / c->L;
     fp.P = c->P;
-    if (with_energy)
-        rbe::f_kernel<4, true><<<c->li.f_grid, c->li.f_threads, c->li.f_smem_bytes, st>>>(fp);
-    else
-        rbe::f_kernel<4, false><<<c->li.f_grid, c->li.f_threads, c->li.f_smem_bytes, st>>>(fp);
+    fp.pdl = 1;
+    // programmatic dependent launch: the grid may be scheduled while the structure-factor grid
+    // drains; the kernel waits (griddepcontrol.wait) before reading anything that grid wrote
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(c->li.f_grid);
+    cfg.blockDim = dim3(c->li.f_threads);
+    cfg.dynamicSmemBytes = (size_t)c->li.f_smem_bytes;
+    cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    if (with_energy) RBE_CUDA(c, cudaLaunchKernelEx(&cfg, rbe::f_kernel<true>, fp));
+    else RBE_CUDA(c, cudaLaunchKernelEx(&cfg, rbe::f_kernel<false>, fp));
     RBE_CUDA(c, cudaGetLastError());
     return RBE_OK;
 }

@@ -10,6 +10,9 @@
 // out-of-box atoms wrap for free.  The signed result in [-2^31, 2^31) is converted to fp32 and
 // scaled so that the FMUL by fl(1/2pi) inside sin.approx/cos.approx lands on turns; MUFU.SIN /
 // MUFU.COS then evaluate sin/cos(2 pi t), |t| <= 1/2.
+//
+// Measured on B200 (csrc/pipe_probe.cu, profiles/): MUFU 16 lanes/SM/clk, IMAD and I2FP 64,
+// FFMA 128; a MUFU also costs ~3 issue slots.  Both hot kernels are bound by MUFU + issue.
 #pragma once
 #include <cstdint>
 #include <cuda_runtime.h>
@@ -19,17 +22,20 @@ namespace rbe {
 // ---------------------------------------------------------------------------------------
 // tunables (compile time)
 // ---------------------------------------------------------------------------------------
-constexpr int SF_KPT = 4;       // wavevectors owned by one thread of the structure-factor kernel
-constexpr int SF_TMAX = 512;    // max threads per CTA (structure-factor kernel)
-constexpr int SF_AI = 64;       // max atoms one atom-group accumulates in fp32 before the fp64 flush
-constexpr int F_THREADS = 256;  // threads per CTA (force kernel)
-constexpr int F_KCHUNK = 2048;  // wavevectors staged in shared memory at a time (force kernel)
-constexpr int FIN_KB = 32;      // wavevectors per CTA (finalise kernel)
-constexpr int FIN_SL = 32;      // row slices per wavevector (finalise kernel)
+constexpr int SF_KPT = 4;        // wavevectors owned by one thread of the structure-factor kernel
+constexpr int SF_TMAX = 1024;    // max threads per CTA (structure-factor kernel): 1 CTA/SM, <= 64 regs
+constexpr int SF_DEPTH = 64;     // max atoms a thread accumulates in fp32 before the fp64 flush
+constexpr int F_THREADS = 256;   // threads per CTA (force kernel)
+constexpr int F_RMAX = 4;        // max atoms per thread per pass (force kernel)
+constexpr int F_KCHUNK = 2048;   // wavevectors staged in shared memory at a time (force kernel)
+constexpr int FIN_KB = 32;       // wavevectors per CTA (stand-alone finalise kernel)
+constexpr int FIN_SL = 32;       // row slices per wavevector (stand-alone finalise kernel)
 
 constexpr double TWO32 = 4294967296.0;
 constexpr double MAGIC = 6755399441055744.0;  // 2^52 + 2^51: low word of (d + MAGIC) = rint(d) mod 2^32
 constexpr double PI_D = 3.14159265358979323846264338327950288;
+constexpr uint32_t QUARTER_TURN = 0x40000000u;
+constexpr unsigned FULL_MASK = 0xffffffffu;
 
 // fl(2^-32 / fl(1/2pi)): sin.approx multiplies its argument by fl(1/2pi) = 0.15915493667125701904
 // (FMUL.RZ) before MUFU; this constant makes that product equal 2^-32 * phase to within 2^-25.
@@ -50,139 +56,24 @@ __device__ __forceinline__ float fast_cos(float x) {
     asm("cos.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
     return r;
 }
+__device__ __forceinline__ float phase_to_arg(uint32_t ph, float K) { return (float)(int32_t)ph * K; }
 
-// ---------------------------------------------------------------------------------------
-// SF kernel -- Algorithm 1 steps 2+3 fused (P:203-204), Eq. (2.9) P:117.
-//
-// Mapping: a thread OWNS SF_KPT wavevectors (their m in registers) and one of `ng` atom
-// groups; the CTA streams its contiguous atom range through shared memory in tiles of
-// ng * ai atoms (already converted to fixed-point turns), group g reading atoms g, g+ng, ...
-// as a shared-memory broadcast.  The N x P array of Fourier modes the paper materialises
-// before its Reduce-by-Key never exists; neither does any cross-lane reduction:
-// each thread sums its own (cos, sin) in fp32 over at most SF_AI atoms, then in fp64.
-// The `ng` groups are combined through shared memory in group order and one fp64 row of P
-// complex partials per CTA goes to global memory.  No atomics anywhere.
-// ---------------------------------------------------------------------------------------
-struct SfParams {
-    const float4* xyzq;
-    int64_t N;
-    const int4* kvec;  // [P] {mx, my, mz, 0}
-    double2* part;     // [gridDim.x][P]
-    double two32_over_L;
-    int32_t P;
-    int32_t gs;    // threads per atom group in this CTA = k-slots / SF_KPT
-    int32_t ng;    // atom groups per CTA
-    int32_t ai;    // atoms per group per tile (<= SF_AI); tile = ng * ai atoms <= 2 * blockDim.x
-};
-
-__device__ __forceinline__ uint4 convert_atom(float4 a, double s) {
-    uint4 r;
-    r.x = to_turns(a.x, s);
-    r.y = to_turns(a.y, s);
-    r.z = to_turns(a.z, s);
-    r.w = __float_as_uint(a.w);
-    return r;
+__device__ __forceinline__ void cp_async16(void* smem_dst, const void* gmem_src) {
+    const uint32_t d = (uint32_t)__cvta_generic_to_shared(smem_dst);
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(d), "l"(gmem_src) : "memory");
 }
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
 
-__global__ void __launch_bounds__(SF_TMAX, 1) sf_kernel(const SfParams p) {
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    uint4* tile = reinterpret_cast<uint4*>(smem_raw);
-    const int tid = threadIdx.x, T = blockDim.x;
-    const int tile_atoms = p.ng * p.ai;
-    const bool active = tid < p.gs * p.ng;
-    const int g = active ? tid / p.gs : 0;
-    const int j = active ? tid - g * p.gs : 0;
-    const int kbase = (blockIdx.y * p.gs + j) * SF_KPT;
-
-    int mx[SF_KPT], my[SF_KPT], mz[SF_KPT];
-#pragma unroll
-    for (int r = 0; r < SF_KPT; ++r) {
-        int4 m = make_int4(0, 0, 0, 0);
-        if (kbase + r < p.P) m = __ldg(&p.kvec[kbase + r]);
-        mx[r] = m.x; my[r] = m.y; mz[r] = m.z;
-    }
-    float c[SF_KPT], s[SF_KPT];
-    double cd[SF_KPT], sd[SF_KPT];
-#pragma unroll
-    for (int r = 0; r < SF_KPT; ++r) { c[r] = s[r] = 0.f; cd[r] = sd[r] = 0.0; }
-
-    const int64_t lo = (p.N * (int64_t)blockIdx.x) / gridDim.x;
-    const int64_t hi = (p.N * (int64_t)(blockIdx.x + 1)) / gridDim.x;
-    const float K = phase_scale();
-    const float4 zero4 = make_float4(0.f, 0.f, 0.f, 0.f);
-
-    // prologue: first tile -> buffer 0
-    {
-        int64_t i0 = lo + tid, i1 = i0 + T;
-        float4 a0 = (tid < tile_atoms && i0 < hi) ? __ldg(&p.xyzq[i0]) : zero4;
-        float4 a1 = (tid + T < tile_atoms && i1 < hi) ? __ldg(&p.xyzq[i1]) : zero4;
-        if (tid < tile_atoms) tile[tid] = convert_atom(a0, p.two32_over_L);
-        if (tid + T < tile_atoms) tile[tid + T] = convert_atom(a1, p.two32_over_L);
-    }
-    __syncthreads();
-
-    int cur = 0;
-    for (int64_t t0 = lo; t0 < hi; t0 += tile_atoms) {
-        // prefetch the next tile into registers (zero charge beyond the range: contributes 0)
-        const int64_t n0 = t0 + tile_atoms + tid, n1 = n0 + T;
-        float4 a0 = (tid < tile_atoms && n0 < hi) ? __ldg(&p.xyzq[n0]) : zero4;
-        float4 a1 = (tid + T < tile_atoms && n1 < hi) ? __ldg(&p.xyzq[n1]) : zero4;
-
-        const int64_t cnt = (hi - t0 < tile_atoms) ? (hi - t0) : tile_atoms;
-        const int n_ai = (int)((cnt + p.ng - 1) / p.ng);  // <= p.ai; uniform over the CTA
-        const uint4* src = tile + cur * tile_atoms + g;
-#pragma unroll 2
-        for (int a = 0; a < n_ai; ++a) {
-            const uint4 at = src[a * p.ng];
-            const float q = __uint_as_float(at.w);
-#pragma unroll
-            for (int r = 0; r < SF_KPT; ++r) {
-                const uint32_t ph = (uint32_t)mx[r] * at.x + (uint32_t)my[r] * at.y + (uint32_t)mz[r] * at.z;
-                const float x = (float)(int32_t)ph * K;
-                c[r] = fmaf(q, fast_cos(x), c[r]);
-                s[r] = fmaf(q, fast_sin(x), s[r]);
-            }
-        }
-#pragma unroll
-        for (int r = 0; r < SF_KPT; ++r) {
-            cd[r] += (double)c[r]; sd[r] += (double)s[r];
-            c[r] = 0.f; s[r] = 0.f;
-        }
-        // stage the prefetched tile into the other buffer
-        uint4* dst = tile + (cur ^ 1) * tile_atoms;
-        if (tid < tile_atoms) dst[tid] = convert_atom(a0, p.two32_over_L);
-        if (tid + T < tile_atoms) dst[tid + T] = convert_atom(a1, p.two32_over_L);
-        __syncthreads();
-        cur ^= 1;
-    }
-
-    // combine the atom groups in group order, one fp64 row per CTA
-    double2* red = reinterpret_cast<double2*>(smem_raw);
-    const int kslots = p.gs * SF_KPT;
-    __syncthreads();
-    if (active) {
-#pragma unroll
-        for (int r = 0; r < SF_KPT; ++r) red[g * kslots + j * SF_KPT + r] = make_double2(cd[r], sd[r]);
-    }
-    __syncthreads();
-    for (int idx = tid; idx < kslots; idx += T) {
-        const int k = blockIdx.y * kslots + idx;
-        if (k < p.P) {
-            double re = 0.0, im = 0.0;
-            for (int gg = 0; gg < p.ng; ++gg) {
-                const double2 v = red[gg * kslots + idx];
-                re += v.x; im += v.y;
-            }
-            p.part[(int64_t)blockIdx.x * p.P + k] = make_double2(re, im);
-        }
-    }
-}
+// Programmatic dependent launch (PDL): the force kernel may start while the structure-factor
+// kernel drains; it waits here before touching anything that kernel writes.
+__device__ __forceinline__ void grid_dependency_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void grid_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
 
 // ---------------------------------------------------------------------------------------
-// FIN kernel -- second pass of the reduction and the per-k force coefficients.
+// Finalise: second pass of the reduction and the per-k force coefficients.
 //
-// rho_l = sum over the SF kernel's per-CTA rows in a FIXED order (row slices sl, sl+32, ...
-// summed sequentially, then the 32 slice sums sequentially), so rho is bitwise reproducible.
+// rho_l = sum over the SF kernel's per-CTA rows in a FIXED order (row slices sl, sl+nsl, ...
+// summed sequentially, then the nsl slice sums sequentially), so rho is bitwise reproducible.
 // Then, with w_l the sample weight (S/P of Eq. 2.12 unless the caller gave weights):
 //   Im(e^{-i phi} rho) = |rho| sin(theta - phi),  theta = arg rho,
 // so Eq. (2.12) becomes  F_i = q_i sum_l G_l sin(2 pi (theta_l - m_l . s_i))  with
@@ -205,6 +96,50 @@ struct FinParams {
     double* uk;           // [P] out e_l |rho_l|^2
 };
 
+__device__ __forceinline__ void fin_coefficients(const FinParams& p, int k, double re, double im) {
+    const int4 m = p.kvec[k];
+    const double w = p.w ? p.w[k] : p.w_uniform;
+    const double m2 = (double)m.x * m.x + (double)m.y * m.y + (double)m.z * m.z;
+    const double mag = sqrt(re * re + im * im);
+    const double theta = atan2(im, re) * (1.0 / (2.0 * PI_D));        // turns, [-1/2, 1/2]
+    const double gs = -2.0 * w / (p.L * p.L * m2) * mag;
+    const double el = w / (2.0 * PI_D * p.L * m2);
+    p.rho[k] = make_double2(re, im);
+    if (p.rho_user) p.rho_user[k] = make_double2(re, im);
+    p.ka[k] = make_int4(-m.x, -m.y, -m.z, __double2loint(fma(theta, TWO32, MAGIC)));
+    p.kb[k] = make_float4((float)(gs * m.x), (float)(gs * m.y), (float)(gs * m.z), (float)(el * mag));
+    p.uk[k] = el * mag * mag;
+}
+
+// One CTA of `nt` threads finalises all P wavevectors; `scratch` holds nt double2.
+// Used by the LAST structure-factor CTA to finish (no separate launch on the hot path).
+__device__ __forceinline__ void fin_cta(const FinParams& p, double2* scratch, int tid, int nt) {
+    const int kc = p.P < nt ? p.P : nt;   // wavevectors per chunk
+    const int nsl = nt / kc;              // row slices per wavevector (>= 1)
+    const int kk = tid % kc, sl = tid / kc;
+    for (int k0 = 0; k0 < p.P; k0 += kc) {
+        const int k = k0 + kk;
+        double re = 0.0, im = 0.0;
+        if (sl < nsl && k < p.P) {
+#pragma unroll 8
+            for (int row = sl; row < p.nrows; row += nsl) {
+                const double2 v = __ldcg(&p.part[(int64_t)row * p.P + k]);
+                re += v.x; im += v.y;
+            }
+        }
+        if (sl < nsl) scratch[sl * kc + kk] = make_double2(re, im);
+        __syncthreads();
+        if (sl == 0 && k < p.P) {
+            re = 0.0; im = 0.0;
+#pragma unroll 1
+            for (int t = 0; t < nsl; ++t) { re += scratch[t * kc + kk].x; im += scratch[t * kc + kk].y; }
+            fin_coefficients(p, k, re, im);
+        }
+        __syncthreads();
+    }
+}
+
+// Stand-alone finalise (rbe_set_rho: the multi-GPU exchange point injects a global rho).
 __global__ void __launch_bounds__(FIN_KB * FIN_SL) fin_kernel(const FinParams p) {
     __shared__ double2 sl_sum[FIN_SL][FIN_KB];
     const int kk = threadIdx.x % FIN_KB, sl = threadIdx.x / FIN_KB;
@@ -222,19 +157,7 @@ __global__ void __launch_bounds__(FIN_KB * FIN_SL) fin_kernel(const FinParams p)
     re = 0.0; im = 0.0;
 #pragma unroll 1
     for (int t = 0; t < FIN_SL; ++t) { re += sl_sum[t][kk].x; im += sl_sum[t][kk].y; }
-
-    const int4 m = p.kvec[k];
-    const double w = p.w ? p.w[k] : p.w_uniform;
-    const double m2 = (double)m.x * m.x + (double)m.y * m.y + (double)m.z * m.z;
-    const double mag = sqrt(re * re + im * im);
-    const double theta = atan2(im, re) * (1.0 / (2.0 * PI_D));        // turns, [-1/2, 1/2]
-    const double gs = -2.0 * w / (p.L * p.L * m2) * mag;
-    const double el = w / (2.0 * PI_D * p.L * m2);
-    p.rho[k] = make_double2(re, im);
-    if (p.rho_user) p.rho_user[k] = make_double2(re, im);
-    p.ka[k] = make_int4(-m.x, -m.y, -m.z, __double2loint(fma(theta, TWO32, MAGIC)));
-    p.kb[k] = make_float4((float)(gs * m.x), (float)(gs * m.y), (float)(gs * m.z), (float)(el * mag));
-    p.uk[k] = el * mag * mag;
+    fin_coefficients(p, k, re, im);
 }
 
 // U = sum_l uk[l] in a fixed order (thread-strided partials, then a fixed tree).
@@ -252,13 +175,229 @@ __global__ void __launch_bounds__(256) energy_kernel(const double* uk, int32_t P
 }
 
 // ---------------------------------------------------------------------------------------
+// SF kernel -- Algorithm 1 steps 2+3 fused (P:203-204), Eq. (2.9) P:117.
+//
+// Mapping: a thread OWNS SF_KPT wavevectors (their m in registers) and one of `ng` atom
+// groups.  The CTA streams its contiguous atom range through shared memory in tiles of
+// blockDim.x atoms (cp.async prefetch of the raw float4 records); the N x P array of Fourier
+// modes the paper materialises before its Reduce-by-Key never exists, and there is no
+// cross-lane reduction: each thread sums its own (cos, sin) in fp32 over at most ~SF_DEPTH
+// atoms, then in fp64 (shared-memory accumulators).  Groups are combined in group order and
+// one fp64 row of P complex partials per CTA goes to global memory.  No atomics on data.
+//
+// Equal-|q| pairing (what makes this kernel 3 MUFU per TWO pairs instead of 4).  For two atoms
+// with q_2 = +-q_1 and turns S_1, S_2 let S_d = (S_1 - S_2)/2, S_a = S_2 + S_d.  Then exactly
+//   q_1 e^{i phi_1} + q_2 e^{i phi_2} = 2 q_1 cos(2 pi m.S_d - o) e^{i (2 pi m.S_a + o)},
+// o = 0 for equal charges, a quarter turn for opposite ones (2i sin d = 2 cos(d - pi/2) e^{i pi/2}).
+// While staging a tile each warp matches the 32 atoms of its window by |q| bit pattern
+// (MATCH.ANY) and emits pair records {S_a, o}{S_d, 2 q_1} and single records {S, q} for the
+// leftovers, so ANY charge assignment is handled (all-distinct charges fall back to 2 MUFU per
+// pair).  MD systems have a handful of distinct charge magnitudes, so nearly all atoms pair up.
+// Compaction of the records is by warp counts + a prefix scan: deterministic order.
+//
+// The last CTA to finish (atomicInc ticket; data order never depends on it) finalises:
+// fixed-order sum of the per-CTA rows and the per-k force coefficients (fin_cta).
+// ---------------------------------------------------------------------------------------
+struct SfParams {
+    const float4* xyzq;
+    int64_t N;
+    const int4* kvec;  // [P] {mx, my, mz, 0}
+    double2* part;     // [gridDim.x][P]
+    double two32_over_L;
+    int32_t P;
+    int32_t gs;        // threads per atom group in this CTA = k-slots / SF_KPT
+    int32_t ng;        // atom groups per CTA
+    int32_t flush_every;  // tiles between fp64 flushes (keeps the fp32 depth <= ~SF_DEPTH atoms)
+    int32_t pairing;      // bit 0: pair equal charges, bit 1: pair opposite charges (3 = both)
+    unsigned int* ticket;  // zero-initialised, self-resetting (atomicInc wraps)
+    FinParams fin;
+};
+
+// acc points at this thread's slot of component 0; component r lives `stride` entries further
+// (layout [SF_KPT][blockDim.x]: conflict-free).
+__device__ __forceinline__ void sf_flush(double2* acc, int stride, float (&c)[SF_KPT], float (&s)[SF_KPT]) {
+#pragma unroll
+    for (int r = 0; r < SF_KPT; ++r) {
+        double2 v = acc[r * stride];
+        v.x += (double)c[r]; v.y += (double)s[r];
+        acc[r * stride] = v;
+        c[r] = 0.f; s[r] = 0.f;
+    }
+}
+
+template <bool DEEP>
+__global__ void __launch_bounds__(SF_TMAX, 1) sf_kernel(const SfParams p) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int tid = threadIdx.x, T = blockDim.x, lane = tid & 31, warp = tid >> 5, nwarps = T >> 5;
+    float4* raw = reinterpret_cast<float4*>(smem_raw);               // [T] raw atom records of the tile
+    uint4* arena = reinterpret_cast<uint4*>(smem_raw) + T;           // [T] pair records from the front, singles from the back
+    double2* acc_all = reinterpret_cast<double2*>(arena + T);        // [SF_KPT][T] fp64 accumulators
+    __shared__ uint32_t wcount[SF_TMAX / 32];
+    __shared__ uint32_t s_last;
+
+    const bool active = tid < p.gs * p.ng;
+    const int g = active ? tid / p.gs : (1 << 28);  // inactive threads: group index past every list -> empty loops
+    const int j = active ? tid % p.gs : 0;
+    const int kbase = (blockIdx.y * p.gs + j) * SF_KPT;
+    double2* acc = acc_all + tid;
+
+    int mx[SF_KPT], my[SF_KPT], mz[SF_KPT];
+    float c[SF_KPT], s[SF_KPT];
+#pragma unroll
+    for (int r = 0; r < SF_KPT; ++r) {
+        int4 m = make_int4(0, 0, 0, 0);
+        if (active && kbase + r < p.P) m = __ldg(&p.kvec[kbase + r]);
+        mx[r] = m.x; my[r] = m.y; mz[r] = m.z;
+        c[r] = s[r] = 0.f;
+        acc[r * T] = make_double2(0.0, 0.0);
+    }
+
+    // this CTA's atom range, aligned to 32-atom windows
+    const int64_t units = (p.N + 31) >> 5;
+    const int64_t lo = (units * blockIdx.x / gridDim.x) << 5;
+    int64_t hi = (units * (blockIdx.x + 1) / gridDim.x) << 5;
+    if (hi > p.N) hi = p.N;
+    const float K = phase_scale();
+    const uint32_t lt_mask = (1u << lane) - 1u;
+
+    if (lo + tid < hi) cp_async16(&raw[tid], &p.xyzq[lo + tid]);
+    int since_flush = 0;
+
+    for (int64_t t0 = lo; t0 < hi; t0 += T) {
+        const int cnt = (int)((hi - t0 < T) ? (hi - t0) : T);
+        cp_async_wait_all();
+        __syncthreads();  // raw holds the tile; everyone is done with the previous arena
+
+        // ---- stage: window = this warp's 32 atoms; match equal |q|, convert to turns
+        const bool in_range = tid < cnt;
+        const float4 a = in_range ? raw[tid] : make_float4(0.f, 0.f, 0.f, 0.f);
+        const uint32_t key = __float_as_uint(a.w) & ((p.pairing & 3) == 3 ? 0x7fffffffu : 0xffffffffu);
+        const bool valid = in_range && (key & 0x7fffffffu) != 0u;   // zero charges contribute nothing: dropped
+        const uint32_t vmask = __ballot_sync(FULL_MASK, valid);
+        const uint32_t peers = (p.pairing & 3) ? (__match_any_sync(FULL_MASK, key) & vmask) : (valid ? 1u << lane : 0u);
+        const int rank = __popc(peers & lt_mask);
+        const bool has_next = (peers >> lane) > 1u;  // a peer in a higher lane exists
+        const bool leader = valid && !(rank & 1) && has_next;
+        const bool single = valid && !(rank & 1) && !has_next;
+        const uint32_t lmask = __ballot_sync(FULL_MASK, leader);
+        const uint32_t smask = __ballot_sync(FULL_MASK, single);
+        if (lane == 0) wcount[warp] = (uint32_t)__popc(lmask) | ((uint32_t)__popc(smask) << 16);
+        const uint32_t higher = (peers >> lane) >> 1;                 // peers above this lane
+        const int partner = leader ? lane + __ffs(higher) : lane;
+        const uint32_t Sx = to_turns(a.x, p.two32_over_L);
+        const uint32_t Sy = to_turns(a.y, p.two32_over_L);
+        const uint32_t Sz = to_turns(a.z, p.two32_over_L);
+        const uint32_t Px = __shfl_sync(FULL_MASK, Sx, partner);
+        const uint32_t Py = __shfl_sync(FULL_MASK, Sy, partner);
+        const uint32_t Pz = __shfl_sync(FULL_MASK, Sz, partner);
+        const uint32_t Pq = __shfl_sync(FULL_MASK, __float_as_uint(a.w), partner);
+        __syncthreads();  // wcount visible; raw fully consumed
+
+        // prefetch the next tile while this one is processed
+        if (t0 + T + tid < hi) cp_async16(&raw[tid], &p.xyzq[t0 + T + tid]);
+
+        // every warp scans the (<= 32) window counts: deterministic record positions
+        uint32_t v = lane < nwarps ? wcount[lane] : 0u, incl = v;
+#pragma unroll
+        for (int d = 1; d < 32; d <<= 1) {
+            const uint32_t n = __shfl_up_sync(FULL_MASK, incl, d);
+            if (lane >= d) incl += n;
+        }
+        const uint32_t base = __shfl_sync(FULL_MASK, incl - v, warp);
+        const uint32_t total = __shfl_sync(FULL_MASK, incl, 31);
+        const int np = (int)(total & 0xffffu), ns = (int)(total >> 16);
+        if (leader) {
+            // S_d = (S_1 - S_2) / 2 (arithmetic shift of the wrapped difference), S_a = S_2 + S_d
+            const int e = (int)(base & 0xffffu) + __popc(lmask & lt_mask);
+            const uint32_t dx = (uint32_t)((int32_t)(Sx - Px) >> 1);
+            const uint32_t dy = (uint32_t)((int32_t)(Sy - Py) >> 1);
+            const uint32_t dz = (uint32_t)((int32_t)(Sz - Pz) >> 1);
+            // o: a quarter turn for opposite charges; plus half a turn on every other pair, which leaves
+            // cos(d - o) e^{i(a + o)} unchanged but alternates the sign of the evaluated amplitude, so
+            // the +1.7e-8 mean error of MUFU.COS (measured) cannot add up coherently over the pairs
+            // (for single atoms it cancels by neutrality; sum of pair amplitudes is not neutral)
+            const uint32_t off = (((__float_as_uint(a.w) ^ Pq) >> 31) ? QUARTER_TURN : 0u) + ((uint32_t)e << 31);
+            arena[2 * e] = make_uint4(Px + dx, Py + dy, Pz + dz, off);
+            arena[2 * e + 1] = make_uint4(dx, dy, dz, __float_as_uint(2.0f * a.w));
+        } else if (single) {
+            const int e = (int)(base >> 16) + __popc(smask & lt_mask);
+            arena[T - 1 - e] = make_uint4(Sx, Sy, Sz, __float_as_uint(a.w));
+        }
+        __syncthreads();
+
+        // ---- accumulate: pair records g, g+ng, ... then single records g, g+ng, ...
+        int depth = 0;
+#pragma unroll 1
+        for (int e = g; e < np; e += p.ng) {
+            const uint4 ra = arena[2 * e];
+            const uint4 rd = arena[2 * e + 1];
+            const float w2 = __uint_as_float(rd.w);
+#pragma unroll
+            for (int r = 0; r < SF_KPT; ++r) {
+                const uint32_t pa = (uint32_t)mx[r] * ra.x + ((uint32_t)my[r] * ra.y + ((uint32_t)mz[r] * ra.z + ra.w));
+                const uint32_t pd = (uint32_t)mx[r] * rd.x + ((uint32_t)my[r] * rd.y + ((uint32_t)mz[r] * rd.z - ra.w));
+                const float xa = phase_to_arg(pa, K);
+                const float amp = w2 * fast_cos(phase_to_arg(pd, K));
+                c[r] = fmaf(amp, fast_cos(xa), c[r]);
+                s[r] = fmaf(amp, fast_sin(xa), s[r]);
+            }
+            if (DEEP) { depth += 2; if (depth >= SF_DEPTH) { sf_flush(acc, T, c, s); depth = 0; } }
+        }
+#pragma unroll 1
+        for (int e = g; e < ns; e += p.ng) {
+            const uint4 at = arena[T - 1 - e];
+            const float q = __uint_as_float(at.w);
+#pragma unroll
+            for (int r = 0; r < SF_KPT; ++r) {
+                const uint32_t ph = (uint32_t)mx[r] * at.x + ((uint32_t)my[r] * at.y + (uint32_t)mz[r] * at.z);
+                const float x = phase_to_arg(ph, K);
+                c[r] = fmaf(q, fast_cos(x), c[r]);
+                s[r] = fmaf(q, fast_sin(x), s[r]);
+            }
+            if (DEEP) { depth += 1; if (depth >= SF_DEPTH) { sf_flush(acc, T, c, s); depth = 0; } }
+        }
+        if (++since_flush >= p.flush_every) { sf_flush(acc, T, c, s); since_flush = 0; }
+    }
+    sf_flush(acc, T, c, s);
+
+    // let the dependent (force) kernel start launching; it waits for this grid's completion
+    grid_launch_dependents();
+
+    // combine the atom groups in group order, one fp64 row per CTA
+    const int kslots = p.gs * SF_KPT;
+    __syncthreads();
+    for (int idx = tid; idx < kslots; idx += T) {
+        const int k = blockIdx.y * kslots + idx;
+        if (k < p.P) {
+            double re = 0.0, im = 0.0;
+            for (int gg = 0; gg < p.ng; ++gg) {
+                const double2 v = acc_all[(idx % SF_KPT) * T + gg * p.gs + idx / SF_KPT];
+                re += v.x; im += v.y;
+            }
+            p.part[(int64_t)blockIdx.x * p.P + k] = make_double2(re, im);
+        }
+    }
+
+    // ---- the last CTA finalises (fixed summation order: independent of which CTA is last)
+    __threadfence();
+    __syncthreads();
+    if (tid == 0) s_last = (atomicInc(p.ticket, gridDim.x * gridDim.y - 1) == gridDim.x * gridDim.y - 1);
+    __syncthreads();
+    if (s_last) {
+        __threadfence();
+        fin_cta(p.fin, acc_all, tid, T);
+    }
+}
+
+// ---------------------------------------------------------------------------------------
 // F kernel -- Algorithm 1 step 4, Eq. (2.12) P:131.
 //
 // Mapping: a thread owns R atoms (coordinates as fixed-point turns in registers) and loops
 // over the wavevectors, whose {-m, theta} and {G, E} records are broadcast from shared memory.
-// Work is dealt to WARPS in units of 32 atoms, balanced over the whole grid, so that every
-// SM sub-partition gets the same number of (atom, k) pairs to within one unit.
-// Per pair: 3 IMAD (phase), I2F, 2 FMUL, 1 MUFU.SIN, 3 FFMA (+ MUFU.COS, FFMA with energy).
+// Work is dealt to WARPS in units of 32 atoms, balanced over the whole grid, and every warp
+// splits its run into equal passes of R <= 4 units, so that every SM sub-partition gets the
+// same number of (atom, k) pairs to within one unit.
+// Per pair: 3 IMAD (phase), I2FP, 2 FMUL, 1 MUFU.SIN, 3 FFMA (+ MUFU.COS, FFMA with energy).
 // ---------------------------------------------------------------------------------------
 struct FParams {
     const float4* xyzq;
@@ -268,14 +407,12 @@ struct FParams {
     const float4* kb;
     double two32_over_L;
     int32_t P;
+    int32_t pdl;   // launched with programmatic stream serialisation: wait before reading ka/kb
 };
 
-template <int R, bool ENERGY, bool ACCUM>
-__device__ __forceinline__ void f_units(const FParams& p, const int4* s_ka, const float4* s_kb,
-                                        int nk, int64_t unit0, int lane) {
-    uint32_t sx[R], sy[R], sz[R];
-    float q[R], fx[R], fy[R], fz[R], en[R];
-    const float K = phase_scale();
+template <int R, bool ENERGY>
+__device__ __forceinline__ void f_load(const FParams& p, int64_t unit0, int lane, uint32_t (&sx)[R], uint32_t (&sy)[R],
+                                       uint32_t (&sz)[R], float (&q)[R]) {
 #pragma unroll
     for (int r = 0; r < R; ++r) {
         const int64_t i = (unit0 + r) * 32 + lane;
@@ -285,16 +422,25 @@ __device__ __forceinline__ void f_units(const FParams& p, const int4* s_ka, cons
         sy[r] = to_turns(a.y, p.two32_over_L);
         sz[r] = to_turns(a.z, p.two32_over_L);
         q[r] = a.w;
-        fx[r] = fy[r] = fz[r] = en[r] = 0.f;
     }
-#pragma unroll 2
+}
+
+template <int R, bool ENERGY, bool ACCUM>
+__device__ __forceinline__ void f_units(const FParams& p, const int4* s_ka, const float4* s_kb, int nk, int64_t unit0,
+                                        int lane, const uint32_t (&sx)[R], const uint32_t (&sy)[R],
+                                        const uint32_t (&sz)[R], const float (&q)[R]) {
+    float fx[R], fy[R], fz[R], en[R];
+    const float K = phase_scale();
+#pragma unroll
+    for (int r = 0; r < R; ++r) fx[r] = fy[r] = fz[r] = en[r] = 0.f;
+#pragma unroll 4
     for (int k = 0; k < nk; ++k) {
         const int4 a = s_ka[k];
         const float4 b = s_kb[k];
 #pragma unroll
         for (int r = 0; r < R; ++r) {
             const uint32_t ph = (uint32_t)a.x * sx[r] + ((uint32_t)a.y * sy[r] + ((uint32_t)a.z * sz[r] + (uint32_t)a.w));
-            const float x = (float)(int32_t)ph * K;
+            const float x = phase_to_arg(ph, K);
             const float sn = fast_sin(x);
             fx[r] = fmaf(sn, b.x, fx[r]);
             fy[r] = fmaf(sn, b.y, fy[r]);
@@ -316,7 +462,31 @@ __device__ __forceinline__ void f_units(const FParams& p, const int4* s_ka, cons
     }
 }
 
-template <int R, bool ENERGY>
+template <int R, bool ENERGY, bool ACCUM>
+__device__ __forceinline__ void f_pass(const FParams& p, const int4* s_ka, const float4* s_kb, int nk, int64_t unit0, int lane) {
+    uint32_t sx[R], sy[R], sz[R];
+    float q[R];
+    f_load<R, ENERGY>(p, unit0, lane, sx, sy, sz, q);
+    f_units<R, ENERGY, ACCUM>(p, s_ka, s_kb, nk, unit0, lane, sx, sy, sz, q);
+}
+
+template <bool ENERGY, bool ACCUM>
+__device__ __forceinline__ void f_run(const FParams& p, const int4* s_ka, const float4* s_kb, int nk, int64_t u, int n, int lane) {
+    // n units in ceil(n / F_RMAX) passes of nearly equal size (e.g. 9 -> 3+3+3, not 4+4+1)
+    int passes = (n + F_RMAX - 1) / F_RMAX;
+    while (n > 0) {
+        const int r = (n + passes - 1) / passes;
+        switch (r) {
+            case 4: f_pass<4, ENERGY, ACCUM>(p, s_ka, s_kb, nk, u, lane); break;
+            case 3: f_pass<3, ENERGY, ACCUM>(p, s_ka, s_kb, nk, u, lane); break;
+            case 2: f_pass<2, ENERGY, ACCUM>(p, s_ka, s_kb, nk, u, lane); break;
+            default: f_pass<1, ENERGY, ACCUM>(p, s_ka, s_kb, nk, u, lane); break;
+        }
+        u += r; n -= r; --passes;
+    }
+}
+
+template <bool ENERGY>
 __global__ void __launch_bounds__(F_THREADS) f_kernel(const FParams p) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int nkmax = p.P < F_KCHUNK ? p.P : F_KCHUNK;
@@ -328,6 +498,8 @@ __global__ void __launch_bounds__(F_THREADS) f_kernel(const FParams p) {
     const int64_t units = (p.N + 31) / 32;
     const int64_t u0 = units * gw / nwarps, u1 = units * (gw + 1) / nwarps;
 
+    if (p.pdl) grid_dependency_wait();   // ka/kb come from the preceding grid
+
     for (int k0 = 0; k0 < p.P; k0 += F_KCHUNK) {
         const int nk = (p.P - k0 < F_KCHUNK) ? (p.P - k0) : F_KCHUNK;
         if (k0 > 0) __syncthreads();
@@ -336,14 +508,8 @@ __global__ void __launch_bounds__(F_THREADS) f_kernel(const FParams p) {
             s_kb[t] = p.kb[k0 + t];
         }
         __syncthreads();
-        int64_t u = u0;
-        if (k0 == 0) {
-            for (; u + R <= u1; u += R) f_units<R, ENERGY, false>(p, s_ka, s_kb, nk, u, lane);
-            for (; u < u1; ++u) f_units<1, ENERGY, false>(p, s_ka, s_kb, nk, u, lane);
-        } else {
-            for (; u + R <= u1; u += R) f_units<R, ENERGY, true>(p, s_ka, s_kb, nk, u, lane);
-            for (; u < u1; ++u) f_units<1, ENERGY, true>(p, s_ka, s_kb, nk, u, lane);
-        }
+        if (k0 == 0) f_run<ENERGY, false>(p, s_ka, s_kb, nk, u0, (int)(u1 - u0), lane);
+        else f_run<ENERGY, true>(p, s_ka, s_kb, nk, u0, (int)(u1 - u0), lane);
     }
 }
 
