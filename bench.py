@@ -4,7 +4,8 @@
     python bench.py [--gpus N] [--steps K] [--warmup W] [--config NAME] [--impl reference]
 
 One *step* = one pass of the whole hot path over one batch of synthetic input:
-rbe_set_kvectors (a fresh, pre-generated k-set) + rbe_structure_factor + rbe_forces.
+rbe_set_kvectors (a fresh, pre-generated k-set) + rbe_structure_factor (sf_kernel, which also
+runs the fixed-order second pass of the reduction) + rbe_forces (f_kernel): two launches.
 Workload at N = 1: BASELINE.json configs[2] (water + NaCl, N = 999 999, P = 200), the one the
 metric is quoted on.  With N > 1 GPUs (torchrun) the atoms are sharded, one rank per GPU, the
 k-set is replicated and the P complex structure factors are summed across ranks (weak
@@ -72,7 +73,7 @@ class ClockSampler:
             fd, self.path = tempfile.mkstemp(suffix=".csv")
             os.close(fd)
             self.proc = subprocess.Popen(
-                ["nvidia-smi", f"--id={self.idx}", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "50"],
+                ["nvidia-smi", f"--id={self.idx}", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "10"],
                 stdout=open(self.path, "w"), stderr=subprocess.DEVNULL)
         except Exception:
             self.proc = None
@@ -166,7 +167,8 @@ def main():
     ap.add_argument("--config", default="water_nacl_1m")
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--ref-atoms", type=int, default=100_000)
-    ap.add_argument("--cpu-baseline-atoms", type=int, default=500_000)
+    ap.add_argument("--cpu-baseline-atoms", type=int, default=1_000_000)
+    ap.add_argument("--cpu-baseline-steps", type=int, default=15)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--with-energy", action="store_true")
@@ -332,9 +334,10 @@ def main():
                    "parallelism": f"atoms sharded over {world} GPU(s), k-set replicated",
                    "launch": info, "with_energy": bool(args.with_energy)},
         "kernels_ms": {"structure_factor_call": ms_sf, "forces_call": ms_f,
-                       "note": "region B (CUDA events around each C-ABI call); structure_factor_call = sf_kernel + fin_kernel"},
+                       "note": "region B (CUDA events around each C-ABI call); structure_factor_call = sf_kernel "
+                               "(incl. its in-kernel second pass), forces_call = f_kernel"},
         "roofline": {
-            "bound": "alu", "kernel": "sf_kernel (+fin_kernel, timed together)",
+            "bound": "alu", "kernel": "sf_kernel",
             "achieved": sf_ops / (ms_sf * 1e-3) / 1e9, "peak": sfu_rate / 1e9, "unit": "G sincos-op/s (MUFU)",
             "frac": (sf_ops / (ms_sf * 1e-3)) / sfu_rate, "traffic": traffic,
             "peak_source": f"derived: {MUFU_LANES_PER_SM} MUFU lanes/SM/clk x {info['num_sms']} SMs x {peaks['sm_max_mhz']:.0f} MHz",
@@ -346,16 +349,18 @@ def main():
             "note": "SURVEY.md s8(d): 4 sincos + 13 FMA per (atom,k) pair per step, 48 B per atom",
         },
         "clocks": clocks,
-        "gpu_launches": 3 * args.steps,
+        "gpu_launches": 2 * args.steps,
         "paper_context": "8.20 ms/step, 1e6 atoms, A100, RBL+RBE nonbonded total, P=100 (PAPER.md P:284); 2.89 ms k-space at 1e5 atoms, P=200 (P:266)",
     }
     if e2e:
         out["e2e"] = e2e
     if not args.no_cpu_baseline and world == 1:
         n_s = min(args.cpu_baseline_atoms, base.N)
-        per_step, ns_cpu, cores, _ = time_oracle(args.config, n_s, 1, 0)
+        k_cpu = max(1, args.cpu_baseline_steps)
+        per_step, ns_cpu, cores, _ = time_oracle(args.config, n_s, k_cpu, 1)
         out["cpu_baseline"] = {"value": ns_cpu, "unit": UNIT, "cores": cores, "kind": "oracle",
-                               "sample": f"first {n_s} atoms of {base.name}, all P={P} wavevectors, oracle.rho + oracle.force, 1 step ({per_step:.1f} s)"}
+                               "sample": f"first {n_s} atoms of {base.name} (N={base.N}), all P={P} wavevectors, oracle.rho + "
+                                         f"oracle.force, {k_cpu} steps after 1 warm-up ({per_step * k_cpu:.1f} s of CPU work)"}
     print(json.dumps(out))
     if world > 1:
         dist.destroy_process_group()

@@ -64,7 +64,7 @@ typedef struct {
     int32_t num_sms;
     int32_t sf_grid_x, sf_grid_y, sf_threads, sf_smem_bytes; /* structure-factor kernel */
     int32_t sf_k_per_thread, sf_atom_groups, sf_tile_atoms;
-    int32_t fin_grid, fin_threads;                           /* fixed-order finalise kernel */
+    int32_t sf_red_group, sf_red_groups;                     /* in-kernel two-level fixed-order reduction */
     int32_t f_grid, f_threads, f_smem_bytes, f_atoms_per_thread; /* force kernel */
 } rbe_launch_info;
 
@@ -81,7 +81,7 @@ rbe_status rbe_destroy(rbe_ctx* ctx);
 /* The paper's normalisation constant Q == S for this context's L and alpha. */
 double rbe_normaliser_S(const rbe_ctx* ctx);
 
-/* Bytes of device scratch the context needs (per-CTA fp64 partials, rho, per-k tables).
+/* Bytes of device scratch the context needs (per-CTA fp64 partials, rho, the k-set).
  * Queries the current CUDA device on first use.  Returns 0 on error (see rbe_last_error). */
 size_t rbe_workspace_bytes(rbe_ctx* ctx);
 
@@ -89,6 +89,16 @@ size_t rbe_workspace_bytes(rbe_ctx* ctx);
  * allocated on the current CUDA device.  Caller keeps ownership and must keep it alive.
  * Errors: RBE_ERR_WORKSPACE, RBE_ERR_NO_DEVICE, RBE_ERR_CUDA. */
 rbe_status rbe_set_workspace(rbe_ctx* ctx, void* d_ws, size_t bytes);
+
+/* How the structure-factor kernel may combine atoms (default 3).  For two atoms with q_2 = +-q_1
+ * the kernel evaluates q_1 e^{i phi_1} + q_2 e^{i phi_2} = 2 q_1 cos(d) e^{i a} (a, d = half sum and
+ * half difference of the phases; a quarter-turn offset for opposite signs): 3 special-function
+ * evaluations for two (atom, k) pairs instead of 4.  Atoms are matched by the bit pattern of |q|
+ * inside windows of 32 consecutive atoms; unmatched atoms, and every atom when mode = 0, take the
+ * plain path, so any charge assignment is handled and the result is the same sum (to rounding).
+ *   mode 0: never pair;  1: pair equal charges only;  3: pair equal and opposite charges.
+ * Errors: RBE_ERR_INVALID_ARG. */
+rbe_status rbe_set_pairing(rbe_ctx* ctx, int32_t mode);
 
 /* Fill *out with the launch geometry chosen for this context (valid after rbe_set_workspace). */
 rbe_status rbe_get_launch_info(const rbe_ctx* ctx, rbe_launch_info* out);
@@ -108,13 +118,12 @@ rbe_status rbe_set_kvectors(rbe_ctx* ctx, const int32_t* h_m, const double* h_w,
  *   d_xyzq  float4 [N] = {x, y, z, q} (AoS), device.
  *   d_rho   double2 [P] = {Re, Im}, device, or NULL if the caller does not want a copy.
  * fp32 phases from 32-bit fixed-point fractional coordinates (m . s mod 1 is exact), fp32
- * sincos, fp32 partial sums over at most 64 atoms, fp64 above that; per-CTA fp64 partials
- * summed in a fixed order by a second kernel.
+ * sincos, fp32 partial sums over at most ~64 atoms, fp64 above that; per-CTA fp64 partials
+ * summed in a fixed order (two-level tree) by the last CTAs of the same launch.
  * Errors: RBE_ERR_NOT_READY, RBE_ERR_INVALID_ARG, RBE_ERR_CUDA. */
 rbe_status rbe_structure_factor(rbe_ctx* ctx, const void* d_xyzq, void* d_rho, void* stream);
 
-/* Replace the context's structure factors by d_rho (double2 [P], device) and rebuild the
- * force coefficients.  This is the multi-GPU exchange point: each rank computes rho over its
+/* Replace the context's structure factors by d_rho (double2 [P], device; copied).  This is the multi-GPU exchange point: each rank computes rho over its
  * own atoms, the ranks sum the P complex numbers (rank order), and each rank injects the
  * global sum here before rbe_forces.  Requires rbe_set_kvectors.
  * Errors: RBE_ERR_NOT_READY, RBE_ERR_INVALID_ARG, RBE_ERR_CUDA. */

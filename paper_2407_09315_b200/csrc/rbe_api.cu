@@ -4,7 +4,6 @@
 
 #include <cmath>
 #include <cstdio>
-#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <string>
@@ -28,11 +27,12 @@ struct rbe_ctx {
     bool dev_ready = false;
     int device = -1;
     rbe_launch_info li{};
-    int sf_gs = 0, sf_ng = 0, sf_flush_every = 1;
+    int sf_gs = 0, sf_ng = 0, sf_flush_every = 1, sf_tile = 0;
     int sf_pairing = 3;
+    int sf_ngroups = 1;
     bool sf_deep = false;   // a group takes more than SF_DEPTH atoms from one tile: flush inside the loops
     size_t ws_bytes = 0;
-    size_t off_kvec = 0, off_w = 0, off_part = 0, off_rho = 0, off_ka = 0, off_kb = 0, off_uk = 0, off_U = 0, off_ticket = 0;
+    size_t off_kvec = 0, off_w = 0, off_part = 0, off_rho = 0, off_grow = 0, off_U = 0, off_ticket = 0;
 
     // workspace
     unsigned char* ws = nullptr;
@@ -104,22 +104,30 @@ rbe_status init_device(rbe_ctx* c) {
     int ng = rbe::SF_TMAX / gs;
     if (ng < 1) ng = 1;
     int threads = (int)align_up((size_t)gs * ng, 32);
-    int gx = li.num_sms / gy;
+    int gx = rbe::SF_CTAS_PER_SM * li.num_sms / gy;
     if (gx < 1) gx = 1;
     // never more CTAs than 32-atom windows to feed them
     const int64_t max_gx = c->N > 0 ? (c->N + 31) / 32 : 1;
     if ((int64_t)gx > max_gx) gx = (int)max_gx;
-    const int per_group = (threads + ng - 1) / ng;   // atoms a group takes from one tile
-    c->sf_gs = gs; c->sf_ng = ng;
+    // tile: up to 4 windows of 32 atoms per warp (amortises the staging barriers), but no more than
+    // one CTA's share of the atoms needs
+    int64_t share = c->N > 0 ? ((c->N + gx - 1) / gx + 31) / 32 * 32 : 32;
+    int tile = 4 * threads;
+    if (tile > rbe::SF_TILE_MAX) tile = rbe::SF_TILE_MAX;
+    if ((int64_t)tile > share) tile = (int)share;
+    if (tile < 32) tile = 32;
+    const int per_group = (tile + ng - 1) / ng;   // atoms a group takes from one tile
+    c->sf_gs = gs; c->sf_ng = ng; c->sf_tile = tile;
     c->sf_flush_every = per_group >= rbe::SF_DEPTH ? 1 : rbe::SF_DEPTH / per_group;
     c->sf_deep = per_group + 1 > rbe::SF_DEPTH;
     li.sf_grid_x = gx; li.sf_grid_y = gy; li.sf_threads = threads;
-    li.sf_k_per_thread = rbe::SF_KPT; li.sf_atom_groups = ng; li.sf_tile_atoms = threads;
+    li.sf_k_per_thread = rbe::SF_KPT; li.sf_atom_groups = ng; li.sf_tile_atoms = tile;
     // raw tile + record arena (16 B per atom each) + fp64 accumulators [SF_KPT][threads]
-    li.sf_smem_bytes = (int32_t)((size_t)threads * (2 * sizeof(uint4) + rbe::SF_KPT * sizeof(double2)));
+    li.sf_smem_bytes = (int32_t)((size_t)tile * 2 * sizeof(uint4) + (size_t)threads * rbe::SF_KPT * sizeof(double2));
 
-    li.fin_grid = (c->P + rbe::FIN_KB - 1) / rbe::FIN_KB;
-    li.fin_threads = rbe::FIN_KB * rbe::FIN_SL;
+    c->sf_ngroups = (gx + rbe::SF_RED_GROUP - 1) / rbe::SF_RED_GROUP;
+    li.sf_red_group = rbe::SF_RED_GROUP;
+    li.sf_red_groups = c->sf_ngroups;
 
     // ---- F kernel: warps take balanced runs of 32-atom units; one wave of CTAs.
     li.f_threads = rbe::F_THREADS;
@@ -150,11 +158,9 @@ rbe_status init_device(rbe_ctx* c) {
     c->off_w = off;    off = align_up(off + P * sizeof(double), 256);
     c->off_part = off; off = align_up(off + (size_t)gx * P * sizeof(double2), 256);
     c->off_rho = off;  off = align_up(off + P * sizeof(double2), 256);
-    c->off_ka = off;   off = align_up(off + P * sizeof(int4), 256);
-    c->off_kb = off;   off = align_up(off + P * sizeof(float4), 256);
-    c->off_uk = off;   off = align_up(off + P * sizeof(double), 256);
+    c->off_grow = off; off = align_up(off + (size_t)c->sf_ngroups * P * sizeof(double2), 256);
     c->off_U = off;    off = align_up(off + sizeof(double), 256);
-    c->off_ticket = off; off = align_up(off + sizeof(unsigned int), 256);
+    c->off_ticket = off; off = align_up(off + (size_t)(c->sf_ngroups + 1) * sizeof(unsigned int), 256);
     c->ws_bytes = off;
 
     c->stage_bytes = P * (sizeof(int4) + sizeof(double));
@@ -165,27 +171,14 @@ rbe_status init_device(rbe_ctx* c) {
 template <typename T>
 T* ws_ptr(rbe_ctx* c, size_t off) { return reinterpret_cast<T*>(c->ws + off); }
 
-rbe::FinParams fin_params(rbe_ctx* c, const double2* part, int nrows, double2* rho_user) {
-    rbe::FinParams fp;
-    fp.part = part; fp.nrows = nrows; fp.P = c->P;
-    fp.kvec = ws_ptr<int4>(c, c->off_kvec);
-    fp.w = c->have_w ? ws_ptr<double>(c, c->off_w) : nullptr;
-    fp.w_uniform = c->S / (double)c->P;
-    fp.L = c->L;
-    fp.rho = ws_ptr<double2>(c, c->off_rho);
-    fp.rho_user = rho_user;
-    fp.ka = ws_ptr<int4>(c, c->off_ka);
-    fp.kb = ws_ptr<float4>(c, c->off_kb);
-    fp.uk = ws_ptr<double>(c, c->off_uk);
-    return fp;
-}
-
-rbe_status launch_fin(rbe_ctx* c, const double2* part, int nrows, double2* rho_user, cudaStream_t st) {
-    const rbe::FinParams fp = fin_params(c, part, nrows, rho_user);
-    rbe::fin_kernel<<<c->li.fin_grid, c->li.fin_threads, 0, st>>>(fp);
-    RBE_CUDA(c, cudaGetLastError());
-    c->have_rho = true;
-    return RBE_OK;
+rbe::KTable k_table(rbe_ctx* c) {
+    rbe::KTable t;
+    t.kvec = ws_ptr<int4>(c, c->off_kvec);
+    t.w = c->have_w ? ws_ptr<double>(c, c->off_w) : nullptr;
+    t.rho = ws_ptr<double2>(c, c->off_rho);
+    t.w_uniform = c->S / (double)c->P;
+    t.L = c->L;
+    return t;
 }
 
 }  // namespace
@@ -202,7 +195,6 @@ rbe_status rbe_create(rbe_ctx** out, int64_t N, double L, double alpha, int32_t 
     if (!c) return RBE_ERR_INVALID_ARG;
     c->N = N; c->L = L; c->alpha = alpha; c->P = P;
     c->S = normaliser_S(L, alpha);
-    if (const char* e = std::getenv("RBE_SF_PAIRING")) c->sf_pairing = std::atoi(e);
     *out = c;
     return RBE_OK;
 }
@@ -235,8 +227,15 @@ rbe_status rbe_set_workspace(rbe_ctx* c, void* d_ws, size_t bytes) {
     c->ws = static_cast<unsigned char*>(d_ws);
     c->have_k = c->have_w = c->have_rho = false;
     // the structure-factor kernel's completion ticket starts at zero and resets itself
-    RBE_CUDA(c, cudaMemset(c->ws + c->off_ticket, 0, sizeof(unsigned int)));
+    RBE_CUDA(c, cudaMemset(c->ws + c->off_ticket, 0, (size_t)(c->sf_ngroups + 1) * sizeof(unsigned int)));
     RBE_CUDA(c, cudaDeviceSynchronize());
+    return RBE_OK;
+}
+
+rbe_status rbe_set_pairing(rbe_ctx* c, int32_t mode) {
+    if (!c) return RBE_ERR_INVALID_ARG;
+    if (mode != 0 && mode != 1 && mode != 3) return fail(c, RBE_ERR_INVALID_ARG, "rbe_set_pairing: mode must be 0, 1 or 3");
+    c->sf_pairing = mode;
     return RBE_OK;
 }
 
@@ -297,11 +296,16 @@ rbe_status rbe_structure_factor(rbe_ctx* c, const void* d_xyzq, void* d_rho, voi
     sp.kvec = ws_ptr<int4>(c, c->off_kvec);
     sp.part = ws_ptr<double2>(c, c->off_part);
     sp.two32_over_L = rbe::TWO32 / c->L;
-    sp.P = c->P; sp.gs = c->sf_gs; sp.ng = c->sf_ng; sp.flush_every = c->sf_flush_every;
+    sp.P = c->P; sp.gs = c->sf_gs; sp.ng = c->sf_ng; sp.flush_every = c->sf_flush_every; sp.tile_atoms = c->sf_tile;
     sp.pairing = c->sf_pairing;
-    sp.ticket = ws_ptr<unsigned int>(c, c->off_ticket);
-    // the last CTA to finish runs the fixed-order finalise: no second launch on the hot path
-    sp.fin = fin_params(c, sp.part, c->li.sf_grid_x, static_cast<double2*>(d_rho));
+    // second pass (fixed-order two-level sum of the per-CTA rows) runs inside the same launch
+    sp.red.part = sp.part;
+    sp.red.grow = ws_ptr<double2>(c, c->off_grow);
+    sp.red.rho = ws_ptr<double2>(c, c->off_rho);
+    sp.red.rho_user = static_cast<double2*>(d_rho);
+    sp.red.tickets = ws_ptr<unsigned int>(c, c->off_ticket);
+    sp.red.group_size = rbe::SF_RED_GROUP;
+    sp.red.ngroups = c->sf_ngroups;
     dim3 grid(c->li.sf_grid_x, c->li.sf_grid_y);
     if (c->sf_deep) rbe::sf_kernel<true><<<grid, c->li.sf_threads, c->li.sf_smem_bytes, st>>>(sp);
     else rbe::sf_kernel<false><<<grid, c->li.sf_threads, c->li.sf_smem_bytes, st>>>(sp);
@@ -315,7 +319,10 @@ rbe_status rbe_set_rho(rbe_ctx* c, const void* d_rho, void* stream) {
     if (!c->ws || !c->have_k) return fail(c, RBE_ERR_NOT_READY, "rbe_set_rho needs a workspace and k-vectors");
     if (!d_rho || (reinterpret_cast<uintptr_t>(d_rho) & 15u))
         return fail(c, RBE_ERR_INVALID_ARG, "rbe_set_rho: null or misaligned pointer");
-    return launch_fin(c, static_cast<const double2*>(d_rho), 1, nullptr, static_cast<cudaStream_t>(stream));
+    RBE_CUDA(c, cudaMemcpyAsync(c->ws + c->off_rho, d_rho, (size_t)c->P * sizeof(double2), cudaMemcpyDeviceToDevice,
+                                static_cast<cudaStream_t>(stream)));
+    c->have_rho = true;
+    return RBE_OK;
 }
 
 rbe_status rbe_forces(rbe_ctx* c, const void* d_xyzq, void* d_force, int32_t with_energy, void* stream) {
@@ -330,8 +337,7 @@ rbe_status rbe_forces(rbe_ctx* c, const void* d_xyzq, void* d_force, int32_t wit
     fp.xyzq = static_cast<const float4*>(d_xyzq);
     fp.force = static_cast<float4*>(d_force);
     fp.N = c->N;
-    fp.ka = ws_ptr<int4>(c, c->off_ka);
-    fp.kb = ws_ptr<float4>(c, c->off_kb);
+    fp.kt = k_table(c);
     fp.two32_over_L = rbe::TWO32 / c->L;
     fp.P = c->P;
     fp.pdl = 1;
@@ -358,7 +364,7 @@ rbe_status rbe_kspace_energy(rbe_ctx* c, double* h_U, void* stream) {
     if (!c->ws || !c->have_k || !c->have_rho) return fail(c, RBE_ERR_NOT_READY, "rbe_kspace_energy needs a structure factor");
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     if (!c->h_U_pinned) RBE_CUDA(c, cudaMallocHost(reinterpret_cast<void**>(&c->h_U_pinned), sizeof(double)));
-    rbe::energy_kernel<<<1, 256, 0, st>>>(ws_ptr<double>(c, c->off_uk), c->P, ws_ptr<double>(c, c->off_U));
+    rbe::energy_kernel<<<1, 256, 0, st>>>(k_table(c), c->P, ws_ptr<double>(c, c->off_U));
     RBE_CUDA(c, cudaGetLastError());
     RBE_CUDA(c, cudaMemcpyAsync(c->h_U_pinned, c->ws + c->off_U, sizeof(double), cudaMemcpyDeviceToHost, st));
     RBE_CUDA(c, cudaStreamSynchronize(st));

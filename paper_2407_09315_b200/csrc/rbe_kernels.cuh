@@ -23,13 +23,14 @@ namespace rbe {
 // tunables (compile time)
 // ---------------------------------------------------------------------------------------
 constexpr int SF_KPT = 4;        // wavevectors owned by one thread of the structure-factor kernel
-constexpr int SF_TMAX = 1024;    // max threads per CTA (structure-factor kernel): 1 CTA/SM, <= 64 regs
+constexpr int SF_TMAX = 1024;    // max threads per CTA (structure-factor kernel): <= 64 registers
+constexpr int SF_CTAS_PER_SM = 1;
+constexpr int SF_TILE_MAX = 4096; // max atoms staged in shared memory at a time (structure-factor kernel)
 constexpr int SF_DEPTH = 64;     // max atoms a thread accumulates in fp32 before the fp64 flush
 constexpr int F_THREADS = 256;   // threads per CTA (force kernel)
 constexpr int F_RMAX = 4;        // max atoms per thread per pass (force kernel)
 constexpr int F_KCHUNK = 2048;   // wavevectors staged in shared memory at a time (force kernel)
-constexpr int FIN_KB = 32;       // wavevectors per CTA (stand-alone finalise kernel)
-constexpr int FIN_SL = 32;       // row slices per wavevector (stand-alone finalise kernel)
+constexpr int SF_RED_GROUP = 16; // CTAs per group in the two-level reduction of the per-CTA rows
 
 constexpr double TWO32 = 4294967296.0;
 constexpr double MAGIC = 6755399441055744.0;  // 2^52 + 2^51: low word of (d + MAGIC) = rint(d) mod 2^32
@@ -70,101 +71,50 @@ __device__ __forceinline__ void grid_dependency_wait() { asm volatile("griddepco
 __device__ __forceinline__ void grid_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
 
 // ---------------------------------------------------------------------------------------
-// Finalise: second pass of the reduction and the per-k force coefficients.
+// Per-k force coefficients, computed in fp64 from the reduced rho.
 //
-// rho_l = sum over the SF kernel's per-CTA rows in a FIXED order (row slices sl, sl+nsl, ...
-// summed sequentially, then the nsl slice sums sequentially), so rho is bitwise reproducible.
-// Then, with w_l the sample weight (S/P of Eq. 2.12 unless the caller gave weights):
+// With w_l the sample weight (S/P of Eq. 2.12 unless the caller gave weights):
 //   Im(e^{-i phi} rho) = |rho| sin(theta - phi),  theta = arg rho,
 // so Eq. (2.12) becomes  F_i = q_i sum_l G_l sin(2 pi (theta_l - m_l . s_i))  with
 //   G_l = -(4 pi w_l / V) (k_l / k_l^2) |rho_l| = -(2 w_l / L^2) (m_l / |m_l|^2) |rho_l|
 // and the force kernel needs ONE special-function evaluation per (atom, k) instead of two.
 // Energy weights (2nd term of Eq. 2.8): e_l = (2 pi w_l / V) / k_l^2 = w_l / (2 pi L |m_l|^2).
+// Every force CTA builds the records for its shared-memory tile itself (a few hundred fp64
+// operations per k, in parallel over the CTAs), so the serial tail of the structure-factor
+// kernel is only the reduction.
 // ---------------------------------------------------------------------------------------
-struct FinParams {
-    const double2* part;  // [nrows][P] (nrows = 1 and part = caller's rho for rbe_set_rho)
-    int32_t nrows;
-    int32_t P;
-    const int4* kvec;     // [P]
+struct KTable {
+    const int4* kvec;     // [P] {mx, my, mz, 0}
     const double* w;      // [P] or nullptr -> w_uniform
+    const double2* rho;   // [P]
     double w_uniform;     // S / P
     double L;
-    double2* rho;         // [P] out
-    double2* rho_user;    // [P] out, or nullptr
-    int4* ka;             // [P] out {-mx, -my, -mz, theta in 2^-32 turns}
-    float4* kb;           // [P] out {Gx, Gy, Gz, E = e_l |rho_l|}
-    double* uk;           // [P] out e_l |rho_l|^2
 };
 
-__device__ __forceinline__ void fin_coefficients(const FinParams& p, int k, double re, double im) {
-    const int4 m = p.kvec[k];
-    const double w = p.w ? p.w[k] : p.w_uniform;
+__device__ __forceinline__ void k_record(const KTable& t, int k, int4& ka, float4& kb) {
+    const int4 m = t.kvec[k];
+    const double2 r = t.rho[k];
+    const double w = t.w ? t.w[k] : t.w_uniform;
     const double m2 = (double)m.x * m.x + (double)m.y * m.y + (double)m.z * m.z;
-    const double mag = sqrt(re * re + im * im);
-    const double theta = atan2(im, re) * (1.0 / (2.0 * PI_D));        // turns, [-1/2, 1/2]
-    const double gs = -2.0 * w / (p.L * p.L * m2) * mag;
-    const double el = w / (2.0 * PI_D * p.L * m2);
-    p.rho[k] = make_double2(re, im);
-    if (p.rho_user) p.rho_user[k] = make_double2(re, im);
-    p.ka[k] = make_int4(-m.x, -m.y, -m.z, __double2loint(fma(theta, TWO32, MAGIC)));
-    p.kb[k] = make_float4((float)(gs * m.x), (float)(gs * m.y), (float)(gs * m.z), (float)(el * mag));
-    p.uk[k] = el * mag * mag;
+    const double mag = sqrt(r.x * r.x + r.y * r.y);
+    const double theta = atan2(r.y, r.x) * (1.0 / (2.0 * PI_D));      // turns, [-1/2, 1/2]
+    const double gs = -2.0 * w / (t.L * t.L * m2) * mag;
+    const double el = w / (2.0 * PI_D * t.L * m2);
+    ka = make_int4(-m.x, -m.y, -m.z, __double2loint(fma(theta, TWO32, MAGIC)));   // {-m, theta in 2^-32 turns}
+    kb = make_float4((float)(gs * m.x), (float)(gs * m.y), (float)(gs * m.z), (float)(el * mag));  // {G, e_l |rho_l|}
 }
 
-// One CTA of `nt` threads finalises all P wavevectors; `scratch` holds nt double2.
-// Used by the LAST structure-factor CTA to finish (no separate launch on the hot path).
-__device__ __forceinline__ void fin_cta(const FinParams& p, double2* scratch, int tid, int nt) {
-    const int kc = p.P < nt ? p.P : nt;   // wavevectors per chunk
-    const int nsl = nt / kc;              // row slices per wavevector (>= 1)
-    const int kk = tid % kc, sl = tid / kc;
-    for (int k0 = 0; k0 < p.P; k0 += kc) {
-        const int k = k0 + kk;
-        double re = 0.0, im = 0.0;
-        if (sl < nsl && k < p.P) {
-#pragma unroll 8
-            for (int row = sl; row < p.nrows; row += nsl) {
-                const double2 v = __ldcg(&p.part[(int64_t)row * p.P + k]);
-                re += v.x; im += v.y;
-            }
-        }
-        if (sl < nsl) scratch[sl * kc + kk] = make_double2(re, im);
-        __syncthreads();
-        if (sl == 0 && k < p.P) {
-            re = 0.0; im = 0.0;
-#pragma unroll 1
-            for (int t = 0; t < nsl; ++t) { re += scratch[t * kc + kk].x; im += scratch[t * kc + kk].y; }
-            fin_coefficients(p, k, re, im);
-        }
-        __syncthreads();
-    }
-}
-
-// Stand-alone finalise (rbe_set_rho: the multi-GPU exchange point injects a global rho).
-__global__ void __launch_bounds__(FIN_KB * FIN_SL) fin_kernel(const FinParams p) {
-    __shared__ double2 sl_sum[FIN_SL][FIN_KB];
-    const int kk = threadIdx.x % FIN_KB, sl = threadIdx.x / FIN_KB;
-    const int k = blockIdx.x * FIN_KB + kk;
-    double re = 0.0, im = 0.0;
-    if (k < p.P) {
-        for (int row = sl; row < p.nrows; row += FIN_SL) {
-            const double2 v = p.part[(int64_t)row * p.P + k];
-            re += v.x; im += v.y;
-        }
-    }
-    sl_sum[sl][kk] = make_double2(re, im);
-    __syncthreads();
-    if (sl != 0 || k >= p.P) return;
-    re = 0.0; im = 0.0;
-#pragma unroll 1
-    for (int t = 0; t < FIN_SL; ++t) { re += sl_sum[t][kk].x; im += sl_sum[t][kk].y; }
-    fin_coefficients(p, k, re, im);
-}
-
-// U = sum_l uk[l] in a fixed order (thread-strided partials, then a fixed tree).
-__global__ void __launch_bounds__(256) energy_kernel(const double* uk, int32_t P, double* U) {
+// U = sum_l e_l |rho_l|^2 in a fixed order (thread-strided partials, then a fixed tree).
+__global__ void __launch_bounds__(256) energy_kernel(const KTable t, int32_t P, double* U) {
     __shared__ double sh[256];
     double a = 0.0;
-    for (int k = threadIdx.x; k < P; k += 256) a += uk[k];
+    for (int k = threadIdx.x; k < P; k += 256) {
+        const int4 m = t.kvec[k];
+        const double2 r = t.rho[k];
+        const double w = t.w ? t.w[k] : t.w_uniform;
+        const double m2 = (double)m.x * m.x + (double)m.y * m.y + (double)m.z * m.z;
+        a += w / (2.0 * PI_D * t.L * m2) * (r.x * r.x + r.y * r.y);
+    }
     sh[threadIdx.x] = a;
     __syncthreads();
     for (int s = 128; s > 0; s >>= 1) {
@@ -172,6 +122,53 @@ __global__ void __launch_bounds__(256) energy_kernel(const double* uk, int32_t P
         __syncthreads();
     }
     if (threadIdx.x == 0) *U = sh[0];
+}
+
+// ---------------------------------------------------------------------------------------
+// Second pass of the structure-factor reduction, inside the SF kernel (no extra launch).
+//
+// The per-CTA rows are summed in a FIXED order by a two-level tree: CTAs form groups of
+// `group_size` consecutive blockIdx.x; the last CTA of a group to finish (atomicInc ticket)
+// sums that group's rows into one group row, and the last group to finish sums the group
+// rows into rho.  Which CTA does the summing depends on timing; the order of the additions
+// does not, so rho is bitwise reproducible.  Tickets wrap to zero by themselves.
+// ---------------------------------------------------------------------------------------
+struct RedParams {
+    double2* part;        // [gridDim.x][P] per-CTA rows
+    double2* grow;        // [ngroups][P] group rows
+    double2* rho;         // [P] out
+    double2* rho_user;    // [P] out, or nullptr
+    unsigned int* tickets;  // [ngroups + 1], zero-initialised
+    int32_t group_size, ngroups;
+};
+
+// dst[k] = sum_{row} src[row][k]: row slices sl, sl+nsl, ... sequentially, then the slices in order
+__device__ __forceinline__ void reduce_rows(const double2* src, int nrows, int P, double2* dst, double2* dst2,
+                                            double2* scratch, int tid, int nt) {
+    const int kc = P < nt ? P : nt;       // wavevectors per chunk
+    const int nsl = nt / kc;              // row slices per wavevector (>= 1)
+    const int kk = tid % kc, sl = tid / kc;
+    for (int k0 = 0; k0 < P; k0 += kc) {
+        const int k = k0 + kk;
+        double re = 0.0, im = 0.0;
+        if (sl < nsl && k < P) {
+#pragma unroll 8
+            for (int row = sl; row < nrows; row += nsl) {
+                const double2 v = __ldcg(&src[(int64_t)row * P + k]);
+                re += v.x; im += v.y;
+            }
+        }
+        if (sl < nsl) scratch[sl * kc + kk] = make_double2(re, im);
+        __syncthreads();
+        if (sl == 0 && k < P) {
+            re = 0.0; im = 0.0;
+#pragma unroll 1
+            for (int t = 0; t < nsl; ++t) { re += scratch[t * kc + kk].x; im += scratch[t * kc + kk].y; }
+            dst[k] = make_double2(re, im);
+            if (dst2) dst2[k] = make_double2(re, im);
+        }
+        __syncthreads();
+    }
 }
 
 // ---------------------------------------------------------------------------------------
@@ -207,10 +204,10 @@ struct SfParams {
     int32_t P;
     int32_t gs;        // threads per atom group in this CTA = k-slots / SF_KPT
     int32_t ng;        // atom groups per CTA
+    int32_t tile_atoms;   // atoms staged per tile: a multiple of 32, <= SF_TILE_MAX
     int32_t flush_every;  // tiles between fp64 flushes (keeps the fp32 depth <= ~SF_DEPTH atoms)
     int32_t pairing;      // bit 0: pair equal charges, bit 1: pair opposite charges (3 = both)
-    unsigned int* ticket;  // zero-initialised, self-resetting (atomicInc wraps)
-    FinParams fin;
+    RedParams red;
 };
 
 // acc points at this thread's slot of component 0; component r lives `stride` entries further
@@ -225,14 +222,44 @@ __device__ __forceinline__ void sf_flush(double2* acc, int stride, float (&c)[SF
     }
 }
 
+// Classification of one 32-atom window (lane = atom) by charge: `leader` lanes own a pair record
+// (with the next lane of equal |q|, `partner`), `single` lanes a single record.
+struct SfWindow {
+    uint32_t lmask, smask;
+    int partner;
+    bool leader, single;
+};
+__device__ __forceinline__ SfWindow sf_classify(uint32_t qbits, bool in_range, int pairing, int lane) {
+    SfWindow w;
+    const uint32_t key = qbits & ((pairing & 3) == 3 ? 0x7fffffffu : 0xffffffffu);
+    const bool valid = in_range && (qbits & 0x7fffffffu) != 0u;   // zero charges contribute nothing: dropped
+    const uint32_t vmask = __ballot_sync(FULL_MASK, valid);
+    const uint32_t peers = (pairing & 3) ? (__match_any_sync(FULL_MASK, key) & vmask) : (valid ? 1u << lane : 0u);
+    const int rank = __popc(peers & ((1u << lane) - 1u));
+    const uint32_t higher = (peers >> lane) >> 1;                  // peers above this lane
+    w.leader = valid && !(rank & 1) && higher != 0u;
+    w.single = valid && !(rank & 1) && higher == 0u;
+    w.lmask = __ballot_sync(FULL_MASK, w.leader);
+    w.smask = __ballot_sync(FULL_MASK, w.single);
+    w.partner = w.leader ? lane + __ffs(higher) : lane;
+    return w;
+}
+__device__ __forceinline__ uint32_t warp_sum(uint32_t v) {
+#pragma unroll
+    for (int d = 16; d > 0; d >>= 1) v += __shfl_xor_sync(FULL_MASK, v, d);
+    return v;
+}
+
 template <bool DEEP>
-__global__ void __launch_bounds__(SF_TMAX, 1) sf_kernel(const SfParams p) {
+__global__ void __launch_bounds__(SF_TMAX, SF_CTAS_PER_SM) sf_kernel(const SfParams p) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int tid = threadIdx.x, T = blockDim.x, lane = tid & 31, warp = tid >> 5, nwarps = T >> 5;
-    float4* raw = reinterpret_cast<float4*>(smem_raw);               // [T] raw atom records of the tile
-    uint4* arena = reinterpret_cast<uint4*>(smem_raw) + T;           // [T] pair records from the front, singles from the back
-    double2* acc_all = reinterpret_cast<double2*>(arena + T);        // [SF_KPT][T] fp64 accumulators
-    __shared__ uint32_t wcount[SF_TMAX / 32];
+    const int TA = p.tile_atoms;                                      // multiple of 32, <= SF_TILE_MAX
+    float4* raw = reinterpret_cast<float4*>(smem_raw);               // [TA] raw atom records of the tile
+    uint4* arena = reinterpret_cast<uint4*>(smem_raw) + TA;          // [TA] pair records from the front, singles from the back
+    double2* acc_all = reinterpret_cast<double2*>(arena + TA);       // [SF_KPT][T] fp64 accumulators
+    __shared__ uint32_t wcount[SF_TILE_MAX / 32], wbase[SF_TILE_MAX / 32 + 1];
+    __shared__ uint16_t roles[SF_TILE_MAX];
     __shared__ uint32_t s_last;
 
     const bool active = tid < p.gs * p.ng;
@@ -260,70 +287,85 @@ __global__ void __launch_bounds__(SF_TMAX, 1) sf_kernel(const SfParams p) {
     const float K = phase_scale();
     const uint32_t lt_mask = (1u << lane) - 1u;
 
-    if (lo + tid < hi) cp_async16(&raw[tid], &p.xyzq[lo + tid]);
+    // a short first tile gets the MUFU-bound loop going early; later tiles are full size
+    int tl = (TA >> 7) << 5;
+    if (tl < 32) tl = 32;
+    for (int i = tid; i < tl && lo + i < hi; i += T) cp_async16(&raw[i], &p.xyzq[lo + i]);
     int since_flush = 0;
 
-    for (int64_t t0 = lo; t0 < hi; t0 += T) {
-        const int cnt = (int)((hi - t0 < T) ? (hi - t0) : T);
+    for (int64_t t0 = lo; t0 < hi; t0 += tl, tl = TA) {
+        const int cnt = (int)((hi - t0 < tl) ? (hi - t0) : tl);
+        const int nwin = (cnt + 31) >> 5;
         cp_async_wait_all();
         __syncthreads();  // raw holds the tile; everyone is done with the previous arena
 
-        // ---- stage: window = this warp's 32 atoms; match equal |q|, convert to turns
-        const bool in_range = tid < cnt;
-        const float4 a = in_range ? raw[tid] : make_float4(0.f, 0.f, 0.f, 0.f);
-        const uint32_t key = __float_as_uint(a.w) & ((p.pairing & 3) == 3 ? 0x7fffffffu : 0xffffffffu);
-        const bool valid = in_range && (key & 0x7fffffffu) != 0u;   // zero charges contribute nothing: dropped
-        const uint32_t vmask = __ballot_sync(FULL_MASK, valid);
-        const uint32_t peers = (p.pairing & 3) ? (__match_any_sync(FULL_MASK, key) & vmask) : (valid ? 1u << lane : 0u);
-        const int rank = __popc(peers & lt_mask);
-        const bool has_next = (peers >> lane) > 1u;  // a peer in a higher lane exists
-        const bool leader = valid && !(rank & 1) && has_next;
-        const bool single = valid && !(rank & 1) && !has_next;
-        const uint32_t lmask = __ballot_sync(FULL_MASK, leader);
-        const uint32_t smask = __ballot_sync(FULL_MASK, single);
-        if (lane == 0) wcount[warp] = (uint32_t)__popc(lmask) | ((uint32_t)__popc(smask) << 16);
-        const uint32_t higher = (peers >> lane) >> 1;                 // peers above this lane
-        const int partner = leader ? lane + __ffs(higher) : lane;
-        const uint32_t Sx = to_turns(a.x, p.two32_over_L);
-        const uint32_t Sy = to_turns(a.y, p.two32_over_L);
-        const uint32_t Sz = to_turns(a.z, p.two32_over_L);
-        const uint32_t Px = __shfl_sync(FULL_MASK, Sx, partner);
-        const uint32_t Py = __shfl_sync(FULL_MASK, Sy, partner);
-        const uint32_t Pz = __shfl_sync(FULL_MASK, Sz, partner);
-        const uint32_t Pq = __shfl_sync(FULL_MASK, __float_as_uint(a.w), partner);
-        __syncthreads();  // wcount visible; raw fully consumed
-
-        // prefetch the next tile while this one is processed
-        if (t0 + T + tid < hi) cp_async16(&raw[tid], &p.xyzq[t0 + T + tid]);
-
-        // every warp scans the (<= 32) window counts: deterministic record positions
-        uint32_t v = lane < nwarps ? wcount[lane] : 0u, incl = v;
-#pragma unroll
-        for (int d = 1; d < 32; d <<= 1) {
-            const uint32_t n = __shfl_up_sync(FULL_MASK, incl, d);
-            if (lane >= d) incl += n;
-        }
-        const uint32_t base = __shfl_sync(FULL_MASK, incl - v, warp);
-        const uint32_t total = __shfl_sync(FULL_MASK, incl, 31);
-        const int np = (int)(total & 0xffffu), ns = (int)(total >> 16);
-        if (leader) {
-            // S_d = (S_1 - S_2) / 2 (arithmetic shift of the wrapped difference), S_a = S_2 + S_d
-            const int e = (int)(base & 0xffffu) + __popc(lmask & lt_mask);
-            const uint32_t dx = (uint32_t)((int32_t)(Sx - Px) >> 1);
-            const uint32_t dy = (uint32_t)((int32_t)(Sy - Py) >> 1);
-            const uint32_t dz = (uint32_t)((int32_t)(Sz - Pz) >> 1);
-            // o: a quarter turn for opposite charges; plus half a turn on every other pair, which leaves
-            // cos(d - o) e^{i(a + o)} unchanged but alternates the sign of the evaluated amplitude, so
-            // the +1.7e-8 mean error of MUFU.COS (measured) cannot add up coherently over the pairs
-            // (for single atoms it cancels by neutrality; sum of pair amplitudes is not neutral)
-            const uint32_t off = (((__float_as_uint(a.w) ^ Pq) >> 31) ? QUARTER_TURN : 0u) + ((uint32_t)e << 31);
-            arena[2 * e] = make_uint4(Px + dx, Py + dy, Pz + dz, off);
-            arena[2 * e + 1] = make_uint4(dx, dy, dz, __float_as_uint(2.0f * a.w));
-        } else if (single) {
-            const int e = (int)(base >> 16) + __popc(smask & lt_mask);
-            arena[T - 1 - e] = make_uint4(Sx, Sy, Sz, __float_as_uint(a.w));
+        // ---- stage 1: per window (one warp each), classify by charge and count the records
+        for (int w = warp; w < nwin; w += nwarps) {
+            const int idx = (w << 5) + lane;
+            const uint32_t qb = idx < cnt ? __float_as_uint(raw[idx].w) : 0u;
+            const SfWindow cw = sf_classify(qb, idx < cnt, p.pairing, lane);
+            // role word: bits 0-4 partner lane, bit 5 leader, bit 6 single, bits 8.. index in the window's list
+            roles[idx] = (uint16_t)(cw.partner | (cw.leader ? 32 : 0) | (cw.single ? 64 : 0) |
+                                    (__popc((cw.leader ? cw.lmask : cw.smask) & lt_mask) << 8));
+            if (lane == 0) wcount[w] = (uint32_t)__popc(cw.lmask) | ((uint32_t)__popc(cw.smask) << 16);
         }
         __syncthreads();
+        // exclusive scan of the window counts (<= SF_TILE_MAX/32 = 128 of them) by one warp: record positions
+        if (warp == 0) {
+            uint32_t v[4], run = 0;
+#pragma unroll
+            for (int i = 0; i < 4; ++i) { v[i] = (4 * lane + i < nwin) ? wcount[4 * lane + i] : 0u; run += v[i]; }
+            uint32_t incl = run;
+#pragma unroll
+            for (int d = 1; d < 32; d <<= 1) {
+                const uint32_t n = __shfl_up_sync(FULL_MASK, incl, d);
+                if (lane >= d) incl += n;
+            }
+            uint32_t ex = incl - run;
+#pragma unroll
+            for (int i = 0; i < 4; ++i) { wbase[4 * lane + i] = ex; ex += v[i]; }
+            if (lane == 31) wbase[SF_TILE_MAX / 32] = incl;
+        }
+        __syncthreads();
+        const uint32_t total = wbase[SF_TILE_MAX / 32];
+        const int np = (int)(total & 0xffffu), ns = (int)(total >> 16);
+
+        // ---- stage 2: convert to turns and write the records at their scanned positions
+        for (int w = warp; w < nwin; w += nwarps) {
+            const int idx = (w << 5) + lane;
+            const uint32_t base = wbase[w];
+            const float4 a = idx < cnt ? raw[idx] : make_float4(0.f, 0.f, 0.f, 0.f);
+            const uint32_t role = roles[idx];
+            const int partner = role & 31, e_in = role >> 8;
+            const uint32_t Sx = to_turns(a.x, p.two32_over_L);
+            const uint32_t Sy = to_turns(a.y, p.two32_over_L);
+            const uint32_t Sz = to_turns(a.z, p.two32_over_L);
+            const uint32_t Px = __shfl_sync(FULL_MASK, Sx, partner);
+            const uint32_t Py = __shfl_sync(FULL_MASK, Sy, partner);
+            const uint32_t Pz = __shfl_sync(FULL_MASK, Sz, partner);
+            const uint32_t Pq = __shfl_sync(FULL_MASK, __float_as_uint(a.w), partner);
+            if (role & 32) {
+                // S_d = (S_1 - S_2) / 2 (arithmetic shift of the wrapped difference), S_a = S_2 + S_d
+                const int e = (int)(base & 0xffffu) + e_in;
+                const uint32_t dx = (uint32_t)((int32_t)(Sx - Px) >> 1);
+                const uint32_t dy = (uint32_t)((int32_t)(Sy - Py) >> 1);
+                const uint32_t dz = (uint32_t)((int32_t)(Sz - Pz) >> 1);
+                // o: a quarter turn for opposite charges; plus half a turn on every other pair, which leaves
+                // cos(d - o) e^{i(a + o)} unchanged but alternates the sign of the evaluated amplitude, so
+                // the +1.7e-8 mean error of MUFU.COS (measured) cannot add up coherently over the pairs
+                // (for single atoms it cancels by neutrality; the sum of pair amplitudes is not neutral)
+                const uint32_t off = (((__float_as_uint(a.w) ^ Pq) >> 31) ? QUARTER_TURN : 0u) + ((uint32_t)e << 31);
+                arena[2 * e] = make_uint4(Px + dx, Py + dy, Pz + dz, off);
+                arena[2 * e + 1] = make_uint4(dx, dy, dz, __float_as_uint(2.0f * a.w));
+            } else if (role & 64) {
+                const int e = (int)(base >> 16) + e_in;
+                arena[TA - 1 - e] = make_uint4(Sx, Sy, Sz, __float_as_uint(a.w));
+            }
+        }
+        __syncthreads();  // records visible; raw fully consumed
+
+        // prefetch the next tile while this one is processed
+        for (int i = tid; i < TA && t0 + tl + i < hi; i += T) cp_async16(&raw[i], &p.xyzq[t0 + tl + i]);
 
         // ---- accumulate: pair records g, g+ng, ... then single records g, g+ng, ...
         int depth = 0;
@@ -345,7 +387,7 @@ __global__ void __launch_bounds__(SF_TMAX, 1) sf_kernel(const SfParams p) {
         }
 #pragma unroll 1
         for (int e = g; e < ns; e += p.ng) {
-            const uint4 at = arena[T - 1 - e];
+            const uint4 at = arena[TA - 1 - e];
             const float q = __uint_as_float(at.w);
 #pragma unroll
             for (int r = 0; r < SF_KPT; ++r) {
@@ -378,15 +420,29 @@ __global__ void __launch_bounds__(SF_TMAX, 1) sf_kernel(const SfParams p) {
         }
     }
 
-    // ---- the last CTA finalises (fixed summation order: independent of which CTA is last)
-    __threadfence();
+    // ---- second pass: the last CTA of each group sums the group, the last group sums the groups
+    const RedParams& rp = p.red;
+    const int grp = blockIdx.x / rp.group_size, first = grp * rp.group_size;
+    const int members = ((int)gridDim.x - first < rp.group_size) ? (int)gridDim.x - first : rp.group_size;
+    // (the barrier orders the CTA's row before thread 0's fence; the fence is cumulative)
     __syncthreads();
-    if (tid == 0) s_last = (atomicInc(p.ticket, gridDim.x * gridDim.y - 1) == gridDim.x * gridDim.y - 1);
-    __syncthreads();
-    if (s_last) {
+    if (tid == 0) {
         __threadfence();
-        fin_cta(p.fin, acc_all, tid, T);
+        s_last = (atomicInc(&rp.tickets[grp], members * gridDim.y - 1) == members * gridDim.y - 1);
+        __threadfence();
     }
+    __syncthreads();
+    if (!s_last) return;
+    reduce_rows(rp.part + (int64_t)first * p.P, members, p.P, rp.grow + (int64_t)grp * p.P, nullptr, acc_all, tid, T);
+    __syncthreads();
+    if (tid == 0) {
+        __threadfence();
+        s_last = (atomicInc(&rp.tickets[rp.ngroups], rp.ngroups - 1) == (unsigned)rp.ngroups - 1);
+        __threadfence();
+    }
+    __syncthreads();
+    if (!s_last) return;
+    reduce_rows(rp.grow, rp.ngroups, p.P, rp.rho, rp.rho_user, acc_all, tid, T);
 }
 
 // ---------------------------------------------------------------------------------------
@@ -403,36 +459,34 @@ struct FParams {
     const float4* xyzq;
     float4* force;
     int64_t N;
-    const int4* ka;
-    const float4* kb;
+    KTable kt;     // rho and the k-set: every CTA builds its {-m, theta}, {G, E} records from these
     double two32_over_L;
     int32_t P;
-    int32_t pdl;   // launched with programmatic stream serialisation: wait before reading ka/kb
+    int32_t pdl;   // launched with programmatic stream serialisation: wait before reading rho
 };
 
-template <int R, bool ENERGY>
-__device__ __forceinline__ void f_load(const FParams& p, int64_t unit0, int lane, uint32_t (&sx)[R], uint32_t (&sy)[R],
-                                       uint32_t (&sz)[R], float (&q)[R]) {
+__device__ __forceinline__ float4 f_fetch(const FParams& p, int64_t unit, int lane) {
+    const int64_t i = unit * 32 + lane;
+    return i < p.N ? __ldg(&p.xyzq[i]) : make_float4(0.f, 0.f, 0.f, 0.f);
+}
+
+// One pass: R units (R atoms per thread) against the nk wavevector records in shared memory.
+// `pre` != nullptr: the atom records were fetched earlier (prologue overlap), else fetch here.
+template <int R, bool ENERGY, bool ACCUM>
+__device__ __forceinline__ void f_pass(const FParams& p, const int4* s_ka, const float4* s_kb, int nk, int64_t unit0,
+                                       int lane, const float4* pre) {
+    uint32_t sx[R], sy[R], sz[R];
+    float q[R], fx[R], fy[R], fz[R], en[R];
+    const float K = phase_scale();
 #pragma unroll
     for (int r = 0; r < R; ++r) {
-        const int64_t i = (unit0 + r) * 32 + lane;
-        float4 a = make_float4(0.f, 0.f, 0.f, 0.f);
-        if (i < p.N) a = __ldg(&p.xyzq[i]);
+        const float4 a = pre ? pre[r] : f_fetch(p, unit0 + r, lane);
         sx[r] = to_turns(a.x, p.two32_over_L);
         sy[r] = to_turns(a.y, p.two32_over_L);
         sz[r] = to_turns(a.z, p.two32_over_L);
         q[r] = a.w;
+        fx[r] = fy[r] = fz[r] = en[r] = 0.f;
     }
-}
-
-template <int R, bool ENERGY, bool ACCUM>
-__device__ __forceinline__ void f_units(const FParams& p, const int4* s_ka, const float4* s_kb, int nk, int64_t unit0,
-                                        int lane, const uint32_t (&sx)[R], const uint32_t (&sy)[R],
-                                        const uint32_t (&sz)[R], const float (&q)[R]) {
-    float fx[R], fy[R], fz[R], en[R];
-    const float K = phase_scale();
-#pragma unroll
-    for (int r = 0; r < R; ++r) fx[r] = fy[r] = fz[r] = en[r] = 0.f;
 #pragma unroll 4
     for (int k = 0; k < nk; ++k) {
         const int4 a = s_ka[k];
@@ -462,32 +516,31 @@ __device__ __forceinline__ void f_units(const FParams& p, const int4* s_ka, cons
     }
 }
 
-template <int R, bool ENERGY, bool ACCUM>
-__device__ __forceinline__ void f_pass(const FParams& p, const int4* s_ka, const float4* s_kb, int nk, int64_t unit0, int lane) {
-    uint32_t sx[R], sy[R], sz[R];
-    float q[R];
-    f_load<R, ENERGY>(p, unit0, lane, sx, sy, sz, q);
-    f_units<R, ENERGY, ACCUM>(p, s_ka, s_kb, nk, unit0, lane, sx, sy, sz, q);
+// n units in ceil(n / F_RMAX) passes of nearly equal size (e.g. 9 -> 3+3+3, not 4+4+1)
+__device__ __forceinline__ int f_first_pass(int n) {
+    const int passes = (n + F_RMAX - 1) / F_RMAX;
+    return passes ? (n + passes - 1) / passes : 0;
 }
 
 template <bool ENERGY, bool ACCUM>
-__device__ __forceinline__ void f_run(const FParams& p, const int4* s_ka, const float4* s_kb, int nk, int64_t u, int n, int lane) {
-    // n units in ceil(n / F_RMAX) passes of nearly equal size (e.g. 9 -> 3+3+3, not 4+4+1)
+__device__ __forceinline__ void f_run(const FParams& p, const int4* s_ka, const float4* s_kb, int nk, int64_t u, int n,
+                                      int lane, const float4* pre) {
     int passes = (n + F_RMAX - 1) / F_RMAX;
     while (n > 0) {
         const int r = (n + passes - 1) / passes;
         switch (r) {
-            case 4: f_pass<4, ENERGY, ACCUM>(p, s_ka, s_kb, nk, u, lane); break;
-            case 3: f_pass<3, ENERGY, ACCUM>(p, s_ka, s_kb, nk, u, lane); break;
-            case 2: f_pass<2, ENERGY, ACCUM>(p, s_ka, s_kb, nk, u, lane); break;
-            default: f_pass<1, ENERGY, ACCUM>(p, s_ka, s_kb, nk, u, lane); break;
+            case 4: f_pass<4, ENERGY, ACCUM>(p, s_ka, s_kb, nk, u, lane, pre); break;
+            case 3: f_pass<3, ENERGY, ACCUM>(p, s_ka, s_kb, nk, u, lane, pre); break;
+            case 2: f_pass<2, ENERGY, ACCUM>(p, s_ka, s_kb, nk, u, lane, pre); break;
+            default: f_pass<1, ENERGY, ACCUM>(p, s_ka, s_kb, nk, u, lane, pre); break;
         }
         u += r; n -= r; --passes;
+        pre = nullptr;
     }
 }
 
 template <bool ENERGY>
-__global__ void __launch_bounds__(F_THREADS) f_kernel(const FParams p) {
+__global__ void __launch_bounds__(F_THREADS, 4) f_kernel(const FParams p) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int nkmax = p.P < F_KCHUNK ? p.P : F_KCHUNK;
     int4* s_ka = reinterpret_cast<int4*>(smem_raw);
@@ -497,19 +550,24 @@ __global__ void __launch_bounds__(F_THREADS) f_kernel(const FParams p) {
     const int64_t gw = (int64_t)blockIdx.x * (F_THREADS / 32) + (threadIdx.x >> 5);
     const int64_t units = (p.N + 31) / 32;
     const int64_t u0 = units * gw / nwarps, u1 = units * (gw + 1) / nwarps;
+    const int n = (int)(u1 - u0);
 
-    if (p.pdl) grid_dependency_wait();   // ka/kb come from the preceding grid
+    // fetch the first pass's atoms before waiting for the structure factors: the loads (and, with
+    // PDL, this grid's launch) overlap the tail of the preceding grid
+    float4 pre[F_RMAX];
+    const int r0 = f_first_pass(n);
+#pragma unroll
+    for (int r = 0; r < F_RMAX; ++r) pre[r] = r < r0 ? f_fetch(p, u0 + r, lane) : make_float4(0.f, 0.f, 0.f, 0.f);
+
+    if (p.pdl) grid_dependency_wait();   // rho comes from the preceding grid
 
     for (int k0 = 0; k0 < p.P; k0 += F_KCHUNK) {
         const int nk = (p.P - k0 < F_KCHUNK) ? (p.P - k0) : F_KCHUNK;
         if (k0 > 0) __syncthreads();
-        for (int t = threadIdx.x; t < nk; t += F_THREADS) {
-            s_ka[t] = p.ka[k0 + t];
-            s_kb[t] = p.kb[k0 + t];
-        }
+        for (int t = threadIdx.x; t < nk; t += F_THREADS) k_record(p.kt, k0 + t, s_ka[t], s_kb[t]);
         __syncthreads();
-        if (k0 == 0) f_run<ENERGY, false>(p, s_ka, s_kb, nk, u0, (int)(u1 - u0), lane);
-        else f_run<ENERGY, true>(p, s_ka, s_kb, nk, u0, (int)(u1 - u0), lane);
+        if (k0 == 0) f_run<ENERGY, false>(p, s_ka, s_kb, nk, u0, n, lane, pre);
+        else f_run<ENERGY, true>(p, s_ka, s_kb, nk, u0, n, lane, nullptr);
     }
 }
 

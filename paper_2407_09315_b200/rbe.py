@@ -28,7 +28,7 @@ class RbeError(RuntimeError):
 class LaunchInfo(ctypes.Structure):
     _fields_ = [(n, ctypes.c_int32) for n in (
         "num_sms", "sf_grid_x", "sf_grid_y", "sf_threads", "sf_smem_bytes", "sf_k_per_thread",
-        "sf_atom_groups", "sf_tile_atoms", "fin_grid", "fin_threads", "f_grid", "f_threads",
+        "sf_atom_groups", "sf_tile_atoms", "sf_red_group", "sf_red_groups", "f_grid", "f_threads",
         "f_smem_bytes", "f_atoms_per_thread")]
 
     def as_dict(self):
@@ -58,6 +58,8 @@ def lib():
         L.rbe_workspace_bytes.argtypes = [vp]
         L.rbe_set_workspace.restype = ctypes.c_int
         L.rbe_set_workspace.argtypes = [vp, vp, sz]
+        L.rbe_set_pairing.restype = ctypes.c_int
+        L.rbe_set_pairing.argtypes = [vp, i32]
         L.rbe_get_launch_info.restype = ctypes.c_int
         L.rbe_get_launch_info.argtypes = [vp, ctypes.POINTER(LaunchInfo)]
         L.rbe_set_kvectors.restype = ctypes.c_int
@@ -113,8 +115,8 @@ class Rbe:
             raise RbeError(st, lib().rbe_last_error(self._h).decode())
 
     def close(self):
-        if getattr(self, "_h", None) is not None and self._h.value:
-            lib().rbe_destroy(self._h)
+        if getattr(self, "_h", None) is not None and self._h.value and _lib is not None:
+            _lib.rbe_destroy(self._h)
             self._h = ctypes.c_void_p()
 
     __del__ = close
@@ -135,6 +137,9 @@ class Rbe:
             ws = torch.empty(self.rbe_workspace_bytes(), dtype=torch.uint8, device="cuda")
         self._check(lib().rbe_set_workspace(self._h, ctypes.c_void_p(ws.data_ptr()), ws.numel() * ws.element_size()))
         self._ws = ws  # keep alive
+
+    def rbe_set_pairing(self, mode: int):
+        self._check(lib().rbe_set_pairing(self._h, int(mode)))
 
     def rbe_get_launch_info(self) -> dict:
         li = LaunchInfo()

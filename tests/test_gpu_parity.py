@@ -122,6 +122,62 @@ def test_ragged_batch_sizes(P):
     check(atoms, cfg.L, cfg.alpha, m, with_energy=(P % 2 == 1))
 
 
+# ------------------------------------------------------------ equal-|q| pairing (sf_kernel)
+def _charge_case(kind, n, rng):
+    if kind == "all_distinct":          # nothing pairs: every atom takes the plain path
+        return (rng.random(n) * 2 - 1 + 1e-3).astype(np.float32)
+    if kind == "all_equal":             # one class, non-neutral
+        return np.full(n, 0.75, dtype=np.float32)
+    if kind == "with_zeros":            # zero charges are dropped, the rest pair
+        q = np.where(np.arange(n) % 3 == 0, 0.0, np.where(np.arange(n) % 2 == 0, 1.0, -1.0))
+        return q.astype(np.float32)
+    if kind == "odd_classes":           # class sizes are odd inside most 32-atom windows
+        return np.array([0.5, -0.5, 0.5, 1.25, -0.5, 0.5, 2.0], dtype=np.float32)[np.arange(n) % 7]
+    if kind == "negative_zero":
+        q = np.where(np.arange(n) % 2 == 0, 1.0, -1.0).astype(np.float32)
+        q[::5] = -0.0
+        return q
+    raise ValueError(kind)
+
+
+@pytest.mark.parametrize("kind", ["all_distinct", "all_equal", "with_zeros", "odd_classes", "negative_zero"])
+def test_pairing_handles_any_charge_assignment(kind):
+    rng = np.random.default_rng(21)
+    n, L, alpha = 9_001, 40.0, 0.09
+    atoms = np.empty((n, 4), dtype=np.float32)
+    atoms[:, :3] = rng.random((n, 3)) * L
+    atoms[:, 3] = _charge_case(kind, n, rng)
+    m = inputs.sample_kset(L, alpha, 100, 22)
+    check(atoms, L, alpha, m, with_energy=True)
+
+
+@pytest.mark.parametrize("name", ["water_96k", "ions_20000"])
+def test_pairing_modes_agree(name):
+    """rbe_set_pairing 0 / 1 / 3 evaluate the same sum: rho agrees to rounding, well inside the
+    tolerance, whichever atoms the kernel combines."""
+    cfg = inputs.CONFIGS[name] if name in inputs.CONFIGS else inputs.ions_config(20_000)
+    atoms = inputs.make_atoms(cfg)
+    m = inputs.sample_kset(cfg.L, cfg.alpha, cfg.P, cfg.seed, 3)
+    xyzq = torch.from_numpy(atoms).cuda()
+    out = {}
+    for mode in (0, 1, 3):
+        ctx = rbe.Rbe(cfg.N, cfg.L, cfg.alpha, cfg.P)
+        ctx.rbe_set_pairing(mode)
+        rho = torch.empty((cfg.P, 2), dtype=torch.float64, device="cuda")
+        ctx.rbe_set_kvectors(m)
+        ctx.rbe_structure_factor(xyzq, rho)
+        out[mode] = rho.cpu().numpy()
+    qsum = np.abs(atoms[:, 3].astype(np.float64)).sum()
+    rho_o = oracle.rho(atoms, cfg.L, m)
+    for mode in (0, 1, 3):
+        assert np.abs(out[mode] - rho_o).max() <= RHO_TOL * qsum
+        # far tighter than the bar: relative to |rho| itself (cancellation in neutral molecules kept)
+        rel = np.hypot(*(out[mode] - rho_o).T) / np.hypot(*rho_o.T)
+        assert np.median(rel) <= 2e-5, (mode, np.median(rel))
+    with pytest.raises(rbe.RbeError):
+        ctx.rbe_set_pairing(2)
+
+
 def test_empty_system():
     m = inputs.sample_kset(20.0, 0.09, 16, 1)
     ctx, rho, F, U = gpu_step(np.zeros((0, 4), dtype=np.float32), 20.0, 0.09, m)
