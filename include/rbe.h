@@ -148,11 +148,22 @@ rbe_status rbe_kspace_energy(rbe_ctx* ctx, double* h_U, void* stream);
  * device, uploads the k-set, runs rbe_structure_factor and rbe_forces, copies the forces back
  * into h_force (float [N][4]) and, if h_U != NULL, the energy into *h_U; synchronises `stream`.
  * d_scratch: caller-owned device buffer of at least 32 * N bytes (positions + forces).
- * Pinned host buffers make the copies asynchronous; pageable ones work but are slower.
+ * With N >= 131 072 the atoms travel in up to 4 chunks on two internal copy streams so that the
+ * transfers overlap the kernels (every chunk adds to the same per-CTA fp64 partial rows in stream
+ * order: the result stays bitwise reproducible).  Pinned host buffers (rbe_host_alloc) make the
+ * copies asynchronous; pageable ones work but are slower.
  * Errors: as the calls it is made of, plus RBE_ERR_WORKSPACE if d_scratch is too small. */
 rbe_status rbe_step_host(rbe_ctx* ctx, const float* h_xyzq, const int32_t* h_m, const double* h_w,
                          float* h_force, int32_t with_energy, double* h_U, void* d_scratch,
                          size_t scratch_bytes, void* stream);
+
+/* Page-locked (pinned) HOST memory for the end-to-end path: cudaHostAlloc'ed, so that the copies of
+ * rbe_step_host are asynchronous DMA transfers at full PCIe rate (measured on B200 hosts: 55 GB/s
+ * from such a buffer, 15-40 GB/s and erratic from memory pinned after allocation).  The caller
+ * owns the buffer until rbe_host_free.  No context is needed.
+ * Errors: RBE_ERR_INVALID_ARG (out == NULL or bytes == 0), RBE_ERR_NO_DEVICE, RBE_ERR_CUDA. */
+rbe_status rbe_host_alloc(void** out, size_t bytes);
+rbe_status rbe_host_free(void* h_ptr);
 
 /* Text of the last error on this context (owned by the context; "" if none).  For ctx == NULL
  * returns a static string. */

@@ -22,12 +22,29 @@ namespace rbe {
 // ---------------------------------------------------------------------------------------
 // tunables (compile time)
 // ---------------------------------------------------------------------------------------
+// (each may be overridden with -DRBE_<NAME>=value when sweeping; the defaults are the tuned ones)
+#ifndef RBE_SF_TMAX
+#define RBE_SF_TMAX 1024
+#endif
+#ifndef RBE_SF_CTAS_PER_SM
+#define RBE_SF_CTAS_PER_SM 1
+#endif
+#ifndef RBE_SF_TILE_MAX
+#define RBE_SF_TILE_MAX 4096
+#endif
+#ifndef RBE_F_THREADS
+#define RBE_F_THREADS 512
+#endif
+#ifndef RBE_F_CTAS_PER_SM
+#define RBE_F_CTAS_PER_SM 2
+#endif
 constexpr int SF_KPT = 4;        // wavevectors owned by one thread of the structure-factor kernel
-constexpr int SF_TMAX = 1024;    // max threads per CTA (structure-factor kernel): <= 64 registers
-constexpr int SF_CTAS_PER_SM = 1;
-constexpr int SF_TILE_MAX = 4096; // max atoms staged in shared memory at a time (structure-factor kernel)
+constexpr int SF_TMAX = RBE_SF_TMAX;    // max threads per CTA (structure-factor kernel): <= 64 registers
+constexpr int SF_CTAS_PER_SM = RBE_SF_CTAS_PER_SM;
+constexpr int SF_TILE_MAX = RBE_SF_TILE_MAX; // max atoms staged in shared memory at a time (structure-factor kernel)
 constexpr int SF_DEPTH = 64;     // max atoms a thread accumulates in fp32 before the fp64 flush
-constexpr int F_THREADS = 256;   // threads per CTA (force kernel)
+constexpr int F_THREADS = RBE_F_THREADS;   // threads per CTA (force kernel)
+constexpr int F_CTAS_PER_SM = RBE_F_CTAS_PER_SM;
 constexpr int F_RMAX = 4;        // max atoms per thread per pass (force kernel)
 constexpr int F_KCHUNK = 2048;   // wavevectors staged in shared memory at a time (force kernel)
 constexpr int SF_RED_GROUP = 16; // CTAs per group in the two-level reduction of the per-CTA rows
@@ -207,8 +224,19 @@ struct SfParams {
     int32_t tile_atoms;   // atoms staged per tile: a multiple of 32, <= SF_TILE_MAX
     int32_t flush_every;  // tiles between fp64 flushes (keeps the fp32 depth <= ~SF_DEPTH atoms)
     int32_t pairing;      // bit 0: pair equal charges, bit 1: pair opposite charges (3 = both)
+    int32_t accumulate;   // add this launch's per-CTA rows to what `part` holds (chunked host step: one launch per chunk)
+    int32_t finalise;     // run the second pass (rows -> rho) at the end of this launch
     RedParams red;
+#ifdef RBE_SF_PROFILE
+    long long* prof;      // [gridDim.x][64] globaltimer stamps of thread 0 (sweep builds only)
+#endif
 };
+
+#ifdef RBE_SF_PROFILE
+#define RBE_STAMP() do { if (tid == 0 && prof_n < 64) { long long t_; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t_)); p.prof[blockIdx.x * 64 + prof_n++] = t_; } } while (0)
+#else
+#define RBE_STAMP() do { } while (0)
+#endif
 
 // acc points at this thread's slot of component 0; component r lives `stride` entries further
 // (layout [SF_KPT][blockDim.x]: conflict-free).
@@ -258,7 +286,9 @@ __global__ void __launch_bounds__(SF_TMAX, SF_CTAS_PER_SM) sf_kernel(const SfPar
     float4* raw = reinterpret_cast<float4*>(smem_raw);               // [TA] raw atom records of the tile
     uint4* arena = reinterpret_cast<uint4*>(smem_raw) + TA;          // [TA] pair records from the front, singles from the back
     double2* acc_all = reinterpret_cast<double2*>(arena + TA);       // [SF_KPT][T] fp64 accumulators
-    __shared__ uint32_t wcount[SF_TILE_MAX / 32], wbase[SF_TILE_MAX / 32 + 1];
+    constexpr int WIN_MAX = 128;   // the one-warp scan below covers 4 windows per lane
+    static_assert(SF_TILE_MAX / 32 <= WIN_MAX, "tile too large for the window scan");
+    __shared__ uint32_t wcount[WIN_MAX], wbase[WIN_MAX + 1];
     __shared__ uint16_t roles[SF_TILE_MAX];
     __shared__ uint32_t s_last;
 
@@ -292,12 +322,17 @@ __global__ void __launch_bounds__(SF_TMAX, SF_CTAS_PER_SM) sf_kernel(const SfPar
     if (tl < 32) tl = 32;
     for (int i = tid; i < tl && lo + i < hi; i += T) cp_async16(&raw[i], &p.xyzq[lo + i]);
     int since_flush = 0;
+#ifdef RBE_SF_PROFILE
+    int prof_n = 0;
+#endif
+    RBE_STAMP();
 
     for (int64_t t0 = lo; t0 < hi; t0 += tl, tl = TA) {
         const int cnt = (int)((hi - t0 < tl) ? (hi - t0) : tl);
         const int nwin = (cnt + 31) >> 5;
         cp_async_wait_all();
         __syncthreads();  // raw holds the tile; everyone is done with the previous arena
+        RBE_STAMP();
 
         // ---- stage 1: per window (one warp each), classify by charge and count the records
         for (int w = warp; w < nwin; w += nwarps) {
@@ -324,10 +359,10 @@ __global__ void __launch_bounds__(SF_TMAX, SF_CTAS_PER_SM) sf_kernel(const SfPar
             uint32_t ex = incl - run;
 #pragma unroll
             for (int i = 0; i < 4; ++i) { wbase[4 * lane + i] = ex; ex += v[i]; }
-            if (lane == 31) wbase[SF_TILE_MAX / 32] = incl;
+            if (lane == 31) wbase[WIN_MAX] = incl;
         }
         __syncthreads();
-        const uint32_t total = wbase[SF_TILE_MAX / 32];
+        const uint32_t total = wbase[WIN_MAX];
         const int np = (int)(total & 0xffffu), ns = (int)(total >> 16);
 
         // ---- stage 2: convert to turns and write the records at their scanned positions
@@ -363,6 +398,7 @@ __global__ void __launch_bounds__(SF_TMAX, SF_CTAS_PER_SM) sf_kernel(const SfPar
             }
         }
         __syncthreads();  // records visible; raw fully consumed
+        RBE_STAMP();
 
         // prefetch the next tile while this one is processed
         for (int i = tid; i < TA && t0 + tl + i < hi; i += T) cp_async16(&raw[i], &p.xyzq[t0 + tl + i]);
@@ -401,6 +437,7 @@ __global__ void __launch_bounds__(SF_TMAX, SF_CTAS_PER_SM) sf_kernel(const SfPar
         if (++since_flush >= p.flush_every) { sf_flush(acc, T, c, s); since_flush = 0; }
     }
     sf_flush(acc, T, c, s);
+    RBE_STAMP();
 
     // let the dependent (force) kernel start launching; it waits for this grid's completion
     grid_launch_dependents();
@@ -416,9 +453,12 @@ __global__ void __launch_bounds__(SF_TMAX, SF_CTAS_PER_SM) sf_kernel(const SfPar
                 const double2 v = acc_all[(idx % SF_KPT) * T + gg * p.gs + idx / SF_KPT];
                 re += v.x; im += v.y;
             }
-            p.part[(int64_t)blockIdx.x * p.P + k] = make_double2(re, im);
+            double2* row = &p.part[(int64_t)blockIdx.x * p.P + k];
+            if (p.accumulate) { const double2 old = *row; re += old.x; im += old.y; }   // chunks arrive in stream order
+            *row = make_double2(re, im);
         }
     }
+    if (!p.finalise) return;
 
     // ---- second pass: the last CTA of each group sums the group, the last group sums the groups
     const RedParams& rp = p.red;
@@ -432,6 +472,7 @@ __global__ void __launch_bounds__(SF_TMAX, SF_CTAS_PER_SM) sf_kernel(const SfPar
         __threadfence();
     }
     __syncthreads();
+    RBE_STAMP();
     if (!s_last) return;
     reduce_rows(rp.part + (int64_t)first * p.P, members, p.P, rp.grow + (int64_t)grp * p.P, nullptr, acc_all, tid, T);
     __syncthreads();
@@ -442,7 +483,9 @@ __global__ void __launch_bounds__(SF_TMAX, SF_CTAS_PER_SM) sf_kernel(const SfPar
     }
     __syncthreads();
     if (!s_last) return;
+    RBE_STAMP();
     reduce_rows(rp.grow, rp.ngroups, p.P, rp.rho, rp.rho_user, acc_all, tid, T);
+    RBE_STAMP();
 }
 
 // ---------------------------------------------------------------------------------------
@@ -540,7 +583,7 @@ __device__ __forceinline__ void f_run(const FParams& p, const int4* s_ka, const 
 }
 
 template <bool ENERGY>
-__global__ void __launch_bounds__(F_THREADS, 4) f_kernel(const FParams p) {
+__global__ void __launch_bounds__(F_THREADS, F_CTAS_PER_SM) f_kernel(const FParams p) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int nkmax = p.P < F_KCHUNK ? p.P : F_KCHUNK;
     int4* s_ka = reinterpret_cast<int4*>(smem_raw);

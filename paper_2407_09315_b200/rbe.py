@@ -74,6 +74,10 @@ def lib():
         L.rbe_kspace_energy.argtypes = [vp, ctypes.POINTER(dbl), vp]
         L.rbe_step_host.restype = ctypes.c_int
         L.rbe_step_host.argtypes = [vp, vp, vp, vp, vp, i32, ctypes.POINTER(dbl), vp, sz, vp]
+        L.rbe_host_alloc.restype = ctypes.c_int
+        L.rbe_host_alloc.argtypes = [ctypes.POINTER(vp), sz]
+        L.rbe_host_free.restype = ctypes.c_int
+        L.rbe_host_free.argtypes = [vp]
         L.rbe_last_error.restype = ctypes.c_char_p
         L.rbe_last_error.argtypes = [vp]
         L.rbe_status_string.restype = ctypes.c_char_p
@@ -81,6 +85,34 @@ def lib():
         L.rbe_version.restype = i32
         _lib = L
     return _lib
+
+
+class _HostBlock:
+    """Owner of one rbe_host_alloc block: freed when the last numpy view of it is gone."""
+
+    def __init__(self, nbytes):
+        self.ptr = ctypes.c_void_p()
+        st = lib().rbe_host_alloc(ctypes.byref(self.ptr), nbytes)
+        if st != RBE_OK:
+            raise RbeError(st, "rbe_host_alloc failed")
+
+    def __del__(self):
+        if getattr(self, "ptr", None) is not None and self.ptr.value and _lib is not None:
+            _lib.rbe_host_free(self.ptr)
+            self.ptr = ctypes.c_void_p()
+
+
+def rbe_host_alloc(shape, dtype="float32"):
+    """numpy array in page-locked host memory from the library's rbe_host_alloc (cudaHostAlloc): the
+    buffers to hand to rbe_step_host.  Freed (rbe_host_free) when the array and its views are gone."""
+    import numpy as np
+    dt = np.dtype(dtype)
+    count = int(np.prod(shape))
+    nbytes = max(count * dt.itemsize, 1)
+    blk = _HostBlock(nbytes)
+    buf = (ctypes.c_ubyte * nbytes).from_address(blk.ptr.value)
+    buf._rbe_owner = blk          # numpy keeps `buf` alive through .base; `buf` keeps the owner alive
+    return np.frombuffer(buf, dtype=dt, count=count).reshape(shape)
 
 
 def _stream_ptr(stream):

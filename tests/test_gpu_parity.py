@@ -295,3 +295,40 @@ def test_host_buffer_step_matches_device_path():
     h_f = torch.empty((cfg.N, 4), dtype=torch.float32).pin_memory()
     U = ctx.rbe_step_host(h_x, m, h_f, with_energy=True, want_energy=True)
     assert np.array_equal(h_f.numpy(), F_g) and U == U_g
+
+
+@pytest.mark.parametrize("N", [131_073, 300_000])
+def test_host_buffer_step_chunked_pipeline(N):
+    """rbe_step_host splits N >= 131 072 atoms into up to 4 chunks (copy/compute pipeline); every chunk
+    adds to the same per-CTA rows in stream order, so the result is the oracle's to the usual
+    tolerances and bitwise reproducible run to run (the fp32 partial sums group the atoms differently
+    from the one-launch device path, so the two agree to fp32 rounding of those, not bitwise)."""
+    cfg = inputs.ions_config(300_000)
+    atoms = inputs.make_atoms(cfg)[:N].copy()
+    m = inputs.sample_kset(cfg.L, cfg.alpha, 64, 31)
+    ctx, rho_g, F_g, U_g = gpu_step(atoms, cfg.L, cfg.alpha, m, with_energy=True)
+    h_x = torch.from_numpy(atoms).pin_memory()
+    outs = []
+    for rep in range(2):
+        h_f = torch.full((N, 4), float("nan"), dtype=torch.float32).pin_memory()
+        U = ctx.rbe_step_host(h_x, m, h_f, with_energy=True, want_energy=True)
+        outs.append((h_f.numpy().copy(), U))
+    assert np.array_equal(outs[0][0], outs[1][0]) and outs[0][1] == outs[1][1]
+    F_h, U_h = outs[0]
+    S = oracle.S(cfg.L, cfg.alpha)
+    rho_o = oracle.rho(atoms, cfg.L, m)
+    F_o, e_o = oracle.force(atoms, cfg.L, m, S, rho_o, with_energy=True)
+    assert np.linalg.norm(F_h[:, :3] - F_o) / np.linalg.norm(F_o) <= F_TOL
+    assert np.linalg.norm(F_h[:, 3] - e_o) <= 2e-5 * np.linalg.norm(e_o)
+    assert abs(U_h - oracle.energy(cfg.L, m, S, rho_o)) <= U_TOL * abs(U_g)
+    assert abs(U_h - U_g) <= 1e-6 * abs(U_g)
+    # the library's own page-locked buffers (rbe_host_alloc), as bench.py's e2e leg uses them
+    a_x, a_f = rbe.rbe_host_alloc((N, 4)), rbe.rbe_host_alloc((N, 4))
+    a_x[:] = atoms
+    a_f[:] = np.nan
+    ctx.rbe_step_host(a_x, m, a_f, with_energy=True)
+    assert np.array_equal(a_f, F_h)
+    # pageable host memory takes the same path (the copies are then staged by the driver)
+    h_f2 = np.full((N, 4), np.nan, dtype=np.float32)
+    ctx.rbe_step_host(atoms, m, h_f2, with_energy=True)
+    assert np.array_equal(h_f2, F_h)
