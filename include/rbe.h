@@ -113,6 +113,39 @@ rbe_status rbe_get_launch_info(const rbe_ctx* ctx, rbe_launch_info* out);
  * Errors: RBE_ERR_BAD_KVECTOR, RBE_ERR_NOT_READY (no workspace), RBE_ERR_CUDA. */
 rbe_status rbe_set_kvectors(rbe_ctx* ctx, const int32_t* h_m, const double* h_w, void* stream);
 
+/* Algorithm 1 step 1 on the device: draw this context's batch of P wavevectors on the GPU,
+ * m != 0 with probability ~ exp(-|2 pi m / L|^2 / 4 alpha), weights w_l = S / P.  Exact iid
+ * draws (the paper's Metropolis chain is under-specified): each m_d by inverse CDF of
+ * the 1-D discrete Gaussian, the zero triple rejected.  Counter-based, so the batch is a pure
+ * function of (L, alpha, P, seed, step):
+ *   candidate j = 0, 1, ... : words (x, y, z) = first three outputs of Philox4x32-10 with counter
+ *   (j mod 2^32, j >> 32, step mod 2^32, step >> 32) and key (seed mod 2^32, seed >> 32);
+ *   m_d = #{ i : T_i <= word_d } - M, where c = pi^2 / (alpha L^2), M = ceil(sqrt(40 ln 2 / c)),
+ *   T_i = min(2^32 - 1, floor(2^32 * sum_{i' <= i} exp(-c (i' - M)^2) / sum_{all})), i = 0 .. 2M - 1
+ *   (fp64, host);
+ *   the batch = the first P candidates != (0, 0, 0), in order of j.
+ * No host-to-device traffic; replaces rbe_set_kvectors for this step (and invalidates any previous
+ * structure factor).  Errors: RBE_ERR_NOT_READY (no workspace), RBE_ERR_INVALID_ARG (M > 2^20:
+ * table too large for this L, alpha), RBE_ERR_CUDA. */
+rbe_status rbe_sample_kvectors(rbe_ctx* ctx, uint64_t seed, uint64_t step, void* stream);
+
+/* Copy the current k-set back to the host: h_m int32 [P][3].  Synchronises `stream`.
+ * Errors: RBE_ERR_NOT_READY (no k-set), RBE_ERR_INVALID_ARG, RBE_ERR_CUDA. */
+rbe_status rbe_get_kvectors(rbe_ctx* ctx, int32_t* h_m, void* stream);
+
+/* One whole step -- rbe_sample_kvectors(seed, step) + rbe_structure_factor + rbe_forces -- captured
+ * once as a CUDA graph bound to d_xyzq / d_force (float4 [N], device, caller-owned, must stay valid)
+ * and replayed with ONE launch per step and no host-to-device traffic: (seed, step) live in the
+ * workspace and every replay advances the step by one, starting at first_step.  Meant for the
+ * launch-bound small systems and for MD loops that keep positions on the device.
+ * rbe_graph_capture synchronises (it uploads the step counter and instantiates the graph);
+ * rbe_graph_launch only enqueues on `stream`.  After a replay rbe_kspace_energy and
+ * rbe_get_kvectors refer to that step.  A new rbe_set_workspace discards the graph.
+ * Errors: RBE_ERR_NOT_READY, RBE_ERR_INVALID_ARG, RBE_ERR_CUDA. */
+rbe_status rbe_graph_capture(rbe_ctx* ctx, const void* d_xyzq, void* d_force, int32_t with_energy,
+                             uint64_t seed, uint64_t first_step);
+rbe_status rbe_graph_launch(rbe_ctx* ctx, void* stream);
+
 /* Algorithm 1 steps 2-3, Eq. (2.9): rho(k_l) for l = 0..P-1 over this context's
  * N atoms, then the per-k force coefficients for rbe_forces.
  *   d_xyzq  float4 [N] = {x, y, z, q} (AoS), device.

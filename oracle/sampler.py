@@ -13,7 +13,7 @@ random numbers so that a GPU implementation can be compared bit for bit:
     and key (s mod 2^32, s >> 32);
   * 1-D table: c = pi^2 / (alpha L^2), M = ceil(sqrt(40 ln 2 / c)), p_i = exp(-c (i - M)^2) for
     i = 0 .. 2M summed in ascending i (fp64), T_i = floor(2^32 * (p_0 + .. + p_i) / total) for
-    i = 0 .. 2M - 1 (the last bin takes the rest);
+    i = 0 .. 2M - 1, clamped to 2^32 - 1 (the last bin takes the rest);
   * m_d = #{ i : T_i <= word_d } - M   (an upper bound search: integer comparisons only);
   * the batch is the first P candidates that are not (0, 0, 0), in order of j.
 
@@ -23,6 +23,8 @@ Random123 known-answer vectors for Philox4x32-10 in tests/golden/philox4x32_10_k
 table against the pmf; the rejection rule by brute force; chi-square and second moment).
 """
 from __future__ import annotations
+
+import math
 
 import numpy as np
 
@@ -51,21 +53,22 @@ def philox4x32_10(counter, key):
 
 
 def half_width(L: float, alpha: float) -> int:
-    c = np.pi ** 2 / (alpha * L * L)
-    return int(np.ceil(np.sqrt(40.0 * np.log(2.0) / c)))
+    c = math.pi * math.pi / (alpha * L * L)
+    return int(math.ceil(math.sqrt(40.0 * math.log(2.0) / c)))
 
 
 def thresholds(L: float, alpha: float):
     """(M, T): T uint32 [2M], T_i = floor(2^32 * CDF(i)) of the 1-D discrete Gaussian on -M..M."""
-    c = np.pi ** 2 / (alpha * L * L)
+    c = math.pi * math.pi / (alpha * L * L)
     M = half_width(L, alpha)
     run, cum = 0.0, []
-    for i in range(2 * M + 1):             # ascending, sequential fp64 sum
-        run += float(np.exp(-c * float(i - M) ** 2))
+    for i in range(2 * M + 1):             # ascending, sequential fp64 sum; libm exp
+        d = float(i - M)
+        run += math.exp(-c * (d * d))
         cum.append(run)
     total = cum[-1]
-    T = np.array([int(np.floor(4294967296.0 * (s / total))) for s in cum[:-1]], dtype=np.uint64)
-    assert T.max() < 2 ** 32
+    # clamp: when the tail bins' mass is below fp64 resolution CDF_i rounds to 1 and the floor is 2^32
+    T = np.array([min(4294967295, int(math.floor(4294967296.0 * (s / total)))) for s in cum[:-1]], dtype=np.uint64)
     return M, T.astype(np.uint32)
 
 

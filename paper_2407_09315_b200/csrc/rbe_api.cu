@@ -7,6 +7,7 @@
 #include <cstring>
 #include <new>
 #include <string>
+#include <vector>
 
 #include "rbe_kernels.cuh"
 
@@ -58,6 +59,16 @@ struct rbe_ctx {
     cudaEvent_t ev_start = nullptr, ev_done = nullptr;
     cudaEvent_t ev_in[HOST_MAX_CHUNKS] = {}, ev_f[HOST_MAX_CHUNKS] = {};
 
+    // device sampler (Algorithm 1 step 1 on the GPU): integer inverse-CDF thresholds, built on the host
+    std::vector<uint32_t> sampler_T;
+    int32_t sampler_M = 0;
+    size_t off_T = 0, off_state = 0;
+
+    // one whole step (sampler + structure factor + force) as an instantiated CUDA graph
+    cudaStream_t s_cap = nullptr;
+    cudaGraph_t graph = nullptr;
+    cudaGraphExec_t graph_exec = nullptr;
+
     std::string err;
 };
 
@@ -88,6 +99,31 @@ double normaliser_S(double L, double alpha) {
         H += 2.0 * t;
     }
     return H * H * H - 1.0;
+}
+
+// Thresholds of the 1-D discrete Gaussian exp(-c m^2), c = pi^2 / (alpha L^2), on m = -M .. M
+// (reading Q17): M = ceil(sqrt(40 ln 2 / c)); p_i summed in ascending i in fp64;
+// T_i = min(2^32 - 1, floor(2^32 * CDF_i)) for i = 0 .. 2M - 1 (the last bin takes the rest).  Returns false
+// when the table would be unreasonably large (the device sampler is then unavailable).
+constexpr int32_t SAMPLER_M_MAX = 1 << 20;
+bool build_sampler_table(double L, double alpha, std::vector<uint32_t>& T, int32_t& M) {
+    const double c = rbe::PI_D * rbe::PI_D / (alpha * L * L);
+    const double m = std::ceil(std::sqrt(40.0 * std::log(2.0) / c));
+    if (!(m >= 1.0) || m > (double)SAMPLER_M_MAX) return false;
+    M = (int32_t)m;
+    std::vector<double> cum((size_t)2 * M + 1);
+    double run = 0.0;
+    for (int32_t i = 0; i <= 2 * M; ++i) {
+        const double d = (double)(i - M);
+        run += std::exp(-c * (d * d));
+        cum[i] = run;
+    }
+    T.resize((size_t)2 * M);
+    for (int32_t i = 0; i < 2 * M; ++i) {
+        const double t = std::floor(4294967296.0 * (cum[i] / run));
+        T[i] = t >= 4294967295.0 ? 4294967295u : (uint32_t)t;   // CDF_i can round to 1 in the far tail
+    }
+    return true;
 }
 
 // Shared-memory tile of the structure-factor kernel for a launch over n atoms: up to 4 windows of
@@ -184,6 +220,8 @@ rbe_status init_device(rbe_ctx* c) {
     c->off_grow = off; off = align_up(off + (size_t)c->sf_ngroups * P * sizeof(double2), 256);
     c->off_U = off;    off = align_up(off + sizeof(double), 256);
     c->off_ticket = off; off = align_up(off + (size_t)(c->sf_ngroups + 1) * sizeof(unsigned int), 256);
+    c->off_T = off;    off = align_up(off + c->sampler_T.size() * sizeof(uint32_t) + 4, 256);
+    c->off_state = off; off = align_up(off + 2 * sizeof(unsigned long long), 256);
     c->ws_bytes = off;
 
     c->stage_bytes = P * (sizeof(int4) + sizeof(double));
@@ -202,6 +240,21 @@ rbe::KTable k_table(rbe_ctx* c) {
     t.w_uniform = c->S / (double)c->P;
     t.L = c->L;
     return t;
+}
+
+// Algorithm 1 step 1 on the device.  from_state: (seed, step) come from the workspace and the
+// step is advanced by the kernel (graph replay); else they are the arguments.
+rbe_status launch_sampler(rbe_ctx* c, bool from_state, uint64_t seed, uint64_t step, cudaStream_t st) {
+    rbe::SampleParams p;
+    p.T = ws_ptr<uint32_t>(c, c->off_T);
+    p.M = c->sampler_M;
+    p.P = c->P;
+    p.kvec = ws_ptr<int4>(c, c->off_kvec);
+    p.state = from_state ? ws_ptr<unsigned long long>(c, c->off_state) : nullptr;
+    p.seed = seed; p.step = step;
+    rbe::sample_kernel<<<1, 1024, 0, st>>>(p);
+    RBE_CUDA(c, cudaGetLastError());
+    return RBE_OK;
 }
 
 // One launch of the structure-factor kernel over n atoms.  accumulate: add to the per-CTA rows
@@ -292,6 +345,7 @@ rbe_status rbe_create(rbe_ctx** out, int64_t N, double L, double alpha, int32_t 
     if (!c) return RBE_ERR_INVALID_ARG;
     c->N = N; c->L = L; c->alpha = alpha; c->P = P;
     c->S = normaliser_S(L, alpha);
+    if (!build_sampler_table(L, alpha, c->sampler_T, c->sampler_M)) { c->sampler_T.clear(); c->sampler_M = 0; }
     *out = c;
     return RBE_OK;
 }
@@ -309,6 +363,9 @@ rbe_status rbe_destroy(rbe_ctx* c) {
     }
     if (c->ev_start) cudaEventDestroy(c->ev_start);
     if (c->ev_done) cudaEventDestroy(c->ev_done);
+    if (c->graph_exec) cudaGraphExecDestroy(c->graph_exec);
+    if (c->graph) cudaGraphDestroy(c->graph);
+    if (c->s_cap) cudaStreamDestroy(c->s_cap);
     if (c->s_h2d) cudaStreamDestroy(c->s_h2d);
     if (c->s_d2h) cudaStreamDestroy(c->s_d2h);
     delete c;
@@ -333,6 +390,11 @@ rbe_status rbe_set_workspace(rbe_ctx* c, void* d_ws, size_t bytes) {
     c->have_k = c->have_w = c->have_rho = false;
     // the structure-factor kernel's completion ticket starts at zero and resets itself
     RBE_CUDA(c, cudaMemset(c->ws + c->off_ticket, 0, (size_t)(c->sf_ngroups + 1) * sizeof(unsigned int)));
+    if (!c->sampler_T.empty())
+        RBE_CUDA(c, cudaMemcpy(c->ws + c->off_T, c->sampler_T.data(), c->sampler_T.size() * sizeof(uint32_t), cudaMemcpyHostToDevice));
+    RBE_CUDA(c, cudaMemset(c->ws + c->off_state, 0, 2 * sizeof(unsigned long long)));
+    if (c->graph_exec) { cudaGraphExecDestroy(c->graph_exec); c->graph_exec = nullptr; }   // bound to the old workspace
+    if (c->graph) { cudaGraphDestroy(c->graph); c->graph = nullptr; }
     RBE_CUDA(c, cudaDeviceSynchronize());
     return RBE_OK;
 }
@@ -431,6 +493,61 @@ rbe_status rbe_kspace_energy(rbe_ctx* c, double* h_U, void* stream) {
     RBE_CUDA(c, cudaMemcpyAsync(c->h_U_pinned, c->ws + c->off_U, sizeof(double), cudaMemcpyDeviceToHost, st));
     RBE_CUDA(c, cudaStreamSynchronize(st));
     *h_U = *c->h_U_pinned;
+    return RBE_OK;
+}
+
+rbe_status rbe_sample_kvectors(rbe_ctx* c, uint64_t seed, uint64_t step, void* stream) {
+    if (!c) return RBE_ERR_INVALID_ARG;
+    if (!c->ws) return fail(c, RBE_ERR_NOT_READY, "rbe_sample_kvectors before rbe_set_workspace");
+    if (c->sampler_T.empty()) return fail(c, RBE_ERR_INVALID_ARG, "rbe_sample_kvectors: the inverse-CDF table for this L, alpha is too large");
+    rbe_status s = launch_sampler(c, false, seed, step, static_cast<cudaStream_t>(stream));
+    if (s != RBE_OK) return s;
+    c->have_k = true; c->have_w = false; c->have_rho = false;
+    return RBE_OK;
+}
+
+rbe_status rbe_get_kvectors(rbe_ctx* c, int32_t* h_m, void* stream) {
+    if (!c || !h_m) return fail(c, RBE_ERR_INVALID_ARG, "rbe_get_kvectors: null argument");
+    if (!c->ws || !c->have_k) return fail(c, RBE_ERR_NOT_READY, "rbe_get_kvectors: no k-set");
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    std::vector<int4> tmp((size_t)c->P);
+    RBE_CUDA(c, cudaMemcpyAsync(tmp.data(), c->ws + c->off_kvec, tmp.size() * sizeof(int4), cudaMemcpyDeviceToHost, st));
+    RBE_CUDA(c, cudaStreamSynchronize(st));
+    for (int32_t l = 0; l < c->P; ++l) { h_m[3 * l] = tmp[l].x; h_m[3 * l + 1] = tmp[l].y; h_m[3 * l + 2] = tmp[l].z; }
+    return RBE_OK;
+}
+
+rbe_status rbe_graph_capture(rbe_ctx* c, const void* d_xyzq, void* d_force, int32_t with_energy, uint64_t seed,
+                             uint64_t first_step) {
+    if (!c) return RBE_ERR_INVALID_ARG;
+    if (!c->ws) return fail(c, RBE_ERR_NOT_READY, "rbe_graph_capture before rbe_set_workspace");
+    if (c->sampler_T.empty()) return fail(c, RBE_ERR_INVALID_ARG, "rbe_graph_capture: the device sampler is unavailable for this L, alpha");
+    if (c->N > 0 && (!d_xyzq || !d_force || (reinterpret_cast<uintptr_t>(d_xyzq) & 15u) || (reinterpret_cast<uintptr_t>(d_force) & 15u)))
+        return fail(c, RBE_ERR_INVALID_ARG, "rbe_graph_capture: null or misaligned pointer");
+    if (c->graph_exec) { cudaGraphExecDestroy(c->graph_exec); c->graph_exec = nullptr; }
+    if (c->graph) { cudaGraphDestroy(c->graph); c->graph = nullptr; }
+    if (!c->s_cap) RBE_CUDA(c, cudaStreamCreateWithFlags(&c->s_cap, cudaStreamNonBlocking));
+    const unsigned long long st8[2] = {seed, first_step};
+    RBE_CUDA(c, cudaMemcpy(c->ws + c->off_state, st8, sizeof(st8), cudaMemcpyHostToDevice));
+    RBE_CUDA(c, cudaStreamBeginCapture(c->s_cap, cudaStreamCaptureModeThreadLocal));
+    rbe_status s = launch_sampler(c, true, 0, 0, c->s_cap);
+    c->have_w = false;   // the graph's batch carries the uniform weights S / P
+    if (s == RBE_OK) s = launch_sf(c, d_xyzq, c->N, 0, 1, nullptr, c->s_cap);
+    if (s == RBE_OK && c->N > 0) s = launch_f(c, d_xyzq, d_force, c->N, with_energy, c->s_cap);
+    cudaGraph_t g = nullptr;
+    const cudaError_t e = cudaStreamEndCapture(c->s_cap, &g);
+    if (s != RBE_OK) { if (g) cudaGraphDestroy(g); return s; }
+    if (e != cudaSuccess) return cuda_fail(c, "cudaStreamEndCapture", e);
+    c->graph = g;
+    RBE_CUDA(c, cudaGraphInstantiate(&c->graph_exec, c->graph, 0));
+    return RBE_OK;
+}
+
+rbe_status rbe_graph_launch(rbe_ctx* c, void* stream) {
+    if (!c) return RBE_ERR_INVALID_ARG;
+    if (!c->graph_exec) return fail(c, RBE_ERR_NOT_READY, "rbe_graph_launch before rbe_graph_capture");
+    RBE_CUDA(c, cudaGraphLaunch(c->graph_exec, static_cast<cudaStream_t>(stream)));
+    c->have_k = true; c->have_w = false; c->have_rho = true;
     return RBE_OK;
 }
 

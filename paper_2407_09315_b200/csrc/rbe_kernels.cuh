@@ -614,4 +614,73 @@ __global__ void __launch_bounds__(F_THREADS, F_CTAS_PER_SM) f_kernel(const FPara
     }
 }
 
+// ---------------------------------------------------------------------------------------
+// Sampler kernel -- Algorithm 1 step 1 on the device: P iid draws of m != 0 with
+// probability ~ exp(-|2 pi m / L|^2 / 4 alpha).  DESIGN.md readings Q2 (exact iid draws by
+// per-dimension inverse CDF, the zero triple rejected) and Q17 (the random numbers):
+//   candidate j of step t = first three words of Philox4x32-10, counter (j, t), key = seed;
+//   m_d = #{ i : T_i <= word_d } - M with the host-built integer thresholds T (rbe_api.cu);
+//   the batch = the first P non-zero candidates in order of j.
+// One CTA; candidates are taken 1024 at a time and compacted by ballot + prefix sums, so the
+// result is exactly the sequential definition.  If `state` is given, (seed, step) are read
+// from it and the step is advanced after the draw (graph replay: no host involvement).
+// ---------------------------------------------------------------------------------------
+struct SampleParams {
+    const uint32_t* T;             // [2M] thresholds
+    int32_t M, P;
+    int4* kvec;                    // [P] out
+    unsigned long long* state;     // {seed, step} on the device, or nullptr
+    unsigned long long seed, step; // used when state == nullptr
+};
+
+__device__ __forceinline__ uint4 philox4x32_10(uint4 c, uint2 k) {
+#pragma unroll
+    for (int r = 0; r < 10; ++r) {
+        const uint32_t hi0 = __umulhi(0xD2511F53u, c.x), lo0 = 0xD2511F53u * c.x;
+        const uint32_t hi1 = __umulhi(0xCD9E8D57u, c.z), lo1 = 0xCD9E8D57u * c.z;
+        c = make_uint4(hi1 ^ c.y ^ k.x, lo1, hi0 ^ c.w ^ k.y, lo0);
+        k.x += 0x9E3779B9u; k.y += 0xBB67AE85u;
+    }
+    return c;
+}
+
+__device__ __forceinline__ int sample_dim(const uint32_t* T, int M, uint32_t x) {
+    int lo = 0, hi = 2 * M;      // #{ i in [0, 2M) : T_i <= x }
+    while (lo < hi) {
+        const int mid = (lo + hi) >> 1;
+        if (__ldg(&T[mid]) <= x) lo = mid + 1; else hi = mid;
+    }
+    return lo - M;
+}
+
+__global__ void __launch_bounds__(1024) sample_kernel(const SampleParams p) {
+    __shared__ uint32_t wsum[32];
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const unsigned long long seed = p.state ? p.state[0] : p.seed;
+    const unsigned long long step = p.state ? p.state[1] : p.step;
+    const uint2 key = make_uint2((uint32_t)seed, (uint32_t)(seed >> 32));
+    int accepted = 0;
+    for (unsigned long long j0 = 0; accepted < p.P; j0 += 1024) {
+        const unsigned long long j = j0 + tid;
+        const uint4 w = philox4x32_10(make_uint4((uint32_t)j, (uint32_t)(j >> 32), (uint32_t)step, (uint32_t)(step >> 32)), key);
+        const int mx = sample_dim(p.T, p.M, w.x), my = sample_dim(p.T, p.M, w.y), mz = sample_dim(p.T, p.M, w.z);
+        const bool nz = (mx | my | mz) != 0;
+        const uint32_t bal = __ballot_sync(FULL_MASK, nz);
+        if (lane == 0) wsum[warp] = __popc(bal);
+        __syncthreads();
+        int before = 0, total = 0;
+#pragma unroll
+        for (int i = 0; i < 32; ++i) {
+            const int v = (int)wsum[i];
+            before += i < warp ? v : 0;
+            total += v;
+        }
+        const int pos = accepted + before + __popc(bal & ((1u << lane) - 1u));
+        if (nz && pos < p.P) p.kvec[pos] = make_int4(mx, my, mz, 0);
+        accepted += total;
+        __syncthreads();
+    }
+    if (p.state && tid == 0) p.state[1] = step + 1;
+}
+
 }  // namespace rbe

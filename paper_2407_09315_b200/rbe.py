@@ -64,6 +64,15 @@ def lib():
         L.rbe_get_launch_info.argtypes = [vp, ctypes.POINTER(LaunchInfo)]
         L.rbe_set_kvectors.restype = ctypes.c_int
         L.rbe_set_kvectors.argtypes = [vp, vp, vp, vp]
+        u64 = ctypes.c_uint64
+        L.rbe_sample_kvectors.restype = ctypes.c_int
+        L.rbe_sample_kvectors.argtypes = [vp, u64, u64, vp]
+        L.rbe_get_kvectors.restype = ctypes.c_int
+        L.rbe_get_kvectors.argtypes = [vp, vp, vp]
+        L.rbe_graph_capture.restype = ctypes.c_int
+        L.rbe_graph_capture.argtypes = [vp, vp, vp, i32, u64, u64]
+        L.rbe_graph_launch.restype = ctypes.c_int
+        L.rbe_graph_launch.argtypes = [vp, vp]
         L.rbe_structure_factor.restype = ctypes.c_int
         L.rbe_structure_factor.argtypes = [vp, vp, vp, vp]
         L.rbe_set_rho.restype = ctypes.c_int
@@ -186,6 +195,26 @@ class Rbe:
         ww = None if w is None else np.ascontiguousarray(w, dtype=np.float64)
         assert ww is None or ww.shape == (self.P,)
         self._check(lib().rbe_set_kvectors(self._h, _np_ptr(mm), _np_ptr(ww), _stream_ptr(stream)))
+
+    def rbe_sample_kvectors(self, seed: int, step: int, stream=None):
+        self._check(lib().rbe_sample_kvectors(self._h, int(seed), int(step), _stream_ptr(stream)))
+
+    def rbe_get_kvectors(self, stream=None):
+        """numpy int32 [P,3]: the current k-set (synchronises)."""
+        import numpy as np
+        m = np.empty((self.P, 3), dtype=np.int32)
+        self._check(lib().rbe_get_kvectors(self._h, _np_ptr(m), _stream_ptr(stream)))
+        return m
+
+    def rbe_graph_capture(self, xyzq, force, with_energy: bool, seed: int, first_step: int):
+        _check_tensor(xyzq, (self.N, 4), "float32")
+        _check_tensor(force, (self.N, 4), "float32")
+        self._graph_buffers = (xyzq, force)   # the graph is bound to these: keep them alive
+        self._check(lib().rbe_graph_capture(self._h, ctypes.c_void_p(xyzq.data_ptr()), ctypes.c_void_p(force.data_ptr()),
+                                            int(bool(with_energy)), int(seed), int(first_step)))
+
+    def rbe_graph_launch(self, stream=None):
+        self._check(lib().rbe_graph_launch(self._h, _stream_ptr(stream)))
 
     def rbe_structure_factor(self, xyzq, rho=None, stream=None):
         """xyzq: cuda float32 [N,4]; rho: cuda float64 [P,2] or None."""

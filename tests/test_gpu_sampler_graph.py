@@ -1,0 +1,86 @@
+"""Device sampler (Algorithm 1 step 1 on the GPU, bit-exact against oracle/sampler.py) and the
+graph-captured whole step (sampler + structure factor + force in one launch)."""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+from oracle import sampler as osampler
+from paper_2407_09315_b200 import inputs, rbe
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.mark.parametrize("L,alpha,P,seed,step", [
+    (31.04, 0.09, 100, 1, 0),
+    (215.443, 0.09, 200, 3, 17),
+    (6.0, 0.3, 200, 7, 3),                     # zero triples are frequent: the rejection rule matters
+    (1000.0, 0.09, 1600, 5, (1 << 40) + 3),    # widest table of the sweep; high word of the step
+    (98.65, 0.09, 5000, (1 << 35) + 9, 2),     # several 1024-candidate rounds; high word of the seed
+    (4.0, 0.05, 1, 2, 2),                      # M = 1: the smallest table; P = 1
+])
+def test_device_sampler_is_bit_exact(L, alpha, P, seed, step):
+    ctx = rbe.Rbe(64, L, alpha, P)
+    ctx.rbe_sample_kvectors(seed, step)
+    got = ctx.rbe_get_kvectors()
+    want = osampler.sample_kset(L, alpha, P, seed, step)
+    assert got.dtype == np.int32 and np.array_equal(got, want)
+    assert np.all(np.any(got != 0, axis=1))
+
+
+def test_sampled_step_matches_oracle_and_host_fed_path():
+    cfg = inputs.CONFIGS["water_96k"]
+    atoms = inputs.make_atoms(cfg)
+    x = torch.from_numpy(atoms).cuda()
+    F1 = torch.empty((cfg.N, 4), dtype=torch.float32, device="cuda")
+    F2 = torch.empty_like(F1)
+    ctx = rbe.Rbe(cfg.N, cfg.L, cfg.alpha, cfg.P)
+    ctx.rbe_sample_kvectors(42, 5)
+    ctx.rbe_structure_factor(x)
+    ctx.rbe_forces(x, F1, True)
+    U1 = ctx.rbe_kspace_energy()
+    m = osampler.sample_kset(cfg.L, cfg.alpha, cfg.P, 42, 5)
+    ctx.rbe_set_kvectors(m)                       # the same batch handed over from the host
+    ctx.rbe_structure_factor(x)
+    ctx.rbe_forces(x, F2, True)
+    assert torch.equal(F1, F2) and ctx.rbe_kspace_energy() == U1
+    S = oracle.S(cfg.L, cfg.alpha)
+    rho_o = oracle.rho(atoms, cfg.L, m)
+    F_o = oracle.force(atoms, cfg.L, m, S, rho_o)
+    assert np.linalg.norm(F1.cpu().numpy()[:, :3] - F_o) / np.linalg.norm(F_o) <= 2e-5
+    assert abs(U1 - oracle.energy(cfg.L, m, S, rho_o)) <= 1e-5 * abs(U1)
+
+
+@pytest.mark.parametrize("name", ["water_3k", "water_96k"])
+def test_graph_replay_advances_the_step_and_matches_separate_launches(name):
+    cfg = inputs.CONFIGS[name]
+    atoms = inputs.make_atoms(cfg)
+    x = torch.from_numpy(atoms).cuda()
+    Fg = torch.full((cfg.N, 4), float("nan"), dtype=torch.float32, device="cuda")
+    Fs = torch.empty_like(Fg)
+    ctx = rbe.Rbe(cfg.N, cfg.L, cfg.alpha, cfg.P)
+    ref = rbe.Rbe(cfg.N, cfg.L, cfg.alpha, cfg.P)
+    with pytest.raises(rbe.RbeError):
+        ctx.rbe_graph_launch()
+    ctx.rbe_graph_capture(x, Fg, True, seed=9, first_step=5)
+    S = oracle.S(cfg.L, cfg.alpha)
+    for step in (5, 6, 7):
+        ctx.rbe_graph_launch()
+        torch.cuda.synchronize()
+        m = ctx.rbe_get_kvectors()
+        assert np.array_equal(m, osampler.sample_kset(cfg.L, cfg.alpha, cfg.P, 9, step))
+        ref.rbe_sample_kvectors(9, step)
+        ref.rbe_structure_factor(x)
+        ref.rbe_forces(x, Fs, True)
+        assert torch.equal(Fg, Fs)
+        assert ctx.rbe_kspace_energy() == ref.rbe_kspace_energy()
+        rho_o = oracle.rho(atoms, cfg.L, m)
+        F_o = oracle.force(atoms, cfg.L, m, S, rho_o)
+        assert np.linalg.norm(Fg.cpu().numpy()[:, :3] - F_o) / np.linalg.norm(F_o) <= 2e-5
+    # positions may change between replays (the graph is bound to the buffer, not its contents)
+    x.add_(0.25)
+    ctx.rbe_graph_launch()
+    ref.rbe_sample_kvectors(9, 8)
+    ref.rbe_structure_factor(x)
+    ref.rbe_forces(x, Fs, True)
+    assert torch.equal(Fg, Fs)
