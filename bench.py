@@ -172,6 +172,8 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-graph", action="store_true")
+    ap.add_argument("--exchange", default="fused", choices=["fused", "nccl"],
+                    help="N > 1: how the structure factors are summed across ranks")
     ap.add_argument("--with-energy", action="store_true")
     args = ap.parse_args()
     if args.impl == "reference":
@@ -204,6 +206,22 @@ def main():
 
     ctx = rbe.Rbe(n_local, L, alpha, P)
     info = ctx.rbe_get_launch_info()
+    # N > 1: the P complex structure factors are exchanged INSIDE the kernels over NVLink peer
+    # memory (rbe_set_exchange); NCCL all_gather + rbe_set_rho only if symmetric memory is unavailable
+    fused = False
+    if world > 1 and args.exchange == "fused":
+        ok = torch.ones(1, device="cuda")
+        try:
+            from paper_2407_09315_b200 import exchange
+            exchange.setup_fused_exchange(ctx)
+        except Exception as e:  # noqa: BLE001 - any failure here means "no peer mapping": use NCCL
+            ok.zero_()
+            if rank == 0:
+                print(f"bench: fused exchange unavailable ({type(e).__name__}: {e}); using NCCL all_gather", file=sys.stderr)
+        dist.all_reduce(ok, op=dist.ReduceOp.MIN)
+        fused = bool(ok.item() > 0)
+        if not fused:
+            ctx.rbe_set_exchange(0, 0, None, 0)
     # inputs larger than L2: rotate over enough {xyzq, force} buffer pairs to exceed 126 MB
     n_rot = max(2, int(np.ceil(160e6 / max(1, 32 * n_local))))
     n_rot = min(n_rot, 64)
@@ -218,8 +236,8 @@ def main():
         x, f = xs[i % n_rot], fs[i % n_rot]
         ctx.rbe_set_kvectors(ksets[i % n_k])
         if ev: ev[0].record()
-        ctx.rbe_structure_factor(x, rho_local if world > 1 else None)
-        if world > 1:
+        ctx.rbe_structure_factor(x, rho_local if world > 1 and not fused else None)
+        if world > 1 and not fused:
             dist.all_gather_into_tensor(gathered, rho_local)
             ctx.rbe_set_rho(gathered.sum(0))  # fixed (rank) order
         if ev: ev[1].record()
@@ -257,6 +275,8 @@ def main():
         step(args.warmup + i, evs[i])
     sync()
     clocks = sampler.stop() if rank == 0 else None
+    if fused:
+        ctx.rbe_exchange_check()   # raises if any kernel gave up waiting for a peer
     t_sf = [e[0].elapsed_time(e[1]) for e in evs]
     t_f = [e[1].elapsed_time(e[2]) for e in evs]
     ms_sf, ms_f = sum(t_sf) / len(t_sf), sum(t_f) / len(t_f)
@@ -316,9 +336,10 @@ def main():
             def e2e_step(i):
                 dx.copy_(hx, non_blocking=True)
                 ctx.rbe_set_kvectors(ksets[i % n_k])
-                ctx.rbe_structure_factor(dx, rho_local)
-                dist.all_gather_into_tensor(gathered, rho_local)
-                ctx.rbe_set_rho(gathered.sum(0))
+                ctx.rbe_structure_factor(dx, None if fused else rho_local)
+                if not fused:
+                    dist.all_gather_into_tensor(gathered, rho_local)
+                    ctx.rbe_set_rho(gathered.sum(0))
                 ctx.rbe_forces(dx, df, args.with_energy)
                 hf.copy_(df, non_blocking=True)
                 torch.cuda.current_stream().synchronize()
@@ -359,7 +380,9 @@ def main():
         "vs_baseline": None, "dtype": "f32", "data": "synthetic",
         "config": {"workload": base.name, "N_per_gpu": n_local, "N_total": n_total, "P": P, "L": L, "alpha": alpha,
                    "l2": f"inputs rotate over {n_rot} buffer sets ({32 * n_local * n_rot / 1e6:.0f} MB > 126 MB L2)",
-                   "parallelism": f"atoms sharded over {world} GPU(s), k-set replicated",
+                   "parallelism": f"atoms sharded over {world} GPU(s), k-set replicated" + (
+                       "" if world == 1 else ", rho exchanged inside the kernels over NVLink peer memory (rbe_set_exchange)"
+                       if fused else ", rho exchanged with NCCL all_gather + rank-ordered sum"),
                    "launch": info, "with_energy": bool(args.with_energy)},
         "kernels_ms": {"structure_factor_call": ms_sf, "forces_call": ms_f,
                        "note": "region B (CUDA events around each C-ABI call); structure_factor_call = sf_kernel "

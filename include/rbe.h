@@ -162,6 +162,27 @@ rbe_status rbe_structure_factor(rbe_ctx* ctx, const void* d_xyzq, void* d_rho, v
  * Errors: RBE_ERR_NOT_READY, RBE_ERR_INVALID_ARG, RBE_ERR_CUDA. */
 rbe_status rbe_set_rho(rbe_ctx* ctx, const void* d_rho, void* stream);
 
+/* Fused multi-GPU exchange of the structure factors (one process per GPU, atoms sharded over the
+ * ranks, the k-set replicated: same seed or same host k-set on every rank).  The paper has no
+ * multi-GPU path (future work); what must be exchanged is the sum of P complex numbers
+ * (P:137).  Each rank owns one exchange buffer of rbe_exchange_bytes(ctx, world) bytes that every
+ * peer can address (NVLink peer mapping, e.g. a torch symmetric-memory allocation), zero-filled
+ * before the first step.  With an exchange configured, rbe_structure_factor's last CTA writes
+ * this rank's partial rho into its slot of EVERY rank's buffer and releases a per-rank flag;
+ * rbe_forces / rbe_kspace_energy wait for all `world` flags of the step and add the slots in rank
+ * order (bitwise the same rho on every rank): no collective call, no extra launch.  The d_rho copy
+ * of rbe_structure_factor then holds this rank's PARTIAL sum.  All ranks must run the same
+ * sequence of steps.  A kernel that waits longer than 10 s for a peer gives up and raises a flag
+ * that rbe_exchange_check reports (it never hangs the GPU).
+ *   d_bufs  host array of `world` device pointers, d_bufs[r] = rank r's buffer as mapped in THIS
+ *           process (d_bufs[rank] is the local one), each 256-byte aligned, `bytes` long.
+ * rbe_set_exchange with world < 1 or d_bufs == NULL switches the exchange off.  Not combinable with
+ * rbe_set_rho or rbe_graph_capture (RBE_ERR_INVALID_ARG).
+ * Errors: RBE_ERR_INVALID_ARG, RBE_ERR_WORKSPACE (bytes too small), RBE_ERR_CUDA. */
+size_t     rbe_exchange_bytes(const rbe_ctx* ctx, int32_t world);
+rbe_status rbe_set_exchange(rbe_ctx* ctx, int32_t rank, int32_t world, void* const* d_bufs, size_t bytes);
+rbe_status rbe_exchange_check(rbe_ctx* ctx, void* stream);   /* synchronises `stream` */
+
 /* Algorithm 1 step 4, Eq. (2.12): forces on this context's N atoms from the
  * current k-set and structure factors.
  *   d_xyzq   float4 [N], device: the same positions the structure factor was computed from.

@@ -69,6 +69,12 @@ struct rbe_ctx {
     cudaGraph_t graph = nullptr;
     cudaGraphExec_t graph_exec = nullptr;
 
+    // fused multi-GPU exchange of rho (rbe_set_exchange): peers' buffers, this rank, step epoch
+    int32_t xch_world = 0, xch_rank = 0;
+    uint32_t xch_epoch = 0;
+    unsigned char* xch_buf[rbe::MAX_WORLD] = {};
+    size_t off_xch_err = 0;
+
     std::string err;
 };
 
@@ -222,6 +228,7 @@ rbe_status init_device(rbe_ctx* c) {
     c->off_ticket = off; off = align_up(off + (size_t)(c->sf_ngroups + 1) * sizeof(unsigned int), 256);
     c->off_T = off;    off = align_up(off + c->sampler_T.size() * sizeof(uint32_t) + 4, 256);
     c->off_state = off; off = align_up(off + 2 * sizeof(unsigned long long), 256);
+    c->off_xch_err = off; off = align_up(off + sizeof(int32_t), 256);
     c->ws_bytes = off;
 
     c->stage_bytes = P * (sizeof(int4) + sizeof(double));
@@ -232,6 +239,9 @@ rbe_status init_device(rbe_ctx* c) {
 template <typename T>
 T* ws_ptr(rbe_ctx* c, size_t off) { return reinterpret_cast<T*>(c->ws + off); }
 
+// exchange buffer layout: slots [2][world][P] double2, then flags [2][world] uint32
+size_t xch_flags_offset(int32_t world, int32_t P) { return align_up((size_t)2 * world * P * sizeof(double2), 256); }
+
 rbe::KTable k_table(rbe_ctx* c) {
     rbe::KTable t;
     t.kvec = ws_ptr<int4>(c, c->off_kvec);
@@ -239,6 +249,17 @@ rbe::KTable k_table(rbe_ctx* c) {
     t.rho = ws_ptr<double2>(c, c->off_rho);
     t.w_uniform = c->S / (double)c->P;
     t.L = c->L;
+    t.P = c->P;
+    t.xch.world = c->xch_world;
+    t.xch.epoch = c->xch_epoch;
+    t.xch.slots = nullptr; t.xch.flags = nullptr;
+    t.xch.error = ws_ptr<int32_t>(c, c->off_xch_err);
+    if (c->xch_world > 0) {
+        const size_t parity = c->xch_epoch & 1u;
+        unsigned char* own = c->xch_buf[c->xch_rank];
+        t.xch.slots = reinterpret_cast<const double2*>(own) + parity * (size_t)c->xch_world * (size_t)c->P;
+        t.xch.flags = reinterpret_cast<const uint32_t*>(own + xch_flags_offset(c->xch_world, c->P)) + parity * (size_t)c->xch_world;
+    }
     return t;
 }
 
@@ -278,6 +299,18 @@ rbe_status launch_sf(rbe_ctx* c, const void* d_xyzq, int64_t n, int accumulate, 
     sp.red.tickets = ws_ptr<unsigned int>(c, c->off_ticket);
     sp.red.group_size = rbe::SF_RED_GROUP;
     sp.red.ngroups = c->sf_ngroups;
+    sp.red.xch.world = 0;
+    if (c->xch_world > 0 && finalise) {
+        // one epoch per structure factor; the consumers of this step (k_table) read the same epoch
+        const uint32_t epoch = ++c->xch_epoch;
+        const size_t parity = epoch & 1u, fo = xch_flags_offset(c->xch_world, c->P);
+        sp.red.xch.world = c->xch_world;
+        sp.red.xch.epoch = epoch;
+        for (int r = 0; r < c->xch_world; ++r) {
+            sp.red.xch.slot[r] = reinterpret_cast<double2*>(c->xch_buf[r]) + (parity * c->xch_world + c->xch_rank) * (size_t)c->P;
+            sp.red.xch.flag[r] = reinterpret_cast<uint32_t*>(c->xch_buf[r] + fo) + parity * c->xch_world + c->xch_rank;
+        }
+    }
 #ifdef RBE_SF_PROFILE
     static long long* d_prof = nullptr;
     if (!d_prof) cudaMalloc(&d_prof, 4096 * 64 * sizeof(long long));
@@ -393,6 +426,7 @@ rbe_status rbe_set_workspace(rbe_ctx* c, void* d_ws, size_t bytes) {
     if (!c->sampler_T.empty())
         RBE_CUDA(c, cudaMemcpy(c->ws + c->off_T, c->sampler_T.data(), c->sampler_T.size() * sizeof(uint32_t), cudaMemcpyHostToDevice));
     RBE_CUDA(c, cudaMemset(c->ws + c->off_state, 0, 2 * sizeof(unsigned long long)));
+    RBE_CUDA(c, cudaMemset(c->ws + c->off_xch_err, 0, sizeof(int32_t)));
     if (c->graph_exec) { cudaGraphExecDestroy(c->graph_exec); c->graph_exec = nullptr; }   // bound to the old workspace
     if (c->graph) { cudaGraphDestroy(c->graph); c->graph = nullptr; }
     RBE_CUDA(c, cudaDeviceSynchronize());
@@ -467,6 +501,7 @@ rbe_status rbe_set_rho(rbe_ctx* c, const void* d_rho, void* stream) {
     if (!c->ws || !c->have_k) return fail(c, RBE_ERR_NOT_READY, "rbe_set_rho needs a workspace and k-vectors");
     if (!d_rho || (reinterpret_cast<uintptr_t>(d_rho) & 15u))
         return fail(c, RBE_ERR_INVALID_ARG, "rbe_set_rho: null or misaligned pointer");
+    if (c->xch_world > 0) return fail(c, RBE_ERR_INVALID_ARG, "rbe_set_rho: a fused exchange is configured (rbe_set_exchange)");
     RBE_CUDA(c, cudaMemcpyAsync(c->ws + c->off_rho, d_rho, (size_t)c->P * sizeof(double2), cudaMemcpyDeviceToDevice,
                                 static_cast<cudaStream_t>(stream)));
     c->have_rho = true;
@@ -522,6 +557,7 @@ rbe_status rbe_graph_capture(rbe_ctx* c, const void* d_xyzq, void* d_force, int3
     if (!c) return RBE_ERR_INVALID_ARG;
     if (!c->ws) return fail(c, RBE_ERR_NOT_READY, "rbe_graph_capture before rbe_set_workspace");
     if (c->sampler_T.empty()) return fail(c, RBE_ERR_INVALID_ARG, "rbe_graph_capture: the device sampler is unavailable for this L, alpha");
+    if (c->xch_world > 0) return fail(c, RBE_ERR_INVALID_ARG, "rbe_graph_capture: not available with a fused exchange (the epoch is a launch argument)");
     if (c->N > 0 && (!d_xyzq || !d_force || (reinterpret_cast<uintptr_t>(d_xyzq) & 15u) || (reinterpret_cast<uintptr_t>(d_force) & 15u)))
         return fail(c, RBE_ERR_INVALID_ARG, "rbe_graph_capture: null or misaligned pointer");
     if (c->graph_exec) { cudaGraphExecDestroy(c->graph_exec); c->graph_exec = nullptr; }
@@ -548,6 +584,40 @@ rbe_status rbe_graph_launch(rbe_ctx* c, void* stream) {
     if (!c->graph_exec) return fail(c, RBE_ERR_NOT_READY, "rbe_graph_launch before rbe_graph_capture");
     RBE_CUDA(c, cudaGraphLaunch(c->graph_exec, static_cast<cudaStream_t>(stream)));
     c->have_k = true; c->have_w = false; c->have_rho = true;
+    return RBE_OK;
+}
+
+size_t rbe_exchange_bytes(const rbe_ctx* c, int32_t world) {
+    if (!c || world < 1 || world > rbe::MAX_WORLD) return 0;
+    return xch_flags_offset(world, c->P) + align_up((size_t)2 * world * sizeof(uint32_t), 256);
+}
+
+rbe_status rbe_set_exchange(rbe_ctx* c, int32_t rank, int32_t world, void* const* d_bufs, size_t bytes) {
+    if (!c) return RBE_ERR_INVALID_ARG;
+    if (world < 1 || !d_bufs) {   // switch the exchange off
+        c->xch_world = 0; c->xch_rank = 0;
+        return RBE_OK;
+    }
+    if (world > rbe::MAX_WORLD || rank < 0 || rank >= world)
+        return fail(c, RBE_ERR_INVALID_ARG, "rbe_set_exchange: need 0 <= rank < world <= " + std::to_string(rbe::MAX_WORLD));
+    if (bytes < rbe_exchange_bytes(c, world)) return fail(c, RBE_ERR_WORKSPACE, "rbe_set_exchange: buffers smaller than rbe_exchange_bytes");
+    for (int r = 0; r < world; ++r)
+        if (!d_bufs[r] || (reinterpret_cast<uintptr_t>(d_bufs[r]) & 255u))
+            return fail(c, RBE_ERR_INVALID_ARG, "rbe_set_exchange: null or misaligned buffer of rank " + std::to_string(r));
+    for (int r = 0; r < world; ++r) c->xch_buf[r] = static_cast<unsigned char*>(d_bufs[r]);
+    c->xch_world = world; c->xch_rank = rank; c->xch_epoch = 0;
+    c->have_rho = false;
+    return RBE_OK;
+}
+
+rbe_status rbe_exchange_check(rbe_ctx* c, void* stream) {
+    if (!c) return RBE_ERR_INVALID_ARG;
+    if (!c->ws) return fail(c, RBE_ERR_NOT_READY, "rbe_exchange_check before rbe_set_workspace");
+    int32_t e = 0;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    RBE_CUDA(c, cudaMemcpyAsync(&e, c->ws + c->off_xch_err, sizeof(e), cudaMemcpyDeviceToHost, st));
+    RBE_CUDA(c, cudaStreamSynchronize(st));
+    if (e) return fail(c, RBE_ERR_CUDA, "fused exchange: a peer's structure factors did not arrive within 10 s");
     return RBE_OK;
 }
 

@@ -100,17 +100,83 @@ __device__ __forceinline__ void grid_launch_dependents() { asm volatile("griddep
 // operations per k, in parallel over the CTAs), so the serial tail of the structure-factor
 // kernel is only the reduction.
 // ---------------------------------------------------------------------------------------
+constexpr int MAX_WORLD = 16;   // ranks (GPUs) one fused exchange can span
+
+// Fused multi-GPU exchange of the structure factors.  Every rank
+// owns an exchange buffer that its peers can write (NVLink peer mapping):
+//   slots [2][world][P] double2   -- slot (parity, r) = rank r's partial rho of a step with that parity
+//   flags [2][world]    uint32    -- epoch of the step whose partial is complete in that slot
+// The structure-factor kernel of rank r PUSHES its partial into slot (parity, r) of every rank and
+// then releases the flag; the consumers (force / energy kernels) of every rank WAIT for all `world`
+// flags of the step and add the slots in rank order, so every rank gets the bitwise identical
+// global rho without a collective call or an extra launch.  Two parities: a rank can run at most
+// one step ahead of a peer that is still reading (it cannot finish step n+1 before that peer has
+// pushed step n+1, which the peer does only after its own step-n force kernel).
+struct XchPush {                  // writer side (structure-factor kernel)
+    int32_t world;                // 0: no exchange
+    uint32_t epoch;
+    double2* slot[MAX_WORLD];     // slot (parity, my rank) in rank r's buffer
+    uint32_t* flag[MAX_WORLD];    // flag (parity, my rank) in rank r's buffer
+};
+struct XchPull {                  // reader side (force / energy kernels): this rank's own buffer
+    int32_t world;
+    uint32_t epoch;
+    const double2* slots;         // [world][P] of this step's parity
+    const uint32_t* flags;        // [world]
+    int32_t* error;               // set to 1 if a flag did not arrive within XCH_TIMEOUT_NS
+};
+constexpr unsigned long long XCH_TIMEOUT_NS = 10ull * 1000 * 1000 * 1000;
+
+__device__ __forceinline__ uint32_t ld_acquire_sys(const uint32_t* p) {
+    uint32_t v;
+    asm volatile("ld.acquire.sys.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+    return v;
+}
+__device__ __forceinline__ void st_release_sys(uint32_t* p, uint32_t v) {
+    asm volatile("st.release.sys.global.u32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
+}
+__device__ __forceinline__ unsigned long long global_timer_ns() {
+    unsigned long long t;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+    return t;
+}
+
+// All threads of the CTA call this; returns when every rank's partial of this step has arrived.
+__device__ __forceinline__ void xch_wait(const XchPull& x) {
+    if (x.world < 1) return;
+    if ((int)threadIdx.x < x.world) {
+        const unsigned long long t0 = global_timer_ns();
+        while ((int32_t)(ld_acquire_sys(&x.flags[threadIdx.x]) - x.epoch) < 0) {
+            if (global_timer_ns() - t0 > XCH_TIMEOUT_NS) { *x.error = 1; break; }   // never hang the GPU
+            __nanosleep(100);
+        }
+    }
+    __syncthreads();
+}
+
 struct KTable {
     const int4* kvec;     // [P] {mx, my, mz, 0}
     const double* w;      // [P] or nullptr -> w_uniform
-    const double2* rho;   // [P]
+    const double2* rho;   // [P] (this rank's atoms only when an exchange is configured)
     double w_uniform;     // S / P
     double L;
+    int32_t P;
+    XchPull xch;          // world > 0: rho(k) = sum over ranks, in rank order, of the exchange slots
 };
+
+__device__ __forceinline__ double2 k_rho(const KTable& t, int k) {
+    if (t.xch.world < 1) return t.rho[k];
+    double re = 0.0, im = 0.0;
+    for (int r = 0; r < t.xch.world; ++r) {
+        const double2 v = __ldcg(&t.xch.slots[(int64_t)r * t.P + k]);   // written by a peer: not through L1
+        re += v.x; im += v.y;
+    }
+    return make_double2(re, im);
+}
 
 __device__ __forceinline__ void k_record(const KTable& t, int k, int4& ka, float4& kb) {
     const int4 m = t.kvec[k];
-    const double2 r = t.rho[k];
+    const double2 r = k_rho(t, k);
     const double w = t.w ? t.w[k] : t.w_uniform;
     const double m2 = (double)m.x * m.x + (double)m.y * m.y + (double)m.z * m.z;
     const double mag = sqrt(r.x * r.x + r.y * r.y);
@@ -124,10 +190,11 @@ __device__ __forceinline__ void k_record(const KTable& t, int k, int4& ka, float
 // U = sum_l e_l |rho_l|^2 in a fixed order (thread-strided partials, then a fixed tree).
 __global__ void __launch_bounds__(256) energy_kernel(const KTable t, int32_t P, double* U) {
     __shared__ double sh[256];
+    xch_wait(t.xch);
     double a = 0.0;
     for (int k = threadIdx.x; k < P; k += 256) {
         const int4 m = t.kvec[k];
-        const double2 r = t.rho[k];
+        const double2 r = k_rho(t, k);
         const double w = t.w ? t.w[k] : t.w_uniform;
         const double m2 = (double)m.x * m.x + (double)m.y * m.y + (double)m.z * m.z;
         a += w / (2.0 * PI_D * t.L * m2) * (r.x * r.x + r.y * r.y);
@@ -157,6 +224,7 @@ struct RedParams {
     double2* rho_user;    // [P] out, or nullptr
     unsigned int* tickets;  // [ngroups + 1], zero-initialised
     int32_t group_size, ngroups;
+    XchPush xch;          // world > 0: push rho to every rank's exchange buffer after the second pass
 };
 
 // dst[k] = sum_{row} src[row][k]: row slices sl, sl+nsl, ... sequentially, then the slices in order
@@ -486,6 +554,16 @@ __global__ void __launch_bounds__(SF_TMAX, SF_CTAS_PER_SM) sf_kernel(const SfPar
     RBE_STAMP();
     reduce_rows(rp.grow, rp.ngroups, p.P, rp.rho, rp.rho_user, acc_all, tid, T);
     RBE_STAMP();
+    if (rp.xch.world > 0) {
+        // fused exchange: this CTA (the last one of the grid) writes the partial rho into its slot on
+        // every rank over NVLink, then releases the per-rank flags (stores, fence, flag)
+        __syncthreads();
+        for (int r = 0; r < rp.xch.world; ++r)
+            for (int k = tid; k < p.P; k += T) rp.xch.slot[r][k] = __ldcg(&rp.rho[k]);
+        __threadfence_system();
+        __syncthreads();
+        if (tid < rp.xch.world) st_release_sys(rp.xch.flag[tid], rp.xch.epoch);
+    }
 }
 
 // ---------------------------------------------------------------------------------------
@@ -603,6 +681,7 @@ __global__ void __launch_bounds__(F_THREADS, F_CTAS_PER_SM) f_kernel(const FPara
     for (int r = 0; r < F_RMAX; ++r) pre[r] = r < r0 ? f_fetch(p, u0 + r, lane) : make_float4(0.f, 0.f, 0.f, 0.f);
 
     if (p.pdl) grid_dependency_wait();   // rho comes from the preceding grid
+    xch_wait(p.kt.xch);                  // ... and, with a multi-GPU exchange, from the peers' grids
 
     for (int k0 = 0; k0 < p.P; k0 += F_KCHUNK) {
         const int nk = (p.P - k0 < F_KCHUNK) ? (p.P - k0) : F_KCHUNK;

@@ -73,6 +73,12 @@ def lib():
         L.rbe_graph_capture.argtypes = [vp, vp, vp, i32, u64, u64]
         L.rbe_graph_launch.restype = ctypes.c_int
         L.rbe_graph_launch.argtypes = [vp, vp]
+        L.rbe_exchange_bytes.restype = sz
+        L.rbe_exchange_bytes.argtypes = [vp, i32]
+        L.rbe_set_exchange.restype = ctypes.c_int
+        L.rbe_set_exchange.argtypes = [vp, i32, i32, ctypes.POINTER(vp), sz]
+        L.rbe_exchange_check.restype = ctypes.c_int
+        L.rbe_exchange_check.argtypes = [vp, vp]
         L.rbe_structure_factor.restype = ctypes.c_int
         L.rbe_structure_factor.argtypes = [vp, vp, vp, vp]
         L.rbe_set_rho.restype = ctypes.c_int
@@ -215,6 +221,23 @@ class Rbe:
 
     def rbe_graph_launch(self, stream=None):
         self._check(lib().rbe_graph_launch(self._h, _stream_ptr(stream)))
+
+    def rbe_exchange_bytes(self, world: int) -> int:
+        return int(lib().rbe_exchange_bytes(self._h, int(world)))
+
+    def rbe_set_exchange(self, rank: int, world: int, buf_ptrs, nbytes: int, keep_alive=None):
+        """buf_ptrs: `world` device pointers (ints), buf_ptrs[r] = rank r's exchange buffer as mapped
+        in this process; None switches the exchange off."""
+        if buf_ptrs is None:
+            self._check(lib().rbe_set_exchange(self._h, 0, 0, None, 0))
+            self._xch_keep = None
+            return
+        arr = (ctypes.c_void_p * int(world))(*[int(p) for p in buf_ptrs])
+        self._check(lib().rbe_set_exchange(self._h, int(rank), int(world), arr, int(nbytes)))
+        self._xch_keep = keep_alive
+
+    def rbe_exchange_check(self, stream=None):
+        self._check(lib().rbe_exchange_check(self._h, _stream_ptr(stream)))
 
     def rbe_structure_factor(self, xyzq, rho=None, stream=None):
         """xyzq: cuda float32 [N,4]; rho: cuda float64 [P,2] or None."""
