@@ -1,6 +1,6 @@
 """fp64 CPU oracle for the RBE k-space path -- TEST INFRASTRUCTURE, NOT THE PRODUCT.
 
-Thin ctypes marshalling around ``rbe_oracle.c`` and ``ewald_ref.c`` (plain C, fp64, written
+Thin ctypes marshalling around ``rbe_oracle.c``, ``ewald_ref.c`` and ``short_range.c`` (plain C, fp64, written
 from /root/reference/PAPER.md; every function there cites the passage it follows).  No
 arithmetic of the method lives in this file.
 
@@ -18,7 +18,7 @@ import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SO = os.path.join(_HERE, "liboracle.so")
-_SRC = [os.path.join(_HERE, "rbe_oracle.c"), os.path.join(_HERE, "ewald_ref.c")]
+_SRC = [os.path.join(_HERE, "rbe_oracle.c"), os.path.join(_HERE, "ewald_ref.c"), os.path.join(_HERE, "short_range.c")]
 _lib = None
 
 
@@ -58,6 +58,8 @@ def _load():
     lib.oracle_ewald_full.argtypes = [c_i32, vp, vp, c_d, c_d, c_i32, c_i32, vp, vp, vp]
     lib.oracle_direct_image_sum.restype = None
     lib.oracle_direct_image_sum.argtypes = [c_i32, vp, vp, c_d, c_i32, vp, vp]
+    lib.oracle_short_range.restype = None
+    lib.oracle_short_range.argtypes = [c_i64, vp, c_d, c_d, c_d, c_i64, vp, vp, vp]
     _lib = lib
     return lib
 
@@ -151,3 +153,16 @@ def direct_image_sum(r, q, L: float, R: int):
     F = np.empty((n, 3), dtype=np.float64)
     _load().oracle_direct_image_sum(n, _p(rr), _p(qq), float(L), int(R), ctypes.byref(U), _p(F))
     return float(U.value), F
+
+
+def short_range(xyzq, L: float, alpha: float, rs: float, sel=None):
+    """Short-range Ewald force, Eq. (2.10), truncated at r_s (nearest image).  Returns
+    (F float64 [nsel,3], e float64 [nsel]) with sum(e) = U_short when sel is None."""
+    a = _xyzq(xyzq)
+    assert rs <= 0.5 * L + 1e-12, "reading Q18: r_s <= L/2"
+    ss = None if sel is None else np.ascontiguousarray(sel, dtype=np.int64)
+    nsel = a.shape[0] if ss is None else ss.shape[0]
+    F = np.empty((nsel, 3), dtype=np.float64)
+    e = np.empty((nsel,), dtype=np.float64)
+    _load().oracle_short_range(a.shape[0], _p(a), float(L), float(alpha), float(rs), nsel, _p(ss), _p(F), _p(e))
+    return F, e
