@@ -193,6 +193,27 @@ rbe_status rbe_exchange_check(rbe_ctx* ctx, void* stream);   /* synchronises `st
 rbe_status rbe_forces(rbe_ctx* ctx, const void* d_xyzq, void* d_force, int32_t with_energy,
                       void* stream);
 
+/* Real-space partner of the RBE force: the short-range part of the Ewald-split Coulomb force,
+ * Eq. (2.10), truncated at the cutoff radius r_s, over a linked-cell list of cubic
+ * cells of side >= r_s (the cell list of Algorithm 2):
+ *   F_i = - q_i sum_{j != i, r < r_s} q_j ( erfc(sqrt(alpha) r) / r^2
+ *            + 2 sqrt(alpha) exp(-alpha r^2) / (sqrt(pi) r) ) d / r,   d = nearest image of r_j - r_i
+ *   e_i = 1/2 q_i sum_{j != i, r < r_s} q_j erfc(sqrt(alpha) r) / r      (first term of Eq. 2.8)
+ * with this context's L and alpha.  Coincident atoms (r = 0) are skipped.  Independent of the
+ * k-set; needs no rbe_set_workspace.  fp32 arithmetic on exact fixed-point separations; erfc by
+ * Abramowitz-Stegun 7.1.26 (|error| <= 1.5e-7); every atom's sum runs in a fixed order (cells sorted
+ * by atom index), so the result is bitwise reproducible.
+ *   d_xyzq      float4 [N] device;  rs  cutoff radius [A], 0 < rs <= L/3
+ *   d_force     float4 [N] device: {F_x, F_y, F_z, e_i}; e_i = 0 unless with_energy != 0
+ *   accumulate  != 0: add to what d_force holds (e.g. the k-space force of rbe_forces)
+ *   d_ws        caller-owned device scratch of rbe_short_range_bytes(ctx, rs) bytes (~44 B per atom
+ *               + 12 B per cell), 256-byte aligned; its contents are rebuilt by every call
+ * rbe_short_range_bytes returns 0 for an invalid rs.  Enqueues five kernels on `stream`.
+ * Errors: RBE_ERR_INVALID_ARG, RBE_ERR_WORKSPACE, RBE_ERR_NO_DEVICE, RBE_ERR_CUDA. */
+size_t     rbe_short_range_bytes(const rbe_ctx* ctx, double rs);
+rbe_status rbe_short_range(rbe_ctx* ctx, const void* d_xyzq, double rs, void* d_force, int32_t accumulate,
+                           int32_t with_energy, void* d_ws, size_t ws_bytes, void* stream);
+
 /* U = (2 pi / V) sum_l w_l |rho(k_l)|^2 / k_l^2 for the current k-set and structure factors,
  * summed in fp64 in a fixed order; written to *h_U (host).  Synchronises `stream`.
  * Errors: RBE_ERR_NOT_READY, RBE_ERR_INVALID_ARG, RBE_ERR_CUDA. */

@@ -10,6 +10,7 @@
 #include <vector>
 
 #include "rbe_kernels.cuh"
+#include "sr_kernels.cuh"
 
 #ifdef RBE_SF_PROFILE
 static long long* g_rbe_prof = nullptr;
@@ -618,6 +619,81 @@ rbe_status rbe_exchange_check(rbe_ctx* c, void* stream) {
     RBE_CUDA(c, cudaMemcpyAsync(&e, c->ws + c->off_xch_err, sizeof(e), cudaMemcpyDeviceToHost, st));
     RBE_CUDA(c, cudaStreamSynchronize(st));
     if (e) return fail(c, RBE_ERR_CUDA, "fused exchange: a peer's structure factors did not arrive within 10 s");
+    return RBE_OK;
+}
+
+// ---- real-space partner (Eq. 2.10 truncated at r_s): workspace layout and launches
+namespace {
+struct SrLayout {
+    int nc = 0;
+    int64_t ncell = 0;
+    size_t off_turns = 0, off_sorted = 0, off_cell = 0, off_order = 0, off_sidx = 0, off_count = 0, off_cursor = 0, off_start = 0;
+    size_t bytes = 0;
+};
+bool sr_layout(const rbe_ctx* c, double rs, SrLayout& l) {
+    if (!c || !(rs > 0.0) || !std::isfinite(rs) || c->N >= ((int64_t)1 << 32)) return false;
+    const double ncd = std::floor(c->L / rs);
+    if (ncd < 3.0) return false;                       // the 27-cell stencil needs 3 distinct cells per dimension
+    l.nc = ncd > 512.0 ? 512 : (int)ncd;               // larger cells are still correct (side >= r_s)
+    l.ncell = (int64_t)l.nc * l.nc * l.nc;
+    const size_t N = (size_t)c->N, nce = (size_t)l.ncell;
+    size_t off = 0;
+    l.off_turns = off;  off = align_up(off + N * sizeof(uint4), 256);
+    l.off_sorted = off; off = align_up(off + N * sizeof(uint4), 256);
+    l.off_cell = off;   off = align_up(off + N * sizeof(int32_t), 256);
+    l.off_order = off;  off = align_up(off + N * sizeof(uint32_t), 256);
+    l.off_sidx = off;   off = align_up(off + N * sizeof(uint32_t), 256);
+    l.off_count = off;  off = align_up(off + nce * sizeof(uint32_t), 256);
+    l.off_cursor = off; off = align_up(off + nce * sizeof(uint32_t), 256);
+    l.off_start = off;  off = align_up(off + (nce + 1) * sizeof(uint32_t), 256);
+    l.bytes = off;
+    return true;
+}
+}  // namespace
+
+size_t rbe_short_range_bytes(const rbe_ctx* c, double rs) {
+    SrLayout l;
+    return sr_layout(c, rs, l) ? l.bytes : 0;
+}
+
+rbe_status rbe_short_range(rbe_ctx* c, const void* d_xyzq, double rs, void* d_force, int32_t accumulate,
+                           int32_t with_energy, void* d_ws, size_t ws_bytes, void* stream) {
+    if (!c) return RBE_ERR_INVALID_ARG;
+    SrLayout l;
+    if (!sr_layout(c, rs, l)) return fail(c, RBE_ERR_INVALID_ARG, "rbe_short_range: need 0 < r_s <= L/3 (three cells of side >= r_s per dimension) and N < 2^32");
+    rbe_status s0 = init_device(c);
+    if (s0 != RBE_OK) return s0;
+    if (c->N == 0) return RBE_OK;
+    if (!d_xyzq || !d_force || (reinterpret_cast<uintptr_t>(d_xyzq) & 15u) || (reinterpret_cast<uintptr_t>(d_force) & 15u))
+        return fail(c, RBE_ERR_INVALID_ARG, "rbe_short_range: null or misaligned pointer");
+    if (!d_ws || ws_bytes < l.bytes || (reinterpret_cast<uintptr_t>(d_ws) & 255u))
+        return fail(c, RBE_ERR_WORKSPACE, "rbe_short_range: d_ws must hold rbe_short_range_bytes bytes, 256-byte aligned");
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    unsigned char* w = static_cast<unsigned char*>(d_ws);
+    uint4* turns = reinterpret_cast<uint4*>(w + l.off_turns);
+    uint4* sorted = reinterpret_cast<uint4*>(w + l.off_sorted);
+    int32_t* cell_of = reinterpret_cast<int32_t*>(w + l.off_cell);
+    uint32_t* order = reinterpret_cast<uint32_t*>(w + l.off_order);
+    uint32_t* sidx = reinterpret_cast<uint32_t*>(w + l.off_sidx);
+    uint32_t* count = reinterpret_cast<uint32_t*>(w + l.off_count);
+    uint32_t* cursor = reinterpret_cast<uint32_t*>(w + l.off_cursor);
+    uint32_t* start = reinterpret_cast<uint32_t*>(w + l.off_start);
+    const unsigned nb = (unsigned)((c->N + 255) / 256);
+    RBE_CUDA(c, cudaMemsetAsync(count, 0, (size_t)l.ncell * sizeof(uint32_t), st));
+    rbe::sr_bin_kernel<<<nb, 256, 0, st>>>(static_cast<const float4*>(d_xyzq), c->N, rbe::TWO32 / c->L, l.nc, turns, cell_of, count);
+    rbe::sr_scan_kernel<<<1, 1024, 0, st>>>(count, (int)l.ncell, start, cursor);
+    rbe::sr_scatter_kernel<<<nb, 256, 0, st>>>(cell_of, c->N, start, cursor, order);
+    rbe::sr_sort_kernel<<<(unsigned)((l.ncell * 32 + 255) / 256), 256, 0, st>>>(order, start, (int)l.ncell, turns, sorted, sidx);
+    rbe::SrParams sp;
+    sp.sorted = sorted; sp.sidx = sidx; sp.start = start;
+    sp.force = static_cast<float4*>(d_force);
+    sp.nc = l.nc; sp.accumulate = accumulate; sp.with_energy = with_energy;
+    sp.len_unit = (float)(c->L / rbe::TWO32);
+    const double rsu = rs * rbe::TWO32 / c->L;
+    sp.rs2_units = (float)(rsu * rsu);
+    sp.sqrt_alpha = (float)std::sqrt(c->alpha);
+    rbe::sr_force_kernel<<<(unsigned)l.ncell, rbe::SR_THREADS, 0, st>>>(sp);
+    RBE_CUDA(c, cudaGetLastError());
     return RBE_OK;
 }
 

@@ -1,0 +1,192 @@
+// sr_kernels.cuh -- sm_100a kernels of the real-space partner of the RBE force: the short-range part
+// of the Ewald-split Coulomb force, Eq. (2.10), truncated at the cutoff radius r_s
+// (P:127), and the matching first term of Eq. (2.8) P:112.  SURVEY.md s8(f) row 2, first stage: the
+// deterministic truncated sum over a linked-cell list (cubic cells of side >= r_s, as Algorithm 2's
+// cell list); the random-batch core/shell estimator of Eqs. (2.13)-(2.16) is the stage
+// after this one.  Device code only; the C ABI is in rbe_api.cu.
+//
+// Positions are the same 32-bit fixed-point turns as in the k-space kernels (to_turns): the cell of
+// an atom is floor(S * nc / 2^32) = umulhi(S, nc) per dimension (exact, consistent, periodic wrap for
+// free), and the wrapped integer difference S_j - S_i IS the nearest-image separation (in units of
+// L / 2^32, i.e. 1e-7 A at L = 464 A): no fp32 cancellation at large L, no image search.
+//
+// Pipeline per call (all on the caller's stream, no host synchronisation):
+//   sr_bin      cell index per atom, per-cell counts (integer atomics: the counts are deterministic)
+//   sr_scan     exclusive prefix sum of the counts (one CTA)
+//   sr_scatter  atom indices into their cell's segment (slot by integer atomic: arbitrary order)
+//   sr_sort     one warp per cell: rank-sort the segment by atom index, gather {S, q} in that order
+//               -> the layout and therefore every sum below is bitwise reproducible
+//   sr_force    one CTA per cell: neighbour cells staged in shared memory, a thread owns an atom
+#pragma once
+#include <cstdint>
+#include <cuda_runtime.h>
+
+#include "rbe_kernels.cuh"
+
+namespace rbe {
+
+constexpr int SR_THREADS = 128;   // force kernel: threads per CTA = atoms of the cell handled per pass
+constexpr int SR_TILE = 256;      // neighbour atoms staged in shared memory at a time
+
+__device__ __forceinline__ int sr_cell_of(uint32_t Sx, uint32_t Sy, uint32_t Sz, int nc) {
+    return ((int)__umulhi(Sz, (uint32_t)nc) * nc + (int)__umulhi(Sy, (uint32_t)nc)) * nc + (int)__umulhi(Sx, (uint32_t)nc);
+}
+
+__global__ void __launch_bounds__(256) sr_bin_kernel(const float4* __restrict__ xyzq, int64_t N, double two32_over_L, int nc,
+                                                      uint4* __restrict__ turns, int32_t* __restrict__ cell_of,
+                                                      uint32_t* __restrict__ count) {
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= N) return;
+    const float4 a = __ldg(&xyzq[i]);
+    const uint32_t Sx = to_turns(a.x, two32_over_L), Sy = to_turns(a.y, two32_over_L), Sz = to_turns(a.z, two32_over_L);
+    const int c = sr_cell_of(Sx, Sy, Sz, nc);
+    turns[i] = make_uint4(Sx, Sy, Sz, __float_as_uint(a.w));
+    cell_of[i] = c;
+    atomicAdd(&count[c], 1u);
+}
+
+// start[c] = sum_{c' < c} count[c'], start[ncell] = N; cursor[c] = 0.  One CTA of 1024 threads.
+__global__ void __launch_bounds__(1024) sr_scan_kernel(const uint32_t* __restrict__ count, int ncell, uint32_t* __restrict__ start,
+                                                        uint32_t* __restrict__ cursor) {
+    __shared__ uint32_t wsum[32];
+    __shared__ uint32_t carry;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    if (tid == 0) carry = 0;
+    __syncthreads();
+    for (int base = 0; base < ncell; base += 1024) {
+        const int c = base + tid;
+        const uint32_t v = c < ncell ? count[c] : 0u;
+        uint32_t incl = v;
+#pragma unroll
+        for (int d = 1; d < 32; d <<= 1) {
+            const uint32_t n = __shfl_up_sync(FULL_MASK, incl, d);
+            if (lane >= d) incl += n;
+        }
+        if (lane == 31) wsum[warp] = incl;
+        __syncthreads();
+        uint32_t before = 0, total = 0;
+#pragma unroll
+        for (int w = 0; w < 32; ++w) {
+            const uint32_t s = wsum[w];
+            before += w < warp ? s : 0u;
+            total += s;
+        }
+        const uint32_t c0 = carry;
+        if (c < ncell) { start[c] = c0 + before + incl - v; cursor[c] = 0u; }
+        __syncthreads();
+        if (tid == 0) carry = c0 + total;
+        __syncthreads();
+    }
+    if (tid == 0) start[ncell] = carry;
+}
+
+__global__ void __launch_bounds__(256) sr_scatter_kernel(const int32_t* __restrict__ cell_of, int64_t N,
+                                                          const uint32_t* __restrict__ start, uint32_t* __restrict__ cursor,
+                                                          uint32_t* __restrict__ order) {
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= N) return;
+    const int c = cell_of[i];
+    order[start[c] + atomicAdd(&cursor[c], 1u)] = (uint32_t)i;
+}
+
+// One warp per cell: the segment arrives in arbitrary order (atomic slots); rank-sort it by atom
+// index (O(n^2 / 32) per lane, n ~ 100) and gather the atom records in that order.
+__global__ void __launch_bounds__(256) sr_sort_kernel(const uint32_t* __restrict__ order, const uint32_t* __restrict__ start,
+                                                       int ncell, const uint4* __restrict__ turns, uint4* __restrict__ sorted,
+                                                       uint32_t* __restrict__ sidx) {
+    const int c = (int)(((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5), lane = threadIdx.x & 31;
+    if (c >= ncell) return;
+    const uint32_t s0 = start[c], n = start[c + 1] - s0;
+    for (uint32_t e = lane; e < n; e += 32) {
+        const uint32_t me = order[s0 + e];
+        uint32_t rank = 0;
+        for (uint32_t j = 0; j < n; ++j) rank += order[s0 + j] < me ? 1u : 0u;
+        sorted[s0 + rank] = turns[me];
+        sidx[s0 + rank] = me;
+    }
+}
+
+struct SrParams {
+    const uint4* sorted;      // [N] {Sx, Sy, Sz, q} in cell order
+    const uint32_t* sidx;     // [N] original atom index
+    const uint32_t* start;    // [ncell + 1]
+    float4* force;            // [N] {F, e_i}, original atom order
+    int32_t nc;               // cells per dimension (>= 3)
+    int32_t accumulate;       // add to what `force` holds (e.g. the k-space force)
+    int32_t with_energy;
+    float len_unit;           // L / 2^32: length of one fixed-point unit [A]
+    float rs2_units;          // (r_s / len_unit)^2: the cutoff in fixed-point units squared
+    float sqrt_alpha;         // sqrt(alpha) [1/A]
+};
+
+// erfc(x) = t (a1 + t (a2 + t (a3 + t (a4 + t a5)))) exp(-x^2), t = 1 / (1 + p x): Abramowitz & Stegun
+// 7.1.26, |error| <= 1.5e-7 for x >= 0.  E = exp(-x^2) is shared with the Gaussian term of Eq. (2.10).
+__device__ __forceinline__ float sr_erfc_from_exp(float x, float E) {
+    const float t = __frcp_rn(fmaf(0.3275911f, x, 1.0f));
+    float p = fmaf(t, 1.061405429f, -1.453152027f);
+    p = fmaf(t, p, 1.421413741f);
+    p = fmaf(t, p, -0.284496736f);
+    p = fmaf(t, p, 0.254829592f);
+    return t * p * E;
+}
+
+__global__ void __launch_bounds__(SR_THREADS) sr_force_kernel(const SrParams p) {
+    __shared__ uint4 tile[SR_TILE];
+    const int nc = p.nc, c = blockIdx.x, tid = threadIdx.x;
+    const int cx = c % nc, cy = (c / nc) % nc, cz = c / (nc * nc);
+    const uint32_t s0 = p.start[c], n_own = p.start[c + 1] - s0;
+    const float two_sa_over_sqrtpi = 1.1283791670955126f * p.sqrt_alpha;
+
+    for (uint32_t pass = 0; pass < n_own; pass += SR_THREADS) {     // (uniform: every thread runs every pass)
+        const bool have = pass + tid < n_own;
+        const uint4 me = have ? p.sorted[s0 + pass + tid] : make_uint4(0u, 0u, 0u, 0u);
+        float fx = 0.f, fy = 0.f, fz = 0.f, en = 0.f;
+        for (int nb = 0; nb < 27; ++nb) {
+            const int ox = nb % 3 - 1, oy = (nb / 3) % 3 - 1, oz = nb / 9 - 1;
+            const int ncx = (cx + ox + nc) % nc, ncy = (cy + oy + nc) % nc, ncz = (cz + oz + nc) % nc;
+            const int cn = (ncz * nc + ncy) * nc + ncx;
+            const uint32_t n0 = p.start[cn], n1 = p.start[cn + 1];
+            for (uint32_t t0 = n0; t0 < n1; t0 += SR_TILE) {
+                const int cnt = (int)min((uint32_t)SR_TILE, n1 - t0);
+                __syncthreads();
+                for (int k = tid; k < cnt; k += SR_THREADS) tile[k] = p.sorted[t0 + k];
+                __syncthreads();
+                if (!have) continue;
+#pragma unroll 4
+                for (int k = 0; k < cnt; ++k) {
+                    const uint4 o = tile[k];
+                    const float dx = (float)(int32_t)(o.x - me.x), dy = (float)(int32_t)(o.y - me.y), dz = (float)(int32_t)(o.z - me.z);
+                    const float r2u = fmaf(dx, dx, fmaf(dy, dy, dz * dz));
+                    if (r2u < p.rs2_units && r2u > 0.f) {
+                        const float inv_ru = rsqrtf(r2u);                    // 1 / r in fixed-point units
+                        const float inv_r = inv_ru * (1.0f / p.len_unit);    // 1 / r  [1/A]
+                        const float r = r2u * inv_ru * p.len_unit;           // r      [A]
+                        const float x = p.sqrt_alpha * r;
+                        const float E = __expf(-x * x);
+                        const float ec = sr_erfc_from_exp(x, E);
+                        const float qj = __uint_as_float(o.w);
+                        // g / r, then the direction d / r in units: (erfc / r^2 + c E / r) / r * d_units / r_units ...
+                        const float g = fmaf(ec, inv_r, two_sa_over_sqrtpi * E) * inv_r;   // erfc/r^2 + 2 sqrt(alpha/pi) E / r
+                        const float s = qj * g * inv_ru;                                    // q_j g / r_units
+                        fx = fmaf(s, dx, fx);
+                        fy = fmaf(s, dy, fy);
+                        fz = fmaf(s, dz, fz);
+                        en = fmaf(qj * ec, inv_r, en);
+                    }
+                }
+            }
+        }
+        if (have) {
+            const float qi = __uint_as_float(me.w);
+            const uint32_t i = p.sidx[s0 + pass + tid];
+            float4 o = make_float4(-qi * fx, -qi * fy, -qi * fz, p.with_energy ? 0.5f * qi * en : 0.f);
+            if (p.accumulate) {
+                const float4 prev = p.force[i];
+                o.x += prev.x; o.y += prev.y; o.z += prev.z; o.w += prev.w;
+            }
+            p.force[i] = o;
+        }
+    }
+}
+
+}  // namespace rbe

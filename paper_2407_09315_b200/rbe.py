@@ -79,6 +79,10 @@ def lib():
         L.rbe_set_exchange.argtypes = [vp, i32, i32, ctypes.POINTER(vp), sz]
         L.rbe_exchange_check.restype = ctypes.c_int
         L.rbe_exchange_check.argtypes = [vp, vp]
+        L.rbe_short_range_bytes.restype = sz
+        L.rbe_short_range_bytes.argtypes = [vp, dbl]
+        L.rbe_short_range.restype = ctypes.c_int
+        L.rbe_short_range.argtypes = [vp, vp, dbl, vp, i32, i32, vp, sz, vp]
         L.rbe_structure_factor.restype = ctypes.c_int
         L.rbe_structure_factor.argtypes = [vp, vp, vp, vp]
         L.rbe_set_rho.restype = ctypes.c_int
@@ -259,6 +263,23 @@ class Rbe:
         self._check(lib().rbe_forces(self._h, ctypes.c_void_p(xyzq.data_ptr()),
                                      ctypes.c_void_p(force.data_ptr()), int(bool(with_energy)),
                                      _stream_ptr(stream)))
+
+    def rbe_short_range_bytes(self, rs: float) -> int:
+        return int(lib().rbe_short_range_bytes(self._h, float(rs)))
+
+    def rbe_short_range(self, xyzq, rs: float, force, accumulate: bool = False, with_energy: bool = False, stream=None):
+        """Real-space partner (Eq. 2.10 truncated at rs).  xyzq, force: cuda float32 [N,4]."""
+        import torch
+        _check_tensor(xyzq, (self.N, 4), "float32")
+        _check_tensor(force, (self.N, 4), "float32")
+        n = self.rbe_short_range_bytes(rs)
+        if n == 0:
+            raise RbeError(1, "rbe_short_range: need 0 < r_s <= L/3")
+        if getattr(self, "_sr_ws", None) is None or self._sr_ws.numel() < n:
+            self._sr_ws = torch.empty(n, dtype=torch.uint8, device="cuda")
+        self._check(lib().rbe_short_range(self._h, ctypes.c_void_p(xyzq.data_ptr()), float(rs),
+                                          ctypes.c_void_p(force.data_ptr()), int(bool(accumulate)), int(bool(with_energy)),
+                                          ctypes.c_void_p(self._sr_ws.data_ptr()), self._sr_ws.numel(), _stream_ptr(stream)))
 
     def rbe_kspace_energy(self, stream=None) -> float:
         u = ctypes.c_double(0.0)

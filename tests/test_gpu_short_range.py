@@ -1,0 +1,115 @@
+"""Parity of the real-space partner (rbe_short_range: Eq. 2.10 truncated at r_s over a cell list)
+against oracle/short_range.c on the same fp32 inputs.  Tolerances: forces
+2e-5 relative L2 (the bar north_star sets for the k-space force), per-atom energies 2e-5 relative L2."""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+from paper_2407_09315_b200 import inputs, rbe
+
+pytestmark = pytest.mark.gpu
+F_TOL = 2e-5
+
+
+def run(atoms, L, alpha, rs, accumulate=None, with_energy=True):
+    N = atoms.shape[0]
+    ctx = rbe.Rbe(N, L, alpha, 4, allocate=False)
+    x = torch.from_numpy(atoms).cuda()
+    F = torch.full((N, 4), float("nan"), dtype=torch.float32, device="cuda") if accumulate is None else accumulate.clone()
+    ctx.rbe_short_range(x, rs, F, accumulate=accumulate is not None, with_energy=with_energy)
+    torch.cuda.synchronize()
+    return ctx, x, F
+
+
+def check(atoms, L, alpha, rs, sel=None):
+    ctx, x, F = run(atoms, L, alpha, rs)
+    Fg = F.cpu().numpy().astype(np.float64)
+    assert np.isfinite(Fg).all()
+    F_o, e_o = oracle.short_range(atoms, L, alpha, rs, sel=sel)
+    if sel is not None:
+        Fg = Fg[sel]
+    errF = np.linalg.norm(Fg[:, :3] - F_o) / np.linalg.norm(F_o)
+    erre = np.linalg.norm(Fg[:, 3] - e_o) / np.linalg.norm(e_o)
+    assert errF <= F_TOL and erre <= F_TOL, (errF, erre)
+    return F, errF
+
+
+@pytest.mark.parametrize("name,rs", [("water_3k", 10.0), ("water_3k", 6.0), ("ions_20000", 10.0), ("ions_20000", 12.5)])
+def test_small_configs_full_oracle(name, rs):
+    cfg = inputs.CONFIGS[name] if name in inputs.CONFIGS else inputs.ions_config(20_000)
+    atoms = inputs.make_atoms(cfg)
+    F, _ = check(atoms, cfg.L, cfg.alpha, rs)
+    Fd = F[:, :3].double()
+    assert Fd.sum(0).abs().max().item() <= 1e-5 * Fd.abs().sum().item()      # Newton's third law, fp32 sums
+
+
+def test_config_96k_and_1m_sampled():
+    for name, nsel in (("water_96k", 3000), ("water_nacl_1m", 400)):
+        cfg = inputs.CONFIGS[name]
+        atoms = inputs.make_atoms(cfg)
+        sel = np.sort(np.random.default_rng(4).choice(cfg.N, nsel, replace=False)).astype(np.int64)
+        sel[-2:] = [cfg.N - 2, cfg.N - 1]
+        check(atoms, cfg.L, cfg.alpha, 10.0, sel=sel)
+
+
+@pytest.mark.parametrize("N", [1, 2, 33, 129, 1000])
+def test_ragged_sizes_sparse_cells(N):
+    cfg = inputs.ions_config(20_000)
+    atoms = inputs.make_atoms(cfg)[:N].copy()            # mostly empty cells
+    if N == 1:
+        ctx, x, F = run(atoms, cfg.L, cfg.alpha, 10.0)
+        assert torch.all(F == 0)
+        return
+    atoms[1, :3] = atoms[0, :3] + np.float32(1.5)         # at least one interacting pair
+    check(atoms, cfg.L, cfg.alpha, 10.0)
+
+
+def test_crowded_cell_more_atoms_than_threads_and_far_outside_box():
+    """One cell holds 400 atoms (> 128 threads, > one 256-atom tile); positions up to 5 boxes away."""
+    L, alpha, rs = 36.0, 0.09, 12.0
+    rng = np.random.default_rng(6)
+    n = 1200
+    atoms = np.empty((n, 4), dtype=np.float32)
+    atoms[:, :3] = rng.random((n, 3)) * L
+    atoms[:400, :3] = 1.0 + rng.random((400, 3)) * 10.0                   # all in cell (0,0,0)
+    atoms[:, :3] += (rng.integers(-5, 6, size=(n, 3)) * L).astype(np.float32)
+    atoms[:, 3] = np.where(np.arange(n) % 2 == 0, 1.0, -1.0)
+    check(atoms, L, alpha, rs)
+
+
+def test_accumulate_bitwise_reproducible_and_argument_checks():
+    cfg = inputs.CONFIGS["water_3k"]
+    atoms = inputs.make_atoms(cfg)
+    ctx, x, F1 = run(atoms, cfg.L, cfg.alpha, 9.0)
+    _, _, F2 = run(atoms, cfg.L, cfg.alpha, 9.0)
+    assert torch.equal(F1, F2)                                            # atomics only assign slots; sums are ordered
+    base = torch.ones((cfg.N, 4), dtype=torch.float32, device="cuda")
+    _, _, F3 = run(atoms, cfg.L, cfg.alpha, 9.0, accumulate=base)
+    assert torch.allclose(F3, F1 + 1.0, rtol=0, atol=1e-6)
+    _, _, F4 = run(atoms, cfg.L, cfg.alpha, 9.0, with_energy=False)
+    assert torch.equal(F4[:, :3], F1[:, :3]) and torch.all(F4[:, 3] == 0)
+    assert ctx.rbe_short_range_bytes(cfg.L / 2.9) == 0 and ctx.rbe_short_range_bytes(-1.0) == 0
+    with pytest.raises(rbe.RbeError):
+        ctx.rbe_short_range(x, cfg.L / 2.9, F1)                           # fewer than 3 cells per dimension
+
+
+def test_total_coulomb_force_is_kspace_plus_real_space():
+    """Deterministic Ewald through the same kernels: weighted full k-grid (Eq. 2.11) + short range
+    (Eq. 2.10) against oracle.ewald_full's total force on a small cell."""
+    L, alpha, mmax, rs = 30.0, 0.16, 12, 10.0             # erfc(sqrt(alpha) rs) = 1.5e-8
+    cfg = inputs.ions_config(600)
+    atoms = inputs.make_atoms(cfg)
+    atoms[:, :3] *= np.float32(L / cfg.L)
+    m = inputs.full_kgrid(mmax)
+    w = np.exp(-(2 * np.pi / L) ** 2 * (m.astype(np.float64) ** 2).sum(1) / (4 * alpha))
+    ctx = rbe.Rbe(atoms.shape[0], L, alpha, m.shape[0])
+    x = torch.from_numpy(atoms).cuda()
+    F = torch.empty((atoms.shape[0], 4), dtype=torch.float32, device="cuda")
+    ctx.rbe_set_kvectors(m, w)
+    ctx.rbe_structure_factor(x)
+    ctx.rbe_forces(x, F)
+    ctx.rbe_short_range(x, rs, F, accumulate=True)
+    _, Fs, Fl = oracle.ewald_full(atoms[:, :3].astype(np.float64), atoms[:, 3].astype(np.float64), L, alpha, nreal=1, mmax=mmax)
+    tot = Fs + Fl
+    assert np.linalg.norm(F.cpu().numpy()[:, :3] - tot) / np.linalg.norm(tot) <= 5e-5
