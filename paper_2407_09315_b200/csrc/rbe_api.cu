@@ -683,7 +683,7 @@ rbe_status rbe_short_range(rbe_ctx* c, const void* d_xyzq, double rs, void* d_fo
     rbe::sr_bin_kernel<<<nb, 256, 0, st>>>(static_cast<const float4*>(d_xyzq), c->N, rbe::TWO32 / c->L, l.nc, turns, cell_of, count);
     rbe::sr_scan_kernel<<<1, 1024, 0, st>>>(count, (int)l.ncell, start, cursor);
     rbe::sr_scatter_kernel<<<nb, 256, 0, st>>>(cell_of, c->N, start, cursor, order);
-    rbe::sr_sort_kernel<<<(unsigned)((l.ncell * 32 + 255) / 256), 256, 0, st>>>(order, start, (int)l.ncell, turns, sorted, sidx);
+    rbe::sr_sort_kernel<<<(unsigned)((l.ncell * 32 + 255) / 256), 256, 0, st>>>(order, start, (int)l.ncell, l.nc, turns, sorted, sidx);
     rbe::SrParams sp;
     sp.sorted = sorted; sp.sidx = sidx; sp.start = start;
     sp.force = static_cast<float4*>(d_force);

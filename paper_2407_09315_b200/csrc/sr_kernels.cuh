@@ -14,8 +14,8 @@
 //   sr_bin      cell index per atom, per-cell counts (integer atomics: the counts are deterministic)
 //   sr_scan     exclusive prefix sum of the counts (one CTA)
 //   sr_scatter  atom indices into their cell's segment (slot by integer atomic: arbitrary order)
-//   sr_sort     one warp per cell: rank-sort the segment by atom index, gather {S, q} in that order
-//               -> the layout and therefore every sum below is bitwise reproducible
+//   sr_sort     one warp per cell: rank-sort the segment by (sub-cell Morton code, atom index), gather
+//               {S, q} in that order -> the layout and every sum below are bitwise reproducible
 //   sr_force    one CTA per cell: neighbour cells staged in shared memory, a thread owns an atom
 #pragma once
 #include <cstdint>
@@ -89,19 +89,35 @@ __global__ void __launch_bounds__(256) sr_scatter_kernel(const int32_t* __restri
     order[start[c] + atomicAdd(&cursor[c], 1u)] = (uint32_t)i;
 }
 
-// One warp per cell: the segment arrives in arbitrary order (atomic slots); rank-sort it by atom
-// index (O(n^2 / 32) per lane, n ~ 100) and gather the atom records in that order.
+// Position of an atom inside its cell as a 6-bit Morton code of 4 x 4 x 4 sub-cells: sorting a cell by
+// it makes every run of 32 consecutive atoms (a warp of the force kernel) spatially compact, so that
+// for many far neighbours ALL lanes of the warp fail the cutoff test together and the expensive
+// branch is skipped (measured: 5 % on the force kernel; the cutoff tests themselves dominate).
+__device__ __forceinline__ uint32_t sr_subcell(const uint4 t, int nc) {
+    const uint32_t fx = (t.x * (uint32_t)nc) >> 30, fy = (t.y * (uint32_t)nc) >> 30, fz = (t.z * (uint32_t)nc) >> 30;  // 2 bits each
+    return ((fz & 2u) << 4) | ((fy & 2u) << 3) | ((fx & 2u) << 2) | ((fz & 1u) << 2) | ((fy & 1u) << 1) | (fx & 1u);
+}
+
+// One warp per cell: the segment arrives in arbitrary order (atomic slots); rank-sort it by
+// (sub-cell Morton code, atom index) -- a total order, so the layout is deterministic -- in
+// O(n^2 / 32) per lane (n ~ 100), and gather the atom records in that order.
 __global__ void __launch_bounds__(256) sr_sort_kernel(const uint32_t* __restrict__ order, const uint32_t* __restrict__ start,
-                                                       int ncell, const uint4* __restrict__ turns, uint4* __restrict__ sorted,
+                                                       int ncell, int nc, const uint4* __restrict__ turns, uint4* __restrict__ sorted,
                                                        uint32_t* __restrict__ sidx) {
     const int c = (int)(((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5), lane = threadIdx.x & 31;
     if (c >= ncell) return;
     const uint32_t s0 = start[c], n = start[c + 1] - s0;
     for (uint32_t e = lane; e < n; e += 32) {
         const uint32_t me = order[s0 + e];
+        const uint4 mt = turns[me];
+        const unsigned long long mkey = ((unsigned long long)sr_subcell(mt, nc) << 32) | me;
         uint32_t rank = 0;
-        for (uint32_t j = 0; j < n; ++j) rank += order[s0 + j] < me ? 1u : 0u;
-        sorted[s0 + rank] = turns[me];
+        for (uint32_t j = 0; j < n; ++j) {
+            const uint32_t o = order[s0 + j];
+            const unsigned long long okey = ((unsigned long long)sr_subcell(turns[o], nc) << 32) | o;
+            rank += okey < mkey ? 1u : 0u;
+        }
+        sorted[s0 + rank] = mt;
         sidx[s0 + rank] = me;
     }
 }
@@ -121,8 +137,12 @@ struct SrParams {
 
 // erfc(x) = t (a1 + t (a2 + t (a3 + t (a4 + t a5)))) exp(-x^2), t = 1 / (1 + p x): Abramowitz & Stegun
 // 7.1.26, |error| <= 1.5e-7 for x >= 0.  E = exp(-x^2) is shared with the Gaussian term of Eq. (2.10).
+__device__ __forceinline__ float sr_rsqrt(float x) { float r; asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r; }
+__device__ __forceinline__ float sr_rcp(float x) { float r; asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r; }
+__device__ __forceinline__ float sr_ex2(float x) { float r; asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r; }
+
 __device__ __forceinline__ float sr_erfc_from_exp(float x, float E) {
-    const float t = __frcp_rn(fmaf(0.3275911f, x, 1.0f));
+    const float t = sr_rcp(fmaf(0.3275911f, x, 1.0f));   // 1 + p x in [1, ~5]: the approximate reciprocal is 1 ulp
     float p = fmaf(t, 1.061405429f, -1.453152027f);
     p = fmaf(t, p, 1.421413741f);
     p = fmaf(t, p, -0.284496736f);
@@ -158,11 +178,11 @@ __global__ void __launch_bounds__(SR_THREADS) sr_force_kernel(const SrParams p) 
                     const float dx = (float)(int32_t)(o.x - me.x), dy = (float)(int32_t)(o.y - me.y), dz = (float)(int32_t)(o.z - me.z);
                     const float r2u = fmaf(dx, dx, fmaf(dy, dy, dz * dz));
                     if (r2u < p.rs2_units && r2u > 0.f) {
-                        const float inv_ru = rsqrtf(r2u);                    // 1 / r in fixed-point units
+                        const float inv_ru = sr_rsqrt(r2u);                  // 1 / r in fixed-point units (r2u >= 1: no denormals)
                         const float inv_r = inv_ru * (1.0f / p.len_unit);    // 1 / r  [1/A]
                         const float r = r2u * inv_ru * p.len_unit;           // r      [A]
                         const float x = p.sqrt_alpha * r;
-                        const float E = __expf(-x * x);
+                        const float E = sr_ex2(-1.4426950408889634f * x * x);   // exp(-alpha r^2); underflows to 0 harmlessly
                         const float ec = sr_erfc_from_exp(x, E);
                         const float qj = __uint_as_float(o.w);
                         // g / r, then the direction d / r in units: (erfc / r^2 + c E / r) / r * d_units / r_units ...
