@@ -172,6 +172,8 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-graph", action="store_true")
+    ap.add_argument("--no-short-range", action="store_true")
+    ap.add_argument("--rs", type=float, default=10.0, help="cutoff radius of the real-space partner leg [A]")
     ap.add_argument("--exchange", default="fused", choices=["fused", "nccl"],
                     help="N > 1: how the structure factors are summed across ranks")
     ap.add_argument("--with-energy", action="store_true")
@@ -301,6 +303,26 @@ def main():
         ms_graph = e0.elapsed_time(e1) / args.steps
         del gctx
 
+    # ---- real-space partner: Eq. 2.10 truncated at r_s = 10 A on the same atoms
+    sr = None
+    if world == 1 and not args.no_short_range and L >= 3 * args.rs:
+        k_sr = max(3, min(args.steps, 20))
+        for i in range(3):
+            ctx.rbe_short_range(xs[i % n_rot], args.rs, fs[i % n_rot])
+        sync()
+        e0.record()
+        for i in range(k_sr):
+            ctx.rbe_short_range(xs[i % n_rot], args.rs, fs[i % n_rot])
+        e1.record()
+        sync()
+        ms_sr = e0.elapsed_time(e1) / k_sr
+        nbr = 4.0 / 3.0 * np.pi * args.rs ** 3 * n_local / L ** 3          # expected atoms inside the cutoff sphere
+        sr = {"ms_per_call": ms_sr, "value": ms_sr * 1e6 / n_local, "unit": UNIT.replace("/step", "/call"),
+              "r_s": args.rs, "neighbours_per_atom_expected": nbr, "calls": k_sr, "gpu_launches_per_call": 5,
+              "pair_rate_G_per_s": nbr * n_local / (ms_sr * 1e-3) / 1e9,
+              "note": "rbe_short_range: bin + scan + scatter + sort + cell-pair force kernel; every ordered pair "
+                      "inside the cutoff is evaluated once per atom (no Newton-3 sharing); not part of `value`"}
+
     if world > 1:
         t = torch.tensor([ms_total, ms_sf, ms_f], dtype=torch.float64, device="cuda")
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
@@ -403,6 +425,7 @@ def main():
             "ms_per_step": ms_graph, "value": ms_graph * 1e6 / n_total, "unit": UNIT, "gpu_launches_per_step": 1,
             "note": "rbe_graph_launch: device sampler (Philox) + sf_kernel + f_kernel replayed as one CUDA graph, "
                     "no per-step H2D; not the headline (the k-set there comes from the host each step)"},
+        "short_range": sr,
         "clocks": clocks,
         "gpu_launches": 2 * args.steps,
         "paper_context": "8.20 ms/step, 1e6 atoms, A100, RBL+RBE nonbonded total, P=100 (PAPER.md P:284); 2.89 ms k-space at 1e5 atoms, P=200 (P:266)",
