@@ -219,6 +219,14 @@ rbe_status rbe_short_range(rbe_ctx* ctx, const void* d_xyzq, double rs, void* d_
  * Errors: RBE_ERR_NOT_READY, RBE_ERR_INVALID_ARG, RBE_ERR_CUDA. */
 rbe_status rbe_kspace_energy(rbe_ctx* ctx, double* h_U, void* stream);
 
+/* k-space virial of the current k-set and structure factors (for the pressure of the isothermal-
+ * isobaric variant the paper names; the paper gives no estimator): minus the strain derivative
+ * of the second term of Eq. (2.8) P:112 with the weights of Eq. (2.12),
+ *   W_ab = sum_l (2 pi w_l / V) |rho_l|^2 / k_l^2 [ delta_ab - 2 k_la k_lb / k_l^2 (1 + k_l^2 / 4 alpha) ],
+ * h_W double [6] (host) = W_xx, W_yy, W_zz, W_xy, W_xz, W_yz in e^2/A; fp64, fixed order.
+ * Synchronises `stream`.  Errors: RBE_ERR_NOT_READY, RBE_ERR_INVALID_ARG, RBE_ERR_CUDA. */
+rbe_status rbe_kspace_virial(rbe_ctx* ctx, double* h_W, void* stream);
+
 /* One whole step from HOST buffers (the end-to-end path): copies h_xyzq (float [N][4]) to the
  * device, uploads the k-set, runs rbe_structure_factor and rbe_forces, copies the forces back
  * into h_force (float [N][4]) and, if h_U != NULL, the energy into *h_U; synchronises `stream`.

@@ -225,7 +225,7 @@ rbe_status init_device(rbe_ctx* c) {
     c->off_part = off; off = align_up(off + (size_t)gx * P * sizeof(double2), 256);
     c->off_rho = off;  off = align_up(off + P * sizeof(double2), 256);
     c->off_grow = off; off = align_up(off + (size_t)c->sf_ngroups * P * sizeof(double2), 256);
-    c->off_U = off;    off = align_up(off + sizeof(double), 256);
+    c->off_U = off;    off = align_up(off + 8 * sizeof(double), 256);   // U, then the 6 virial components
     c->off_ticket = off; off = align_up(off + (size_t)(c->sf_ngroups + 1) * sizeof(unsigned int), 256);
     c->off_T = off;    off = align_up(off + c->sampler_T.size() * sizeof(uint32_t) + 4, 256);
     c->off_state = off; off = align_up(off + 2 * sizeof(unsigned long long), 256);
@@ -694,6 +694,18 @@ rbe_status rbe_short_range(rbe_ctx* c, const void* d_xyzq, double rs, void* d_fo
     sp.sqrt_alpha = (float)std::sqrt(c->alpha);
     rbe::sr_force_kernel<<<(unsigned)l.ncell, rbe::SR_THREADS, 0, st>>>(sp);
     RBE_CUDA(c, cudaGetLastError());
+    return RBE_OK;
+}
+
+rbe_status rbe_kspace_virial(rbe_ctx* c, double* h_W, void* stream) {
+    if (!c || !h_W) return fail(c, RBE_ERR_INVALID_ARG, "rbe_kspace_virial: null argument");
+    if (!c->ws || !c->have_k || !c->have_rho) return fail(c, RBE_ERR_NOT_READY, "rbe_kspace_virial needs a structure factor");
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    double* d_W = ws_ptr<double>(c, c->off_U) + 1;
+    rbe::virial_kernel<<<1, 256, 0, st>>>(k_table(c), c->P, c->alpha, d_W);
+    RBE_CUDA(c, cudaGetLastError());
+    RBE_CUDA(c, cudaMemcpyAsync(h_W, d_W, 6 * sizeof(double), cudaMemcpyDeviceToHost, st));
+    RBE_CUDA(c, cudaStreamSynchronize(st));
     return RBE_OK;
 }
 

@@ -208,6 +208,36 @@ __global__ void __launch_bounds__(256) energy_kernel(const KTable t, int32_t P, 
     if (threadIdx.x == 0) *U = sh[0];
 }
 
+// k-space virial (reading Q19): W_ab = sum_l e_l |rho_l|^2 [delta_ab - 2 m_a m_b / |m|^2 (1 + pi^2 |m|^2 / (alpha L^2))],
+// the strain derivative of the second term of Eq. (2.8) with the weights of Eq. (2.12); k_a k_b / k^2 =
+// m_a m_b / |m|^2 and k^2 / 4 alpha = pi^2 |m|^2 / (alpha L^2).  W[0..5] = xx, yy, zz, xy, xz, yz.  Fixed order.
+__global__ void __launch_bounds__(256) virial_kernel(const KTable t, int32_t P, double alpha, double* W) {
+    __shared__ double sh[6][256];
+    xch_wait(t.xch);
+    double a[6] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
+    for (int k = threadIdx.x; k < P; k += 256) {
+        const int4 m = t.kvec[k];
+        const double2 r = k_rho(t, k);
+        const double w = t.w ? t.w[k] : t.w_uniform;
+        const double mx = m.x, my = m.y, mz = m.z;
+        const double m2 = mx * mx + my * my + mz * mz;
+        const double u = w / (2.0 * PI_D * t.L * m2) * (r.x * r.x + r.y * r.y);       // e_l |rho_l|^2
+        const double f = 2.0 / m2 * (1.0 + PI_D * PI_D * m2 / (alpha * t.L * t.L));
+        a[0] += u * (1.0 - f * mx * mx); a[1] += u * (1.0 - f * my * my); a[2] += u * (1.0 - f * mz * mz);
+        a[3] += u * (-f * mx * my);      a[4] += u * (-f * mx * mz);      a[5] += u * (-f * my * mz);
+    }
+#pragma unroll
+    for (int c = 0; c < 6; ++c) sh[c][threadIdx.x] = a[c];
+    __syncthreads();
+    for (int s = 128; s > 0; s >>= 1) {
+        if ((int)threadIdx.x < s)
+#pragma unroll
+            for (int c = 0; c < 6; ++c) sh[c][threadIdx.x] += sh[c][threadIdx.x + s];
+        __syncthreads();
+    }
+    if (threadIdx.x < 6) W[threadIdx.x] = sh[threadIdx.x][0];
+}
+
 // ---------------------------------------------------------------------------------------
 // Second pass of the structure-factor reduction, inside the SF kernel (no extra launch).
 //

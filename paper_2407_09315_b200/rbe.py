@@ -91,6 +91,8 @@ def lib():
         L.rbe_forces.argtypes = [vp, vp, vp, i32, vp]
         L.rbe_kspace_energy.restype = ctypes.c_int
         L.rbe_kspace_energy.argtypes = [vp, ctypes.POINTER(dbl), vp]
+        L.rbe_kspace_virial.restype = ctypes.c_int
+        L.rbe_kspace_virial.argtypes = [vp, vp, vp]
         L.rbe_step_host.restype = ctypes.c_int
         L.rbe_step_host.argtypes = [vp, vp, vp, vp, vp, i32, ctypes.POINTER(dbl), vp, sz, vp]
         L.rbe_host_alloc.restype = ctypes.c_int
@@ -285,6 +287,13 @@ class Rbe:
         u = ctypes.c_double(0.0)
         self._check(lib().rbe_kspace_energy(self._h, ctypes.byref(u), _stream_ptr(stream)))
         return float(u.value)
+
+    def rbe_kspace_virial(self, stream=None):
+        """numpy float64 [6] = W_xx, W_yy, W_zz, W_xy, W_xz, W_yz (synchronises)."""
+        import numpy as np
+        W = np.empty(6, dtype=np.float64)
+        self._check(lib().rbe_kspace_virial(self._h, _np_ptr(W), _stream_ptr(stream)))
+        return W
 
     def rbe_step_host(self, h_xyzq, m, h_force, w=None, with_energy=False, want_energy=False, stream=None):
         """End-to-end step from HOST buffers: h_xyzq / h_force are CPU float32 [N,4] torch tensors

@@ -332,3 +332,31 @@ def test_host_buffer_step_chunked_pipeline(N):
     h_f2 = np.full((N, 4), np.nan, dtype=np.float32)
     ctx.rbe_step_host(atoms, m, h_f2, with_energy=True)
     assert np.array_equal(h_f2, F_h)
+
+
+@pytest.mark.parametrize("name,weighted", [("water_3k", False), ("water_96k", False), ("ions_400", True)])
+def test_kspace_virial_matches_oracle(name, weighted):
+    """rbe_kspace_virial against oracle/virial.py (reading Q19): fp64 on both sides from the GPU's rho,
+    so the bar is the energy's (1e-5 relative to the largest component)."""
+    from oracle import virial
+    if weighted:
+        L, alpha, mmax = 12.0, 0.3, 7
+        cfg = inputs.ions_config(400)
+        atoms = inputs.make_atoms(cfg)
+        atoms[:, :3] *= np.float32(L / cfg.L)
+        m = inputs.full_kgrid(mmax)
+        w = np.exp(-(2 * np.pi / L) ** 2 * (m.astype(np.float64) ** 2).sum(1) / (4 * alpha))
+    else:
+        cfg = inputs.CONFIGS[name]
+        atoms, L, alpha, w = inputs.make_atoms(cfg), cfg.L, cfg.alpha, None
+        m = inputs.sample_kset(L, alpha, cfg.P, cfg.seed, 0)
+    ctx = rbe.Rbe(atoms.shape[0], L, alpha, m.shape[0])
+    with pytest.raises(rbe.RbeError):
+        ctx.rbe_kspace_virial()
+    ctx.rbe_set_kvectors(m, w)
+    ctx.rbe_structure_factor(torch.from_numpy(atoms).cuda())
+    W = ctx.rbe_kspace_virial()
+    S = oracle.S(L, alpha)
+    W_o = virial.kspace_virial(L, alpha, m, S, oracle.rho(atoms, L, m), w=w)
+    assert np.abs(W - W_o).max() <= U_TOL * np.abs(W_o).max()
+    assert np.array_equal(W, ctx.rbe_kspace_virial())          # fixed order: bitwise reproducible
