@@ -150,54 +150,65 @@ __device__ __forceinline__ float sr_erfc_from_exp(float x, float E) {
     return t * p * E;
 }
 
+// Coordinates inside the kernel are fp32 Angstrom RELATIVE TO THE CENTRE OF THE CTA's CELL, computed from the
+// wrapped integer difference of the fixed-point turns (so the nearest image is implicit): own atoms lie within
+// half a cell side, the staged neighbours within 1.5 cell sides, and a separation d = t_j - t_i carries an
+// absolute error <= 2^-24 * 1.5 cell sides (1e-6 A at a 10 A cell) -- instead of three integer subtractions
+// and three conversions per candidate pair the conversion is paid once per staged atom.
+__device__ __forceinline__ float4 sr_relative(const uint4 a, uint32_t ox, uint32_t oy, uint32_t oz, float len_unit) {
+    return make_float4((float)(int32_t)(a.x - ox) * len_unit, (float)(int32_t)(a.y - oy) * len_unit,
+                       (float)(int32_t)(a.z - oz) * len_unit, __uint_as_float(a.w));
+}
+
 __global__ void __launch_bounds__(SR_THREADS) sr_force_kernel(const SrParams p) {
-    __shared__ uint4 tile[SR_TILE];
+    __shared__ float4 tile[SR_TILE];
     const int nc = p.nc, c = blockIdx.x, tid = threadIdx.x;
     const int cx = c % nc, cy = (c / nc) % nc, cz = c / (nc * nc);
     const uint32_t s0 = p.start[c], n_own = p.start[c + 1] - s0;
     const float two_sa_over_sqrtpi = 1.1283791670955126f * p.sqrt_alpha;
+    const float rs2 = p.rs2_units * p.len_unit * p.len_unit;                                  // r_s^2 [A^2]
+    // centre of this cell in fixed-point turns: (2 c_d + 1) / (2 nc) of a turn
+    const uint32_t ox = (uint32_t)((((unsigned long long)(2 * cx + 1)) << 31) / (unsigned)nc);
+    const uint32_t oy = (uint32_t)((((unsigned long long)(2 * cy + 1)) << 31) / (unsigned)nc);
+    const uint32_t oz = (uint32_t)((((unsigned long long)(2 * cz + 1)) << 31) / (unsigned)nc);
 
     for (uint32_t pass = 0; pass < n_own; pass += SR_THREADS) {     // (uniform: every thread runs every pass)
         const bool have = pass + tid < n_own;
-        const uint4 me = have ? p.sorted[s0 + pass + tid] : make_uint4(0u, 0u, 0u, 0u);
+        const float4 me = have ? sr_relative(p.sorted[s0 + pass + tid], ox, oy, oz, p.len_unit) : make_float4(0.f, 0.f, 0.f, 0.f);
         float fx = 0.f, fy = 0.f, fz = 0.f, en = 0.f;
         for (int nb = 0; nb < 27; ++nb) {
-            const int ox = nb % 3 - 1, oy = (nb / 3) % 3 - 1, oz = nb / 9 - 1;
-            const int ncx = (cx + ox + nc) % nc, ncy = (cy + oy + nc) % nc, ncz = (cz + oz + nc) % nc;
+            const int dxc = nb % 3 - 1, dyc = (nb / 3) % 3 - 1, dzc = nb / 9 - 1;
+            const int ncx = (cx + dxc + nc) % nc, ncy = (cy + dyc + nc) % nc, ncz = (cz + dzc + nc) % nc;
             const int cn = (ncz * nc + ncy) * nc + ncx;
             const uint32_t n0 = p.start[cn], n1 = p.start[cn + 1];
             for (uint32_t t0 = n0; t0 < n1; t0 += SR_TILE) {
                 const int cnt = (int)min((uint32_t)SR_TILE, n1 - t0);
                 __syncthreads();
-                for (int k = tid; k < cnt; k += SR_THREADS) tile[k] = p.sorted[t0 + k];
+                for (int k = tid; k < cnt; k += SR_THREADS) tile[k] = sr_relative(p.sorted[t0 + k], ox, oy, oz, p.len_unit);
                 __syncthreads();
                 if (!have) continue;
 #pragma unroll 4
                 for (int k = 0; k < cnt; ++k) {
-                    const uint4 o = tile[k];
-                    const float dx = (float)(int32_t)(o.x - me.x), dy = (float)(int32_t)(o.y - me.y), dz = (float)(int32_t)(o.z - me.z);
-                    const float r2u = fmaf(dx, dx, fmaf(dy, dy, dz * dz));
-                    if (r2u < p.rs2_units && r2u > 0.f) {
-                        const float inv_ru = sr_rsqrt(r2u);                  // 1 / r in fixed-point units (r2u >= 1: no denormals)
-                        const float inv_r = inv_ru * (1.0f / p.len_unit);    // 1 / r  [1/A]
-                        const float r = r2u * inv_ru * p.len_unit;           // r      [A]
-                        const float x = p.sqrt_alpha * r;
+                    const float4 o = tile[k];
+                    const float dx = o.x - me.x, dy = o.y - me.y, dz = o.z - me.z;
+                    const float r2 = fmaf(dx, dx, fmaf(dy, dy, dz * dz));
+                    if (r2 < rs2 && r2 > 0.f) {
+                        const float inv_r = sr_rsqrt(r2);
+                        const float x = p.sqrt_alpha * (r2 * inv_r);
                         const float E = sr_ex2(-1.4426950408889634f * x * x);   // exp(-alpha r^2); underflows to 0 harmlessly
                         const float ec = sr_erfc_from_exp(x, E);
-                        const float qj = __uint_as_float(o.w);
-                        // g / r, then the direction d / r in units: (erfc / r^2 + c E / r) / r * d_units / r_units ...
                         const float g = fmaf(ec, inv_r, two_sa_over_sqrtpi * E) * inv_r;   // erfc/r^2 + 2 sqrt(alpha/pi) E / r
-                        const float s = qj * g * inv_ru;                                    // q_j g / r_units
+                        const float s = o.w * g * inv_r;                                    // q_j g / r
                         fx = fmaf(s, dx, fx);
                         fy = fmaf(s, dy, fy);
                         fz = fmaf(s, dz, fz);
-                        en = fmaf(qj * ec, inv_r, en);
+                        en = fmaf(o.w * ec, inv_r, en);
                     }
                 }
             }
         }
         if (have) {
-            const float qi = __uint_as_float(me.w);
+            const float qi = me.w;
             const uint32_t i = p.sidx[s0 + pass + tid];
             float4 o = make_float4(-qi * fx, -qi * fy, -qi * fz, p.with_energy ? 0.5f * qi * en : 0.f);
             if (p.accumulate) {
