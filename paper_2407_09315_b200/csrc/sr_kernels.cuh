@@ -101,12 +101,31 @@ __device__ __forceinline__ uint32_t sr_subcell(const uint4 t, int nc) {
 // One warp per cell: the segment arrives in arbitrary order (atomic slots); rank-sort it by
 // (sub-cell Morton code, atom index) -- a total order, so the layout is deterministic -- in
 // O(n^2 / 32) per lane (n ~ 100), and gather the atom records in that order.
+constexpr int SR_SORT_CAP = 256;   // keys of a cell kept in shared memory by its warp (larger cells: keys recomputed from global)
+
 __global__ void __launch_bounds__(256) sr_sort_kernel(const uint32_t* __restrict__ order, const uint32_t* __restrict__ start,
                                                        int ncell, int nc, const uint4* __restrict__ turns, uint4* __restrict__ sorted,
                                                        uint32_t* __restrict__ sidx) {
-    const int c = (int)(((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5), lane = threadIdx.x & 31;
+    __shared__ unsigned long long keys[8][SR_SORT_CAP];
+    const int c = (int)(((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5), lane = threadIdx.x & 31, w = threadIdx.x >> 5;
     if (c >= ncell) return;
     const uint32_t s0 = start[c], n = start[c + 1] - s0;
+    if (n <= (uint32_t)SR_SORT_CAP) {
+        for (uint32_t e = lane; e < n; e += 32) {
+            const uint32_t o = order[s0 + e];
+            keys[w][e] = ((unsigned long long)sr_subcell(turns[o], nc) << 32) | o;
+        }
+        __syncwarp();
+        for (uint32_t e = lane; e < n; e += 32) {
+            const unsigned long long mkey = keys[w][e];
+            uint32_t rank = 0;
+            for (uint32_t j = 0; j < n; ++j) rank += keys[w][j] < mkey ? 1u : 0u;     // broadcast reads
+            const uint32_t me = (uint32_t)mkey;
+            sorted[s0 + rank] = turns[me];
+            sidx[s0 + rank] = me;
+        }
+        return;
+    }
     for (uint32_t e = lane; e < n; e += 32) {
         const uint32_t me = order[s0 + e];
         const uint4 mt = turns[me];
