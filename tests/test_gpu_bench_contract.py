@@ -1,0 +1,35 @@
+"""bench.py prints ONE JSON line that carries the keys the measurement contract asks for
+(DESIGN.md section 7).  Run on a small parity config so that it takes seconds."""
+import json
+import os
+import subprocess
+import sys
+
+import pytest
+
+pytestmark = pytest.mark.gpu
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def test_bench_json_line_contract():
+    cmd = [sys.executable, os.path.join(ROOT, "bench.py"), "--config", "water_96k", "--steps", "5", "--warmup", "3",
+           "--cpu-baseline-atoms", "20000", "--cpu-baseline-steps", "1"]
+    res = subprocess.run(cmd, capture_output=True, text=True, timeout=600, cwd=ROOT)
+    assert res.returncode == 0, res.stderr[-2000:]
+    lines = [l for l in res.stdout.splitlines() if l.startswith("{")]
+    assert len(lines) == 1
+    d = json.loads(lines[0])
+    assert d["metric"] == "rbe_kspace_ns_per_atom_step" and d["unit"] == "ns/atom/step"
+    assert d["n_gpus"] == 1 and d["steps"] == 5 and d["warmup"] == 3 and d["higher_is_better"] is False
+    assert d["scaling"] == "weak" and d["vs_baseline"] is None and d["dtype"] == "f32" and d["data"] == "synthetic"
+    assert d["config"]["workload"] == "water_96k" and "l2" in d["config"]
+    assert d["value"] > 0 and abs(d["value"] - d["ms_per_step"] * 1e6 / 96000) < 1e-9 * d["value"] + 1e-12
+    r = d["roofline"]
+    assert r["bound"] == "alu" and r["peak"] > 0 and abs(r["frac"] - r["achieved"] / r["peak"]) < 1e-12 and "traffic" in r
+    c = d["cpu_baseline"]
+    assert c["kind"] == "oracle" and c["cores"] >= 1 and c["value"] > d["value"] and "sample" in c
+    e = d["e2e"]
+    assert e["value"] > d["value"] and e["h2d_bytes_per_step"] >= 16 * 96000 and e["d2h_bytes_per_step"] == 16 * 96000
+    assert d["gpu_launches"] == 2 * 5
+    assert set(d["clocks"]) >= {"sm_mhz", "sm_max_mhz", "reasons"}
+    assert d["graph_step"]["gpu_launches_per_step"] == 1 and d["short_range"]["ms_per_call"] > 0
