@@ -307,8 +307,9 @@ __device__ __forceinline__ void reduce_rows(const double2* src, int nrows, int P
 // pair).  MD systems have a handful of distinct charge magnitudes, so nearly all atoms pair up.
 // Compaction of the records is by warp counts + a prefix scan: deterministic order.
 //
-// The last CTA to finish (atomicInc ticket; data order never depends on it) finalises:
-// fixed-order sum of the per-CTA rows and the per-k force coefficients (fin_cta).
+// The last CTAs to finish (atomicInc tickets; data order never depends on them) run the second
+// pass: the fixed-order two-level sum of the per-CTA rows into rho (reduce_rows), and, with a
+// multi-GPU exchange configured, the push of rho into every rank's exchange buffer.
 // ---------------------------------------------------------------------------------------
 struct SfParams {
     const float4* xyzq;
@@ -369,11 +370,6 @@ __device__ __forceinline__ SfWindow sf_classify(uint32_t qbits, bool in_range, i
     w.smask = __ballot_sync(FULL_MASK, w.single);
     w.partner = w.leader ? lane + __ffs(higher) : lane;
     return w;
-}
-__device__ __forceinline__ uint32_t warp_sum(uint32_t v) {
-#pragma unroll
-    for (int d = 16; d > 0; d >>= 1) v += __shfl_xor_sync(FULL_MASK, v, d);
-    return v;
 }
 
 template <bool DEEP>
