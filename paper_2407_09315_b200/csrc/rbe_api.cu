@@ -733,7 +733,21 @@ rbe_status rbe_step_host(rbe_ctx* c, const float* h_xyzq, const int32_t* h_m, co
     int64_t nchunk = c->N / HOST_MIN_CHUNK;
     if (nchunk > HOST_MAX_CHUNKS) nchunk = HOST_MAX_CHUNKS;
     if (nchunk < 1) nchunk = 1;
-    const int64_t chunk = ((c->N + nchunk - 1) / nchunk + 31) / 32 * 32;   // whole 32-atom windows
+    // Chunk boundaries (whole 32-atom windows).  What stays exposed is the structure-factor launch of
+    // the LAST input chunk and the force launch of the FIRST output chunk, so the input chunks shrink
+    // (weights nchunk .. 1) and the output chunks grow (1 .. nchunk); the two splits are independent.
+    int64_t in_lo[HOST_MAX_CHUNKS + 1], out_lo[HOST_MAX_CHUNKS + 1];
+    {
+        const int64_t wsum = nchunk * (nchunk + 1) / 2, units = (c->N + 31) / 32;
+        int64_t acc_in = 0, acc_out = 0;
+        for (int64_t i = 0; i < nchunk; ++i) {
+            in_lo[i] = units * acc_in / wsum * 32;
+            out_lo[i] = units * acc_out / wsum * 32;
+            acc_in += nchunk - i;
+            acc_out += i + 1;
+        }
+        in_lo[nchunk] = out_lo[nchunk] = c->N;
+    }
     const unsigned evflag = cudaEventDisableTiming;
     if (nchunk > 1 && !c->s_h2d) {
         RBE_CUDA(c, cudaStreamCreateWithFlags(&c->s_h2d, cudaStreamNonBlocking));
@@ -757,7 +771,7 @@ rbe_status rbe_step_host(rbe_ctx* c, const float* h_xyzq, const int32_t* h_m, co
         RBE_CUDA(c, cudaStreamWaitEvent(c->s_h2d, c->ev_start, 0));
         RBE_CUDA(c, cudaStreamWaitEvent(c->s_d2h, c->ev_start, 0));
         for (int64_t i = 0; i < nchunk; ++i) {
-            const int64_t lo = i * chunk, n = (lo + chunk <= c->N ? chunk : c->N - lo);
+            const int64_t lo = in_lo[i], n = in_lo[i + 1] - lo;
             RBE_CUDA(c, cudaMemcpyAsync(d_x + lo, h_x + lo, (size_t)n * sizeof(float4), cudaMemcpyHostToDevice, c->s_h2d));
             RBE_CUDA(c, cudaEventRecord(c->ev_in[i], c->s_h2d));
             RBE_CUDA(c, cudaStreamWaitEvent(st, c->ev_in[i], 0));
@@ -766,7 +780,7 @@ rbe_status rbe_step_host(rbe_ctx* c, const float* h_xyzq, const int32_t* h_m, co
         }
         c->have_rho = true;
         for (int64_t i = 0; i < nchunk; ++i) {
-            const int64_t lo = i * chunk, n = (lo + chunk <= c->N ? chunk : c->N - lo);
+            const int64_t lo = out_lo[i], n = out_lo[i + 1] - lo;
             s = launch_f(c, d_x + lo, d_f + lo, n, with_energy, st);
             if (s != RBE_OK) return s;
             RBE_CUDA(c, cudaEventRecord(c->ev_f[i], st));
