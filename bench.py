@@ -318,10 +318,10 @@ def main():
         ms_sr = e0.elapsed_time(e1) / k_sr
         nbr = 4.0 / 3.0 * np.pi * args.rs ** 3 * n_local / L ** 3          # expected atoms inside the cutoff sphere
         sr = {"ms_per_call": ms_sr, "value": ms_sr * 1e6 / n_local, "unit": UNIT.replace("/step", "/call"),
-              "r_s": args.rs, "neighbours_per_atom_expected": nbr, "calls": k_sr, "gpu_launches_per_call": 5,
+              "r_s": args.rs, "neighbours_per_atom_expected": nbr, "calls": k_sr, "gpu_launches_per_call": 7,
               "pair_rate_G_per_s": nbr * n_local / (ms_sr * 1e-3) / 1e9,
-              "note": "rbe_short_range: bin + scan + scatter + sort + cell-pair force kernel; every ordered pair "
-                      "inside the cutoff is evaluated once per atom (no Newton-3 sharing); not part of `value`"}
+              "note": "rbe_short_range: bin + scan + scatter + sort + group boxes + pair kernel (every unordered pair "
+                      "once, fixed-point integer atomics across warps) + finalise; not part of `value`"}
 
     if world > 1:
         t = torch.tensor([ms_total, ms_sf, ms_f], dtype=torch.float64, device="cuda")

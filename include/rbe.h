@@ -200,15 +200,17 @@ rbe_status rbe_forces(rbe_ctx* ctx, const void* d_xyzq, void* d_force, int32_t w
  *            + 2 sqrt(alpha) exp(-alpha r^2) / (sqrt(pi) r) ) d / r,   d = nearest image of r_j - r_i
  *   e_i = 1/2 q_i sum_{j != i, r < r_s} q_j erfc(sqrt(alpha) r) / r      (first term of Eq. 2.8)
  * with this context's L and alpha.  Coincident atoms (r = 0) are skipped.  Independent of the
- * k-set; needs no rbe_set_workspace.  fp32 arithmetic on exact fixed-point separations; erfc by
- * Abramowitz-Stegun 7.1.26 (|error| <= 1.5e-7); every atom's sum runs in a fixed order (cells sorted
- * by atom index), so the result is bitwise reproducible.
+ * k-set; needs no rbe_set_workspace.  fp32 arithmetic on cell-relative coordinates derived from exact
+ * fixed-point separations; erfc by Abramowitz-Stegun 7.1.26 (|error| <= 1.5e-7).  Every unordered pair
+ * is evaluated once (Newton's third law); partial sums of different warps are combined in 64-bit
+ * fixed point with integer atomics (scale 2^36: |F_i / q_i| must stay below 1.3e8 e/A^2), so the result
+ * is bitwise reproducible.
  *   d_xyzq      float4 [N] device;  rs  cutoff radius [A], 0 < rs <= L/3
  *   d_force     float4 [N] device: {F_x, F_y, F_z, e_i}; e_i = 0 unless with_energy != 0
  *   accumulate  != 0: add to what d_force holds (e.g. the k-space force of rbe_forces)
- *   d_ws        caller-owned device scratch of rbe_short_range_bytes(ctx, rs) bytes (~44 B per atom
- *               + 12 B per cell), 256-byte aligned; its contents are rebuilt by every call
- * rbe_short_range_bytes returns 0 for an invalid rs.  Enqueues five kernels on `stream`.
+ *   d_ws        caller-owned device scratch of rbe_short_range_bytes(ctx, rs) bytes (~76 B per atom
+ *               + 204 B per cell), 256-byte aligned; its contents are rebuilt by every call
+ * rbe_short_range_bytes returns 0 for an invalid rs.  Enqueues seven kernels and one memset on `stream`.
  * Errors: RBE_ERR_INVALID_ARG, RBE_ERR_WORKSPACE, RBE_ERR_NO_DEVICE, RBE_ERR_CUDA. */
 size_t     rbe_short_range_bytes(const rbe_ctx* ctx, double rs);
 rbe_status rbe_short_range(rbe_ctx* ctx, const void* d_xyzq, double rs, void* d_force, int32_t accumulate,

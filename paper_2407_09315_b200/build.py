@@ -12,7 +12,7 @@ ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
 SO = os.path.join(HERE, "librbe.so")
 SOURCES = [os.path.join(CSRC, "rbe_api.cu")]
-DEPS = SOURCES + [os.path.join(CSRC, "rbe_kernels.cuh"), os.path.join(CSRC, "sr_kernels.cuh"), os.path.join(ROOT, "include", "rbe.h")]
+DEPS = SOURCES + [os.path.join(CSRC, f) for f in sorted(os.listdir(CSRC)) if f.endswith(".cuh")] + [os.path.join(ROOT, "include", "rbe.h")]
 PROBE = os.path.join(HERE, "pipe_probe")
 PROBE_SRC = os.path.join(CSRC, "pipe_probe.cu")
 

@@ -11,6 +11,7 @@
 
 #include "rbe_kernels.cuh"
 #include "sr_kernels.cuh"
+#include "sr_pair_kernels.cuh"
 
 #ifdef RBE_SF_PROFILE
 static long long* g_rbe_prof = nullptr;
@@ -628,6 +629,7 @@ struct SrLayout {
     int nc = 0;
     int64_t ncell = 0;
     size_t off_turns = 0, off_sorted = 0, off_cell = 0, off_order = 0, off_sidx = 0, off_count = 0, off_cursor = 0, off_start = 0;
+    size_t off_acc = 0, off_gbox = 0;
     size_t bytes = 0;
 };
 bool sr_layout(const rbe_ctx* c, double rs, SrLayout& l) {
@@ -646,6 +648,8 @@ bool sr_layout(const rbe_ctx* c, double rs, SrLayout& l) {
     l.off_count = off;  off = align_up(off + nce * sizeof(uint32_t), 256);
     l.off_cursor = off; off = align_up(off + nce * sizeof(uint32_t), 256);
     l.off_start = off;  off = align_up(off + (nce + 1) * sizeof(uint32_t), 256);
+    l.off_acc = off;    off = align_up(off + N * 4 * sizeof(long long), 256);
+    l.off_gbox = off;   off = align_up(off + nce * rbe::SR_GMAX * 6 * sizeof(float), 256);
     l.bytes = off;
     return true;
 }
@@ -684,15 +688,20 @@ rbe_status rbe_short_range(rbe_ctx* c, const void* d_xyzq, double rs, void* d_fo
     rbe::sr_scan_kernel<<<1, 1024, 0, st>>>(count, (int)l.ncell, start, cursor);
     rbe::sr_scatter_kernel<<<nb, 256, 0, st>>>(cell_of, c->N, start, cursor, order);
     rbe::sr_sort_kernel<<<(unsigned)((l.ncell * 32 + 255) / 256), 256, 0, st>>>(order, start, (int)l.ncell, l.nc, turns, sorted, sidx);
-    rbe::SrParams sp;
-    sp.sorted = sorted; sp.sidx = sidx; sp.start = start;
-    sp.force = static_cast<float4*>(d_force);
-    sp.nc = l.nc; sp.accumulate = accumulate; sp.with_energy = with_energy;
-    sp.len_unit = (float)(c->L / rbe::TWO32);
-    const double rsu = rs * rbe::TWO32 / c->L;
-    sp.rs2_units = (float)(rsu * rsu);
-    sp.sqrt_alpha = (float)std::sqrt(c->alpha);
-    rbe::sr_force_kernel<<<(unsigned)l.ncell, rbe::SR_THREADS, 0, st>>>(sp);
+    long long* acc = reinterpret_cast<long long*>(w + l.off_acc);
+    float* gbox = reinterpret_cast<float*>(w + l.off_gbox);
+    const float len_unit = (float)(c->L / rbe::TWO32);
+    RBE_CUDA(c, cudaMemsetAsync(acc, 0, (size_t)c->N * 4 * sizeof(long long), st));
+    rbe::sr_gbox_kernel<<<(unsigned)((l.ncell * 32 + 255) / 256), 256, 0, st>>>(sorted, start, (int)l.ncell, l.nc, len_unit, gbox);
+    rbe::SrPairParams pp;
+    pp.sorted = sorted; pp.start = start; pp.gbox = gbox; pp.acc = acc;
+    pp.nc = l.nc;
+    pp.len_unit = len_unit;
+    pp.cell_len = (float)(c->L / l.nc);
+    pp.rs2 = (float)(rs * rs);
+    pp.sqrt_alpha = (float)std::sqrt(c->alpha);
+    rbe::sr_pair_kernel<<<(unsigned)l.ncell, 32 * rbe::SR_PAIR_WARPS, 0, st>>>(pp);
+    rbe::sr_finalize_kernel<<<nb, 256, 0, st>>>(acc, sorted, sidx, c->N, static_cast<float4*>(d_force), accumulate, with_energy);
     RBE_CUDA(c, cudaGetLastError());
     return RBE_OK;
 }

@@ -16,7 +16,7 @@
 //   sr_scatter  atom indices into their cell's segment (slot by integer atomic: arbitrary order)
 //   sr_sort     one warp per cell: rank-sort the segment by (sub-cell Morton code, atom index), gather
 //               {S, q} in that order -> the layout and every sum below are bitwise reproducible
-//   sr_force    one CTA per cell: neighbour cells staged in shared memory, a thread owns an atom
+//   sr_gbox, sr_pair, sr_finalize   (sr_pair_kernels.cuh) the force kernel proper
 #pragma once
 #include <cstdint>
 #include <cuda_runtime.h>
@@ -25,8 +25,6 @@
 
 namespace rbe {
 
-constexpr int SR_THREADS = 128;   // force kernel: threads per CTA = atoms of the cell handled per pass
-constexpr int SR_TILE = 256;      // neighbour atoms staged in shared memory at a time
 
 __device__ __forceinline__ int sr_cell_of(uint32_t Sx, uint32_t Sy, uint32_t Sz, int nc) {
     return ((int)__umulhi(Sz, (uint32_t)nc) * nc + (int)__umulhi(Sy, (uint32_t)nc)) * nc + (int)__umulhi(Sx, (uint32_t)nc);
@@ -141,18 +139,6 @@ __global__ void __launch_bounds__(256) sr_sort_kernel(const uint32_t* __restrict
     }
 }
 
-struct SrParams {
-    const uint4* sorted;      // [N] {Sx, Sy, Sz, q} in cell order
-    const uint32_t* sidx;     // [N] original atom index
-    const uint32_t* start;    // [ncell + 1]
-    float4* force;            // [N] {F, e_i}, original atom order
-    int32_t nc;               // cells per dimension (>= 3)
-    int32_t accumulate;       // add to what `force` holds (e.g. the k-space force)
-    int32_t with_energy;
-    float len_unit;           // L / 2^32: length of one fixed-point unit [A]
-    float rs2_units;          // (r_s / len_unit)^2: the cutoff in fixed-point units squared
-    float sqrt_alpha;         // sqrt(alpha) [1/A]
-};
 
 // erfc(x) = t (a1 + t (a2 + t (a3 + t (a4 + t a5)))) exp(-x^2), t = 1 / (1 + p x): Abramowitz & Stegun
 // 7.1.26, |error| <= 1.5e-7 for x >= 0.  E = exp(-x^2) is shared with the Gaussian term of Eq. (2.10).
@@ -177,66 +163,6 @@ __device__ __forceinline__ float sr_erfc_from_exp(float x, float E) {
 __device__ __forceinline__ float4 sr_relative(const uint4 a, uint32_t ox, uint32_t oy, uint32_t oz, float len_unit) {
     return make_float4((float)(int32_t)(a.x - ox) * len_unit, (float)(int32_t)(a.y - oy) * len_unit,
                        (float)(int32_t)(a.z - oz) * len_unit, __uint_as_float(a.w));
-}
-
-__global__ void __launch_bounds__(SR_THREADS) sr_force_kernel(const SrParams p) {
-    __shared__ float4 tile[SR_TILE];
-    const int nc = p.nc, c = blockIdx.x, tid = threadIdx.x;
-    const int cx = c % nc, cy = (c / nc) % nc, cz = c / (nc * nc);
-    const uint32_t s0 = p.start[c], n_own = p.start[c + 1] - s0;
-    const float two_sa_over_sqrtpi = 1.1283791670955126f * p.sqrt_alpha;
-    const float rs2 = p.rs2_units * p.len_unit * p.len_unit;                                  // r_s^2 [A^2]
-    // centre of this cell in fixed-point turns: (2 c_d + 1) / (2 nc) of a turn
-    const uint32_t ox = (uint32_t)((((unsigned long long)(2 * cx + 1)) << 31) / (unsigned)nc);
-    const uint32_t oy = (uint32_t)((((unsigned long long)(2 * cy + 1)) << 31) / (unsigned)nc);
-    const uint32_t oz = (uint32_t)((((unsigned long long)(2 * cz + 1)) << 31) / (unsigned)nc);
-
-    for (uint32_t pass = 0; pass < n_own; pass += SR_THREADS) {     // (uniform: every thread runs every pass)
-        const bool have = pass + tid < n_own;
-        const float4 me = have ? sr_relative(p.sorted[s0 + pass + tid], ox, oy, oz, p.len_unit) : make_float4(0.f, 0.f, 0.f, 0.f);
-        float fx = 0.f, fy = 0.f, fz = 0.f, en = 0.f;
-        for (int nb = 0; nb < 27; ++nb) {
-            const int dxc = nb % 3 - 1, dyc = (nb / 3) % 3 - 1, dzc = nb / 9 - 1;
-            const int ncx = (cx + dxc + nc) % nc, ncy = (cy + dyc + nc) % nc, ncz = (cz + dzc + nc) % nc;
-            const int cn = (ncz * nc + ncy) * nc + ncx;
-            const uint32_t n0 = p.start[cn], n1 = p.start[cn + 1];
-            for (uint32_t t0 = n0; t0 < n1; t0 += SR_TILE) {
-                const int cnt = (int)min((uint32_t)SR_TILE, n1 - t0);
-                __syncthreads();
-                for (int k = tid; k < cnt; k += SR_THREADS) tile[k] = sr_relative(p.sorted[t0 + k], ox, oy, oz, p.len_unit);
-                __syncthreads();
-                if (!have) continue;
-#pragma unroll 4
-                for (int k = 0; k < cnt; ++k) {
-                    const float4 o = tile[k];
-                    const float dx = o.x - me.x, dy = o.y - me.y, dz = o.z - me.z;
-                    const float r2 = fmaf(dx, dx, fmaf(dy, dy, dz * dz));
-                    if (r2 < rs2 && r2 > 0.f) {
-                        const float inv_r = sr_rsqrt(r2);
-                        const float x = p.sqrt_alpha * (r2 * inv_r);
-                        const float E = sr_ex2(-1.4426950408889634f * x * x);   // exp(-alpha r^2); underflows to 0 harmlessly
-                        const float ec = sr_erfc_from_exp(x, E);
-                        const float g = fmaf(ec, inv_r, two_sa_over_sqrtpi * E) * inv_r;   // erfc/r^2 + 2 sqrt(alpha/pi) E / r
-                        const float s = o.w * g * inv_r;                                    // q_j g / r
-                        fx = fmaf(s, dx, fx);
-                        fy = fmaf(s, dy, fy);
-                        fz = fmaf(s, dz, fz);
-                        en = fmaf(o.w * ec, inv_r, en);
-                    }
-                }
-            }
-        }
-        if (have) {
-            const float qi = me.w;
-            const uint32_t i = p.sidx[s0 + pass + tid];
-            float4 o = make_float4(-qi * fx, -qi * fy, -qi * fz, p.with_energy ? 0.5f * qi * en : 0.f);
-            if (p.accumulate) {
-                const float4 prev = p.force[i];
-                o.x += prev.x; o.y += prev.y; o.z += prev.z; o.w += prev.w;
-            }
-            p.force[i] = o;
-        }
-    }
 }
 
 }  // namespace rbe

@@ -1,0 +1,198 @@
+// sr_pair_kernels.cuh -- the force kernel of the real-space partner (Eq. 2.10 P:122 truncated at r_s,
+// P:127), second design: every unordered pair is evaluated ONCE (Newton's third law) and whole
+// 32 x 32 blocks of pairs are skipped by a bounding-box test, yet the result stays bitwise
+// reproducible.  (First design, sr_kernels.cuh::sr_force_kernel: a thread per atom against all 27
+// neighbour cells, every ordered pair tested: 2 900 cutoff tests per atom at r_s = 10 A.)
+//
+// Work unit.  The atoms are sorted by cell and, inside a cell, by a Morton code of sub-cells
+// (sr_sort_kernel), so a GROUP = 32 consecutive atoms of one cell is spatially compact; its bounding
+// box comes from sr_gbox_kernel.  A warp owns one group I of cell c (a lane = an atom, coordinates in
+// fp32 Angstrom relative to the centre of c, nearest image implicit in the wrapped integer
+// difference) and meets the groups J of the 13 "forward" neighbour cells, and of its own cell with
+// J >= I, so that every unordered pair of groups is met exactly once.  Blocks whose boxes are
+// farther apart than r_s are skipped (about half of them).  For a surviving block the J atoms and
+// their accumulators sit in shared memory; in step t lane l handles the pair (l, (l + t) mod 32):
+// all lanes touch different J atoms, so both sides of a pair are accumulated without atomics and in
+// a fixed order.
+//
+// Combining contributions that come from different warps.  A group receives partial forces from
+// ~20 other warps.  They are added in 64-bit FIXED POINT with integer atomics: integer addition is
+// associative, so the sum does not depend on the order in which the warps arrive -- no
+// floating-point atomics anywhere.  Scale 2^36 per e^2/A^2 (resolution 1.5e-11, range +-1.3e8).
+// sr_finalize_kernel converts back to fp32, applies -q_i and scatters to the caller's atom order.
+#pragma once
+#include "sr_kernels.cuh"
+
+namespace rbe {
+
+constexpr int SR_GMAX = 8;                       // groups per cell that carry a bounding box (more: never skipped)
+constexpr double SR_FIXED_SCALE = 68719476736.0; // 2^36
+
+struct SrPairParams {
+    const uint4* sorted;      // [N] {Sx, Sy, Sz, q} in cell order
+    const uint32_t* start;    // [ncell + 1]
+    const float* gbox;        // [ncell][SR_GMAX][6] {lo xyz, hi xyz} of a group, A, relative to its cell's centre
+    long long* acc;           // [N][4] fixed-point {A_x, A_y, A_z, E}, sorted order, zeroed before the launch
+    int32_t nc;
+    float len_unit;           // L / 2^32 [A]
+    float cell_len;           // L / nc [A]
+    float rs2;                // r_s^2 [A^2]
+    float sqrt_alpha;
+};
+
+__device__ __forceinline__ uint32_t sr_cell_centre(int cd, int nc) {
+    return (uint32_t)((((unsigned long long)(2 * cd + 1)) << 31) / (unsigned)nc);   // (2 c + 1) / (2 nc) of a turn
+}
+
+// Bounding boxes of the first SR_GMAX groups of every cell.  One warp per cell.
+__global__ void __launch_bounds__(256) sr_gbox_kernel(const uint4* __restrict__ sorted, const uint32_t* __restrict__ start,
+                                                       int ncell, int nc, float len_unit, float* __restrict__ gbox) {
+    const int c = (int)(((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5), lane = threadIdx.x & 31;
+    if (c >= ncell) return;
+    const uint32_t s0 = start[c], n = start[c + 1] - s0;
+    const uint32_t ox = sr_cell_centre(c % nc, nc), oy = sr_cell_centre((c / nc) % nc, nc), oz = sr_cell_centre(c / (nc * nc), nc);
+    for (int g = 0; g < SR_GMAX && (uint32_t)(32 * g) < n; ++g) {
+        const uint32_t e = 32u * g + lane;
+        float lo[3] = {3.0e38f, 3.0e38f, 3.0e38f}, hi[3] = {-3.0e38f, -3.0e38f, -3.0e38f};
+        if (e < n) {
+            const float4 a = sr_relative(sorted[s0 + e], ox, oy, oz, len_unit);
+            lo[0] = hi[0] = a.x; lo[1] = hi[1] = a.y; lo[2] = hi[2] = a.z;
+        }
+#pragma unroll
+        for (int d = 16; d > 0; d >>= 1)
+#pragma unroll
+            for (int k = 0; k < 3; ++k) {
+                lo[k] = fminf(lo[k], __shfl_xor_sync(FULL_MASK, lo[k], d));
+                hi[k] = fmaxf(hi[k], __shfl_xor_sync(FULL_MASK, hi[k], d));
+            }
+        if (lane < 6) gbox[((int64_t)c * SR_GMAX + g) * 6 + lane] = lane < 3 ? lo[lane] : hi[lane - 3];
+    }
+}
+
+__device__ __forceinline__ void sr_atomic_add_fixed(long long* p, float v) {
+    atomicAdd(reinterpret_cast<unsigned long long*>(p), (unsigned long long)__double2ll_rn((double)v * SR_FIXED_SCALE));
+}
+
+constexpr int SR_PAIR_WARPS = 4;
+
+// the own cell, then the 13 forward neighbours: (dz > 0) or (dz == 0 and dy > 0) or (dz == dy == 0 and dx > 0)
+__constant__ int8_t SR_HALF_STENCIL[14][3] = {
+    {0, 0, 0},  {1, 0, 0},  {-1, 1, 0}, {0, 1, 0},  {1, 1, 0},  {-1, -1, 1}, {0, -1, 1},
+    {1, -1, 1}, {-1, 0, 1}, {0, 0, 1},  {1, 0, 1},  {-1, 1, 1}, {0, 1, 1},   {1, 1, 1}};
+
+__global__ void __launch_bounds__(32 * SR_PAIR_WARPS) sr_pair_kernel(const SrPairParams p) {
+    __shared__ float4 vpos[SR_PAIR_WARPS][32];   // the visiting group: positions relative to THIS cell's centre, charge
+    __shared__ float4 vacc[SR_PAIR_WARPS][32];   // ... and what this warp adds to its atoms
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    const int nc = p.nc, c = blockIdx.x;
+    const int cx = c % nc, cy = (c / nc) % nc, cz = c / (nc * nc);
+    const uint32_t ox = sr_cell_centre(cx, nc), oy = sr_cell_centre(cy, nc), oz = sr_cell_centre(cz, nc);
+    const uint32_t s0 = p.start[c], n_own = p.start[c + 1] - s0;
+    const int ng_own = (int)((n_own + 31) >> 5);
+    const float two_sa_over_sqrtpi = 1.1283791670955126f * p.sqrt_alpha;
+    const float FAR = 1.0e18f;   // position of an empty lane: its pairs always fail the cutoff test (and FAR - FAR = 0 is skipped)
+
+    for (int g = w; g < ng_own; g += SR_PAIR_WARPS) {
+        const uint32_t ei = 32u * g + lane;
+        const bool have = ei < n_own;
+        const float4 me = have ? sr_relative(p.sorted[s0 + ei], ox, oy, oz, p.len_unit) : make_float4(FAR, FAR, FAR, 0.f);
+        float ilo[3] = {-3.0e38f, -3.0e38f, -3.0e38f}, ihi[3] = {3.0e38f, 3.0e38f, 3.0e38f};
+        if (g < SR_GMAX) {
+            const float* b = p.gbox + ((int64_t)c * SR_GMAX + g) * 6;
+#pragma unroll
+            for (int k = 0; k < 3; ++k) { ilo[k] = b[k]; ihi[k] = b[3 + k]; }
+        }
+        float fx = 0.f, fy = 0.f, fz = 0.f, en = 0.f;
+
+        for (int nb = 0; nb < 14; ++nb) {
+            const int dxc = SR_HALF_STENCIL[nb][0], dyc = SR_HALF_STENCIL[nb][1], dzc = SR_HALF_STENCIL[nb][2];
+            const int cn = (((cz + dzc + nc) % nc) * nc + (cy + dyc + nc) % nc) * nc + (cx + dxc + nc) % nc;
+            const uint32_t n0 = p.start[cn], nn = p.start[cn + 1] - n0;
+            const int ngn = (int)((nn + 31) >> 5);
+            const float shift[3] = {dxc * p.cell_len, dyc * p.cell_len, dzc * p.cell_len};
+            for (int h = nb == 0 ? g : 0; h < ngn; ++h) {
+                const bool self_block = nb == 0 && h == g;
+                if (g < SR_GMAX && h < SR_GMAX && !self_block) {
+                    // squared distance between the two bounding boxes: skip the 32 x 32 block when beyond the cutoff
+                    const float* b = p.gbox + ((int64_t)cn * SR_GMAX + h) * 6;
+                    float d2 = 0.f;
+#pragma unroll
+                    for (int k = 0; k < 3; ++k) {
+                        const float gap = fmaxf(0.f, fmaxf(b[k] + shift[k] - ihi[k], ilo[k] - (b[3 + k] + shift[k])));
+                        d2 = fmaf(gap, gap, d2);
+                    }
+                    if (d2 >= p.rs2) continue;
+                }
+                const uint32_t ej = 32u * h + lane;
+                const bool jvalid = ej < nn;
+                __syncwarp();
+                vpos[w][lane] = jvalid ? sr_relative(p.sorted[n0 + ej], ox, oy, oz, p.len_unit) : make_float4(FAR, FAR, FAR, 0.f);
+                vacc[w][lane] = make_float4(0.f, 0.f, 0.f, 0.f);
+                __syncwarp();
+#pragma unroll 4
+                for (int t = 0; t < 32; ++t) {
+                    const int v = (lane + t) & 31;                 // every lane meets a different visitor in every step
+                    const float4 o = vpos[w][v];
+                    const float dx = o.x - me.x, dy = o.y - me.y, dz = o.z - me.z;
+                    const float r2 = fmaf(dx, dx, fmaf(dy, dy, dz * dz));
+                    if (r2 < p.rs2 && r2 > 0.f) {
+                        const float inv_r = sr_rsqrt(r2);
+                        const float x = p.sqrt_alpha * (r2 * inv_r);
+                        const float E = sr_ex2(-1.4426950408889634f * x * x);
+                        const float ec = sr_erfc_from_exp(x, E);
+                        const float s = fmaf(ec, inv_r, two_sa_over_sqrtpi * E) * inv_r * inv_r;   // g / r
+                        const float u = ec * inv_r;
+                        const float sj = o.w * s;
+                        fx = fmaf(sj, dx, fx); fy = fmaf(sj, dy, fy); fz = fmaf(sj, dz, fz);
+                        en = fmaf(o.w, u, en);
+                        if (!self_block) {                          // the same pair term, seen from the visitor (d -> -d)
+                            const float si = me.w * s;
+                            float4 a = vacc[w][v];
+                            a.x = fmaf(-si, dx, a.x); a.y = fmaf(-si, dy, a.y); a.z = fmaf(-si, dz, a.z);
+                            a.w = fmaf(me.w, u, a.w);
+                            vacc[w][v] = a;
+                        }
+                    }
+                    __syncwarp();
+                }
+                if (!self_block && jvalid) {
+                    const float4 a = vacc[w][lane];
+                    long long* dst = p.acc + 4 * (int64_t)(n0 + ej);
+                    if (a.x != 0.f) sr_atomic_add_fixed(dst + 0, a.x);
+                    if (a.y != 0.f) sr_atomic_add_fixed(dst + 1, a.y);
+                    if (a.z != 0.f) sr_atomic_add_fixed(dst + 2, a.z);
+                    if (a.w != 0.f) sr_atomic_add_fixed(dst + 3, a.w);
+                }
+            }
+        }
+        if (have) {
+            long long* dst = p.acc + 4 * (int64_t)(s0 + ei);
+            sr_atomic_add_fixed(dst + 0, fx);
+            sr_atomic_add_fixed(dst + 1, fy);
+            sr_atomic_add_fixed(dst + 2, fz);
+            sr_atomic_add_fixed(dst + 3, en);
+        }
+    }
+}
+
+// Fixed point -> fp32, F_i = -q_i A_i, e_i = q_i E_i / 2, scattered to the caller's atom order.
+__global__ void __launch_bounds__(256) sr_finalize_kernel(const long long* __restrict__ acc, const uint4* __restrict__ sorted,
+                                                           const uint32_t* __restrict__ sidx, int64_t N, float4* __restrict__ force,
+                                                           int accumulate, int with_energy) {
+    const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= N) return;
+    const double inv = 1.0 / SR_FIXED_SCALE;
+    const float q = __uint_as_float(sorted[k].w);
+    const longlong2 a01 = reinterpret_cast<const longlong2*>(acc)[2 * k], a23 = reinterpret_cast<const longlong2*>(acc)[2 * k + 1];
+    float4 o = make_float4(-q * (float)((double)a01.x * inv), -q * (float)((double)a01.y * inv), -q * (float)((double)a23.x * inv),
+                           with_energy ? 0.5f * q * (float)((double)a23.y * inv) : 0.f);
+    const uint32_t i = sidx[k];
+    if (accumulate) {
+        const float4 prev = force[i];
+        o.x += prev.x; o.y += prev.y; o.z += prev.z; o.w += prev.w;
+    }
+    force[i] = o;
+}
+
+
+}  // namespace rbe
