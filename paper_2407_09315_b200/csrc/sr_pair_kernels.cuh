@@ -73,14 +73,20 @@ __device__ __forceinline__ void sr_atomic_add_fixed(long long* p, float v) {
     atomicAdd(reinterpret_cast<unsigned long long*>(p), (unsigned long long)__double2ll_rn((double)v * SR_FIXED_SCALE));
 }
 
-constexpr int SR_PAIR_WARPS = 4;
+#ifndef RBE_SR_PAIR_WARPS
+#define RBE_SR_PAIR_WARPS 4
+#endif
+#ifndef RBE_SR_PAIR_CTAS
+#define RBE_SR_PAIR_CTAS 9
+#endif
+constexpr int SR_PAIR_WARPS = RBE_SR_PAIR_WARPS;
 
 // the own cell, then the 13 forward neighbours: (dz > 0) or (dz == 0 and dy > 0) or (dz == dy == 0 and dx > 0)
 __constant__ int8_t SR_HALF_STENCIL[14][3] = {
     {0, 0, 0},  {1, 0, 0},  {-1, 1, 0}, {0, 1, 0},  {1, 1, 0},  {-1, -1, 1}, {0, -1, 1},
     {1, -1, 1}, {-1, 0, 1}, {0, 0, 1},  {1, 0, 1},  {-1, 1, 1}, {0, 1, 1},   {1, 1, 1}};
 
-__global__ void __launch_bounds__(32 * SR_PAIR_WARPS) sr_pair_kernel(const SrPairParams p) {
+__global__ void __launch_bounds__(32 * SR_PAIR_WARPS, RBE_SR_PAIR_CTAS) sr_pair_kernel(const SrPairParams p) {
     __shared__ float4 vpos[SR_PAIR_WARPS][32];   // the visiting group: positions relative to THIS cell's centre, charge
     __shared__ float4 vacc[SR_PAIR_WARPS][32];   // ... and what this warp adds to its atoms
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;

@@ -84,3 +84,39 @@ def test_graph_replay_advances_the_step_and_matches_separate_launches(name):
     ref.rbe_structure_factor(x)
     ref.rbe_forces(x, Fs, True)
     assert torch.equal(Fg, Fs)
+
+
+def test_mean_of_graph_replays_converges_to_the_deterministic_ewald_force():
+    """End to end on the device (sampler + structure factor + force, one graph launch per step): the RBE
+    force is an unbiased estimator of Eq. (2.11), so the mean over T replays approaches the
+    full k-space force of oracle.ewald_full like 1/sqrt(T); the residual after T and 4T steps must
+    shrink by about 2, and be consistent with the closed-form variance (~ 1/P)."""
+    L, alpha, P = 20.0, 0.25, 50
+    cfg = inputs.ions_config(400)
+    atoms = inputs.make_atoms(cfg)
+    atoms[:, :3] *= np.float32(L / cfg.L)
+    x = torch.from_numpy(atoms).cuda()
+    F = torch.empty((400, 4), dtype=torch.float32, device="cuda")
+    ctx = rbe.Rbe(400, L, alpha, P)
+    ctx.rbe_graph_capture(x, F, False, seed=77, first_step=0)
+    _, _, F_long = oracle.ewald_full(atoms[:, :3].astype(np.float64), atoms[:, 3].astype(np.float64), L, alpha, nreal=0, mmax=14)
+    acc = torch.zeros((400, 3), dtype=torch.float64, device="cuda")
+    sq = torch.zeros((), dtype=torch.float64, device="cuda")
+    res = {}
+    for t in range(1, 1601):
+        ctx.rbe_graph_launch()
+        f = F[:, :3].double()
+        acc += f
+        sq += (f * f).sum()
+        if t in (400, 1600):
+            res[t] = np.linalg.norm((acc / t).cpu().numpy() - F_long)
+    nrm = np.linalg.norm(F_long)
+    # variance of one step's estimate (summed over components), measured, predicts the residual of the mean
+    var1 = float(sq.item()) / 1600 - float(((acc / 1600) ** 2).sum().item())
+    # (the per-step error is heavy-tailed -- rare small-|k| samples carry large weights -- so the typical
+    # residual sits below its rms expectation; a bias would show as a floor that does not shrink)
+    for t in (400, 1600):
+        expect = np.sqrt(var1 / t)
+        assert 0.4 * expect <= res[t] <= 1.5 * expect, (t, res[t], expect)
+    assert 1.4 <= res[400] / res[1600] <= 2.8, res
+    assert res[1600] <= 0.2 * nrm
