@@ -59,7 +59,7 @@ typedef enum {
     RBE_ERR_NO_DEVICE = 6     /* no usable sm_100 device: there is no CPU fallback */
 } rbe_status;
 
-/* Launch geometry of the three kernels, for benchmarks and profiles (read-only information). */
+/* Launch geometry of the two k-space kernels, for benchmarks and profiles (read-only information). */
 typedef struct {
     int32_t num_sms;
     int32_t sf_grid_x, sf_grid_y, sf_threads, sf_smem_bytes; /* structure-factor kernel */
