@@ -1,0 +1,66 @@
+"""Pins of the random-batch-list oracle (oracle/rbl.py; Eqs. 2.13-2.16, reading Q20)."""
+import numpy as np
+
+import oracle
+from oracle import rbl
+
+
+def _cell(n, L, seed):
+    rng = np.random.default_rng(seed)
+    a = np.empty((n, 4), dtype=np.float32)
+    a[:, :3] = rng.random((n, 3)) * L
+    a[:, 3] = np.where(np.arange(n) % 2 == 0, 1.0, -1.0)
+    return a
+
+
+def test_whole_shell_in_the_batch_reproduces_the_deterministic_sum():
+    """p >= N_s for every atom: B(i) = S(i), scale 1, so core + shell = Eq. (2.10) truncated at r_s and the
+    correction vanishes with it (Newton's third law)."""
+    L, alpha, rc, rs = 24.0, 0.09, 4.0, 8.0
+    a = _cell(500, L, 1)
+    F, Ns, Fc = rbl.rbl_forces(a, L, alpha, rc, rs, p=10_000, seed=3, step=0)
+    Fd, _ = oracle.short_range(a, L, alpha, rs)
+    assert np.abs(F - Fd).max() <= 1e-12 * np.abs(Fd).max()
+    assert np.abs(Fc).max() <= 1e-13 * np.abs(Fd).max()
+    # N_s by brute force for a few atoms
+    r = a[:, :3].astype(np.float64)
+    for i in (0, 17, 499):
+        d = r - r[i]
+        d -= L * np.rint(d / L)
+        dist = np.sqrt((d * d).sum(1))
+        assert Ns[i] == ((dist >= rc) & (dist < rs)).sum()
+
+
+def test_momentum_is_conserved_exactly_and_the_batch_is_a_p_subset():
+    L, alpha, rc, rs, p = 24.0, 0.09, 4.0, 8.0, 12
+    a = _cell(500, L, 2)
+    F, Ns, Fc = rbl.rbl_forces(a, L, alpha, rc, rs, p, seed=5, step=7)
+    assert Ns.min() > p                                      # the random branch is exercised for every atom
+    assert np.abs(F.sum(0)).max() <= 1e-12 * np.abs(F).sum()
+    F0, _, _ = rbl.rbl_forces(a, L, alpha, rc, rs, p, seed=5, step=7, correction=False)
+    assert np.allclose(F0 + Fc, F, rtol=0, atol=1e-15) and np.abs(Fc).max() > 0
+    # a different step or seed gives a different batch; the same pair of arguments the same one
+    F1, _, _ = rbl.rbl_forces(a, L, alpha, rc, rs, p, seed=5, step=8)
+    F2, _, _ = rbl.rbl_forces(a, L, alpha, rc, rs, p, seed=5, step=7)
+    assert not np.allclose(F1, F) and np.array_equal(F2, F)
+    # keys: a pure function of (seed, step, i, j), uniform on 32 bits
+    k = rbl.pair_keys(3, np.arange(20000), 5, 7).astype(np.float64) / 2.0 ** 32
+    assert abs(k.mean() - 0.5) < 0.01 and abs(k.var() - 1 / 12) < 0.005
+    assert np.array_equal(rbl.pair_keys(3, [11, 12], 5, 7)[1:], rbl.pair_keys(3, [12], 5, 7))
+    assert rbl.pair_keys(3, [12], 5, 7)[0] != rbl.pair_keys(12, [3], 5, 7)[0]      # (i, j) is ordered
+
+
+def test_unbiased_mean_over_steps_converges_to_the_deterministic_force():
+    """E[F_i^shell*] = F_i^shell: the residual of the mean over T steps falls like 1/sqrt(T)."""
+    L, alpha, rc, rs, p = 18.0, 0.09, 3.0, 7.0, 6
+    a = _cell(150, L, 4)
+    Fd, _ = oracle.short_range(a, L, alpha, rs)
+    acc = np.zeros_like(Fd)
+    res = {}
+    for t in range(1, 257):
+        acc += rbl.rbl_forces(a, L, alpha, rc, rs, p, seed=9, step=t, correction=False)[0]
+        if t in (16, 64, 256):
+            res[t] = np.linalg.norm(acc / t - Fd)
+    assert 1.5 <= res[16] / res[64] <= 2.7 and 1.5 <= res[64] / res[256] <= 2.7, res
+    one = np.linalg.norm(rbl.rbl_forces(a, L, alpha, rc, rs, p, seed=9, step=1, correction=False)[0] - Fd)
+    assert res[256] <= 0.15 * one
