@@ -216,6 +216,20 @@ size_t     rbe_short_range_bytes(const rbe_ctx* ctx, double rs);
 rbe_status rbe_short_range(rbe_ctx* ctx, const void* d_xyzq, double rs, void* d_force, int32_t accumulate,
                            int32_t with_energy, void* d_ws, size_t ws_bytes, void* stream);
 
+/* Random batch list (RBL) estimate of the same short-range force: section 2.3, Eqs. (2.13)-(2.16)
+ * P:145-166, Algorithm 2, with F_ij the electrostatic pair force of Eq. (2.10):
+ *   F_i = sum_{j: r < r_c} F_ij + (N_s / p) sum_{j in B(i)} F_ij + F^corr,  F^corr = -(1/N) sum_i (...)
+ * where N_s counts the shell r_c <= r < r_s of atom i and B(i) holds the min(p, N_s) shell members with
+ * the smallest (u_ij, j), u_ij = first output word of Philox4x32-10 with counter (i, j, step mod 2^32,
+ * step >> 32) and key (seed mod 2^32, seed >> 32), i and j being atom indices: a uniformly random
+ * p-subset, a pure function of (seed, step).  N_s <= p: the whole shell, scale 1.  Forces only
+ * (d_force[i].w = 0, or unchanged with accumulate).  1 <= p <= 32, 0 < rc < rs <= L/3.  d_ws as for
+ * rbe_short_range (rbe_short_range_bytes(ctx, rs)).  Bitwise reproducible.
+ * Errors: RBE_ERR_INVALID_ARG, RBE_ERR_WORKSPACE, RBE_ERR_NO_DEVICE, RBE_ERR_CUDA. */
+rbe_status rbe_rbl_forces(rbe_ctx* ctx, const void* d_xyzq, double rc, double rs, int32_t p, uint64_t seed,
+                          uint64_t step, void* d_force, int32_t accumulate, void* d_ws, size_t ws_bytes,
+                          void* stream);
+
 /* U = (2 pi / V) sum_l w_l |rho(k_l)|^2 / k_l^2 for the current k-set and structure factors,
  * summed in fp64 in a fixed order; written to *h_U (host).  Synchronises `stream`.
  * Errors: RBE_ERR_NOT_READY, RBE_ERR_INVALID_ARG, RBE_ERR_CUDA. */

@@ -12,6 +12,7 @@
 #include "rbe_kernels.cuh"
 #include "sr_kernels.cuh"
 #include "sr_pair_kernels.cuh"
+#include "rbl_kernels.cuh"
 
 #ifdef RBE_SF_PROFILE
 static long long* g_rbe_prof = nullptr;
@@ -660,48 +661,95 @@ size_t rbe_short_range_bytes(const rbe_ctx* c, double rs) {
     return sr_layout(c, rs, l) ? l.bytes : 0;
 }
 
-rbe_status rbe_short_range(rbe_ctx* c, const void* d_xyzq, double rs, void* d_force, int32_t accumulate,
-                           int32_t with_energy, void* d_ws, size_t ws_bytes, void* stream) {
-    if (!c) return RBE_ERR_INVALID_ARG;
-    SrLayout l;
-    if (!sr_layout(c, rs, l)) return fail(c, RBE_ERR_INVALID_ARG, "rbe_short_range: need 0 < r_s <= L/3 (three cells of side >= r_s per dimension) and N < 2^32");
+namespace {
+struct SrBuffers {
+    uint4 *turns, *sorted;
+    int32_t* cell_of;
+    uint32_t *order, *sidx, *count, *cursor, *start;
+    long long* acc;
+    float* gbox;
+};
+// argument checks + the linked-cell list (bin, scan, scatter, sort) shared by rbe_short_range and rbe_rbl_forces
+rbe_status sr_build_cells(rbe_ctx* c, const char* who, const void* d_xyzq, double rs, void* d_force, void* d_ws,
+                          size_t ws_bytes, cudaStream_t st, SrLayout& l, SrBuffers& b) {
+    if (!sr_layout(c, rs, l))
+        return fail(c, RBE_ERR_INVALID_ARG, std::string(who) + ": need 0 < r_s <= L/3 (three cells of side >= r_s per dimension) and N < 2^32");
     rbe_status s0 = init_device(c);
     if (s0 != RBE_OK) return s0;
     if (c->N == 0) return RBE_OK;
     if (!d_xyzq || !d_force || (reinterpret_cast<uintptr_t>(d_xyzq) & 15u) || (reinterpret_cast<uintptr_t>(d_force) & 15u))
-        return fail(c, RBE_ERR_INVALID_ARG, "rbe_short_range: null or misaligned pointer");
+        return fail(c, RBE_ERR_INVALID_ARG, std::string(who) + ": null or misaligned pointer");
     if (!d_ws || ws_bytes < l.bytes || (reinterpret_cast<uintptr_t>(d_ws) & 255u))
-        return fail(c, RBE_ERR_WORKSPACE, "rbe_short_range: d_ws must hold rbe_short_range_bytes bytes, 256-byte aligned");
-    cudaStream_t st = static_cast<cudaStream_t>(stream);
+        return fail(c, RBE_ERR_WORKSPACE, std::string(who) + ": d_ws must hold rbe_short_range_bytes bytes, 256-byte aligned");
     unsigned char* w = static_cast<unsigned char*>(d_ws);
-    uint4* turns = reinterpret_cast<uint4*>(w + l.off_turns);
-    uint4* sorted = reinterpret_cast<uint4*>(w + l.off_sorted);
-    int32_t* cell_of = reinterpret_cast<int32_t*>(w + l.off_cell);
-    uint32_t* order = reinterpret_cast<uint32_t*>(w + l.off_order);
-    uint32_t* sidx = reinterpret_cast<uint32_t*>(w + l.off_sidx);
-    uint32_t* count = reinterpret_cast<uint32_t*>(w + l.off_count);
-    uint32_t* cursor = reinterpret_cast<uint32_t*>(w + l.off_cursor);
-    uint32_t* start = reinterpret_cast<uint32_t*>(w + l.off_start);
+    b.turns = reinterpret_cast<uint4*>(w + l.off_turns);
+    b.sorted = reinterpret_cast<uint4*>(w + l.off_sorted);
+    b.cell_of = reinterpret_cast<int32_t*>(w + l.off_cell);
+    b.order = reinterpret_cast<uint32_t*>(w + l.off_order);
+    b.sidx = reinterpret_cast<uint32_t*>(w + l.off_sidx);
+    b.count = reinterpret_cast<uint32_t*>(w + l.off_count);
+    b.cursor = reinterpret_cast<uint32_t*>(w + l.off_cursor);
+    b.start = reinterpret_cast<uint32_t*>(w + l.off_start);
+    b.acc = reinterpret_cast<long long*>(w + l.off_acc);
+    b.gbox = reinterpret_cast<float*>(w + l.off_gbox);
     const unsigned nb = (unsigned)((c->N + 255) / 256);
-    RBE_CUDA(c, cudaMemsetAsync(count, 0, (size_t)l.ncell * sizeof(uint32_t), st));
-    rbe::sr_bin_kernel<<<nb, 256, 0, st>>>(static_cast<const float4*>(d_xyzq), c->N, rbe::TWO32 / c->L, l.nc, turns, cell_of, count);
-    rbe::sr_scan_kernel<<<1, 1024, 0, st>>>(count, (int)l.ncell, start, cursor);
-    rbe::sr_scatter_kernel<<<nb, 256, 0, st>>>(cell_of, c->N, start, cursor, order);
-    rbe::sr_sort_kernel<<<(unsigned)((l.ncell * 32 + 255) / 256), 256, 0, st>>>(order, start, (int)l.ncell, l.nc, turns, sorted, sidx);
-    long long* acc = reinterpret_cast<long long*>(w + l.off_acc);
-    float* gbox = reinterpret_cast<float*>(w + l.off_gbox);
+    RBE_CUDA(c, cudaMemsetAsync(b.count, 0, (size_t)l.ncell * sizeof(uint32_t), st));
+    rbe::sr_bin_kernel<<<nb, 256, 0, st>>>(static_cast<const float4*>(d_xyzq), c->N, rbe::TWO32 / c->L, l.nc, b.turns, b.cell_of, b.count);
+    rbe::sr_scan_kernel<<<1, 1024, 0, st>>>(b.count, (int)l.ncell, b.start, b.cursor);
+    rbe::sr_scatter_kernel<<<nb, 256, 0, st>>>(b.cell_of, c->N, b.start, b.cursor, b.order);
+    rbe::sr_sort_kernel<<<(unsigned)((l.ncell * 32 + 255) / 256), 256, 0, st>>>(b.order, b.start, (int)l.ncell, l.nc, b.turns, b.sorted, b.sidx);
+    RBE_CUDA(c, cudaGetLastError());
+    return RBE_OK;
+}
+}  // namespace
+
+rbe_status rbe_short_range(rbe_ctx* c, const void* d_xyzq, double rs, void* d_force, int32_t accumulate,
+                           int32_t with_energy, void* d_ws, size_t ws_bytes, void* stream) {
+    if (!c) return RBE_ERR_INVALID_ARG;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    SrLayout l;
+    SrBuffers b;
+    rbe_status s = sr_build_cells(c, "rbe_short_range", d_xyzq, rs, d_force, d_ws, ws_bytes, st, l, b);
+    if (s != RBE_OK || c->N == 0) return s;
+    const unsigned nb = (unsigned)((c->N + 255) / 256);
     const float len_unit = (float)(c->L / rbe::TWO32);
-    RBE_CUDA(c, cudaMemsetAsync(acc, 0, (size_t)c->N * 4 * sizeof(long long), st));
-    rbe::sr_gbox_kernel<<<(unsigned)((l.ncell * 32 + 255) / 256), 256, 0, st>>>(sorted, start, (int)l.ncell, l.nc, len_unit, gbox);
+    RBE_CUDA(c, cudaMemsetAsync(b.acc, 0, (size_t)c->N * 4 * sizeof(long long), st));
+    rbe::sr_gbox_kernel<<<(unsigned)((l.ncell * 32 + 255) / 256), 256, 0, st>>>(b.sorted, b.start, (int)l.ncell, l.nc, len_unit, b.gbox);
     rbe::SrPairParams pp;
-    pp.sorted = sorted; pp.start = start; pp.gbox = gbox; pp.acc = acc;
+    pp.sorted = b.sorted; pp.start = b.start; pp.gbox = b.gbox; pp.acc = b.acc;
     pp.nc = l.nc;
     pp.len_unit = len_unit;
     pp.cell_len = (float)(c->L / l.nc);
     pp.rs2 = (float)(rs * rs);
     pp.sqrt_alpha = (float)std::sqrt(c->alpha);
     rbe::sr_pair_kernel<<<(unsigned)l.ncell, 32 * rbe::SR_PAIR_WARPS, 0, st>>>(pp);
-    rbe::sr_finalize_kernel<<<nb, 256, 0, st>>>(acc, sorted, sidx, c->N, static_cast<float4*>(d_force), accumulate, with_energy);
+    rbe::sr_finalize_kernel<<<nb, 256, 0, st>>>(b.acc, b.sorted, b.sidx, c->N, static_cast<float4*>(d_force), accumulate, with_energy);
+    RBE_CUDA(c, cudaGetLastError());
+    return RBE_OK;
+}
+
+rbe_status rbe_rbl_forces(rbe_ctx* c, const void* d_xyzq, double rc, double rs, int32_t p, uint64_t seed, uint64_t step,
+                          void* d_force, int32_t accumulate, void* d_ws, size_t ws_bytes, void* stream) {
+    if (!c) return RBE_ERR_INVALID_ARG;
+    if (!(rc > 0.0) || !(rc < rs) || p < 1 || p > rbe::RBL_PMAX)
+        return fail(c, RBE_ERR_INVALID_ARG, "rbe_rbl_forces: need 0 < r_c < r_s and 1 <= p <= " + std::to_string(rbe::RBL_PMAX));
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    SrLayout l;
+    SrBuffers b;
+    rbe_status s = sr_build_cells(c, "rbe_rbl_forces", d_xyzq, rs, d_force, d_ws, ws_bytes, st, l, b);
+    if (s != RBE_OK || c->N == 0) return s;
+    RBE_CUDA(c, cudaMemsetAsync(b.acc, 0, 4 * sizeof(long long), st));
+    rbe::RblParams rp;
+    rp.sorted = b.sorted; rp.sidx = b.sidx; rp.start = b.start;
+    rp.force = static_cast<float4*>(d_force);
+    rp.fsum = b.acc;
+    rp.nc = l.nc; rp.p = p; rp.accumulate = accumulate;
+    rp.len_unit = (float)(c->L / rbe::TWO32);
+    rp.rc2 = (float)(rc * rc); rp.rs2 = (float)(rs * rs);
+    rp.sqrt_alpha = (float)std::sqrt(c->alpha);
+    rp.seed = seed; rp.step = step;
+    rbe::rbl_kernel<<<(unsigned)l.ncell, rbe::RBL_THREADS, 0, st>>>(rp);
+    rbe::rbl_correct_kernel<<<(unsigned)((c->N + 255) / 256), 256, 0, st>>>(b.acc, c->N, static_cast<float4*>(d_force));
     RBE_CUDA(c, cudaGetLastError());
     return RBE_OK;
 }

@@ -83,6 +83,8 @@ def lib():
         L.rbe_short_range_bytes.argtypes = [vp, dbl]
         L.rbe_short_range.restype = ctypes.c_int
         L.rbe_short_range.argtypes = [vp, vp, dbl, vp, i32, i32, vp, sz, vp]
+        L.rbe_rbl_forces.restype = ctypes.c_int
+        L.rbe_rbl_forces.argtypes = [vp, vp, dbl, dbl, i32, ctypes.c_uint64, ctypes.c_uint64, vp, i32, vp, sz, vp]
         L.rbe_structure_factor.restype = ctypes.c_int
         L.rbe_structure_factor.argtypes = [vp, vp, vp, vp]
         L.rbe_set_rho.restype = ctypes.c_int
@@ -282,6 +284,20 @@ class Rbe:
         self._check(lib().rbe_short_range(self._h, ctypes.c_void_p(xyzq.data_ptr()), float(rs),
                                           ctypes.c_void_p(force.data_ptr()), int(bool(accumulate)), int(bool(with_energy)),
                                           ctypes.c_void_p(self._sr_ws.data_ptr()), self._sr_ws.numel(), _stream_ptr(stream)))
+
+    def rbe_rbl_forces(self, xyzq, rc: float, rs: float, p: int, seed: int, step: int, force, accumulate: bool = False, stream=None):
+        """Random batch list estimate of the short-range force (Eqs. 2.13-2.16).  xyzq, force: cuda float32 [N,4]."""
+        import torch
+        _check_tensor(xyzq, (self.N, 4), "float32")
+        _check_tensor(force, (self.N, 4), "float32")
+        n = self.rbe_short_range_bytes(rs)
+        if n == 0:
+            raise RbeError(1, "rbe_rbl_forces: need 0 < r_s <= L/3")
+        if getattr(self, "_sr_ws", None) is None or self._sr_ws.numel() < n:
+            self._sr_ws = torch.empty(n, dtype=torch.uint8, device="cuda")
+        self._check(lib().rbe_rbl_forces(self._h, ctypes.c_void_p(xyzq.data_ptr()), float(rc), float(rs), int(p), int(seed),
+                                         int(step), ctypes.c_void_p(force.data_ptr()), int(bool(accumulate)),
+                                         ctypes.c_void_p(self._sr_ws.data_ptr()), self._sr_ws.numel(), _stream_ptr(stream)))
 
     def rbe_kspace_energy(self, stream=None) -> float:
         u = ctypes.c_double(0.0)
