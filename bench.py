@@ -316,10 +316,23 @@ def main():
         e1.record()
         sync()
         ms_sr = e0.elapsed_time(e1) / k_sr
+        # the paper's own estimator of the same force: random batch list, r_c = r_s / 2, p = 30
+        for i in range(2):
+            ctx.rbe_rbl_forces(xs[i % n_rot], args.rs / 2, args.rs, 30, base.seed, i, fs[i % n_rot])
+        sync()
+        e0.record()
+        for i in range(3):
+            ctx.rbe_rbl_forces(xs[i % n_rot], args.rs / 2, args.rs, 30, base.seed, 2 + i, fs[i % n_rot])
+        e1.record()
+        sync()
+        ms_rbl = e0.elapsed_time(e1) / 3
         nbr = 4.0 / 3.0 * np.pi * args.rs ** 3 * n_local / L ** 3          # expected atoms inside the cutoff sphere
         sr = {"ms_per_call": ms_sr, "value": ms_sr * 1e6 / n_local, "unit": UNIT.replace("/step", "/call"),
               "r_s": args.rs, "neighbours_per_atom_expected": nbr, "calls": k_sr, "gpu_launches_per_call": 7,
               "pair_rate_G_per_s": nbr * n_local / (ms_sr * 1e-3) / 1e9,
+              "rbl": {"ms_per_call": ms_rbl, "r_c": args.rs / 2, "p": 30,
+                      "note": "rbe_rbl_forces (Eqs. 2.13-2.16): first implementation, parity-exact batch; slower than "
+                              "the deterministic sum on B200 (DESIGN.md section 11)"},
               "note": "rbe_short_range: bin + scan + scatter + sort + group boxes + pair kernel (every unordered pair "
                       "once, fixed-point integer atomics across warps) + finalise; not part of `value`"}
 
