@@ -53,6 +53,15 @@ def test_config_96k_and_1m_sampled():
         check(atoms, cfg.L, cfg.alpha, 10.0, sel=sel)
 
 
+def test_config_10m_sampled_largest_box():
+    """L = 464 A: the separations come from wrapped fixed-point differences, so the error does not grow with L."""
+    cfg = inputs.CONFIGS["water_10m"]
+    atoms = inputs.make_atoms(cfg)
+    sel = np.sort(np.random.default_rng(8).choice(cfg.N, 150, replace=False)).astype(np.int64)
+    sel[-1] = cfg.N - 1
+    check(atoms, cfg.L, cfg.alpha, 10.0, sel=sel)
+
+
 @pytest.mark.parametrize("N", [1, 2, 33, 129, 1000])
 def test_ragged_sizes_sparse_cells(N):
     cfg = inputs.ions_config(20_000)
