@@ -722,7 +722,8 @@ rbe_status rbe_short_range(rbe_ctx* c, const void* d_xyzq, double rs, void* d_fo
     pp.cell_len = (float)(c->L / l.nc);
     pp.rs2 = (float)(rs * rs);
     pp.sqrt_alpha = (float)std::sqrt(c->alpha);
-    rbe::sr_pair_kernel<<<(unsigned)l.ncell, 32 * rbe::SR_PAIR_WARPS, 0, st>>>(pp);
+    if (with_energy) rbe::sr_pair_kernel<true><<<(unsigned)l.ncell, 32 * rbe::SR_PAIR_WARPS, 0, st>>>(pp);
+    else rbe::sr_pair_kernel<false><<<(unsigned)l.ncell, 32 * rbe::SR_PAIR_WARPS, 0, st>>>(pp);
     rbe::sr_finalize_kernel<<<nb, 256, 0, st>>>(b.acc, b.sorted, b.sidx, c->N, static_cast<float4*>(d_force), accumulate, with_energy);
     RBE_CUDA(c, cudaGetLastError());
     return RBE_OK;

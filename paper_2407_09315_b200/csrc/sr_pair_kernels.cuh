@@ -86,6 +86,7 @@ __constant__ int8_t SR_HALF_STENCIL[14][3] = {
     {0, 0, 0},  {1, 0, 0},  {-1, 1, 0}, {0, 1, 0},  {1, 1, 0},  {-1, -1, 1}, {0, -1, 1},
     {1, -1, 1}, {-1, 0, 1}, {0, 0, 1},  {1, 0, 1},  {-1, 1, 1}, {0, 1, 1},   {1, 1, 1}};
 
+template <bool ENERGY>
 __global__ void __launch_bounds__(32 * SR_PAIR_WARPS, RBE_SR_PAIR_CTAS) sr_pair_kernel(const SrPairParams p) {
     __shared__ float4 vpos[SR_PAIR_WARPS][32];   // the visiting group: positions relative to THIS cell's centre, charge
     __shared__ float4 vacc[SR_PAIR_WARPS][32];   // ... and what this warp adds to its atoms
@@ -150,12 +151,12 @@ __global__ void __launch_bounds__(32 * SR_PAIR_WARPS, RBE_SR_PAIR_CTAS) sr_pair_
                         const float u = ec * inv_r;
                         const float sj = o.w * s;
                         fx = fmaf(sj, dx, fx); fy = fmaf(sj, dy, fy); fz = fmaf(sj, dz, fz);
-                        en = fmaf(o.w, u, en);
+                        if (ENERGY) en = fmaf(o.w, u, en);
                         if (!self_block) {                          // the same pair term, seen from the visitor (d -> -d)
                             const float si = me.w * s;
                             float4 a = vacc[w][v];
                             a.x = fmaf(-si, dx, a.x); a.y = fmaf(-si, dy, a.y); a.z = fmaf(-si, dz, a.z);
-                            a.w = fmaf(me.w, u, a.w);
+                            if (ENERGY) a.w = fmaf(me.w, u, a.w);
                             vacc[w][v] = a;
                         }
                     }
@@ -167,7 +168,7 @@ __global__ void __launch_bounds__(32 * SR_PAIR_WARPS, RBE_SR_PAIR_CTAS) sr_pair_
                     if (a.x != 0.f) sr_atomic_add_fixed(dst + 0, a.x);
                     if (a.y != 0.f) sr_atomic_add_fixed(dst + 1, a.y);
                     if (a.z != 0.f) sr_atomic_add_fixed(dst + 2, a.z);
-                    if (a.w != 0.f) sr_atomic_add_fixed(dst + 3, a.w);
+                    if (ENERGY && a.w != 0.f) sr_atomic_add_fixed(dst + 3, a.w);
                 }
             }
         }
@@ -176,7 +177,7 @@ __global__ void __launch_bounds__(32 * SR_PAIR_WARPS, RBE_SR_PAIR_CTAS) sr_pair_
             sr_atomic_add_fixed(dst + 0, fx);
             sr_atomic_add_fixed(dst + 1, fy);
             sr_atomic_add_fixed(dst + 2, fz);
-            sr_atomic_add_fixed(dst + 3, en);
+            if (ENERGY) sr_atomic_add_fixed(dst + 3, en);
         }
     }
 }
