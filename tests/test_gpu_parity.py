@@ -360,3 +360,21 @@ def test_kspace_virial_matches_oracle(name, weighted):
     W_o = virial.kspace_virial(L, alpha, m, S, oracle.rho(atoms, L, m), w=w)
     assert np.abs(W - W_o).max() <= U_TOL * np.abs(W_o).max()
     assert np.array_equal(W, ctx.rbe_kspace_virial())          # fixed order: bitwise reproducible
+
+
+def test_deterministic_ewald_mode_with_a_large_k_grid():
+    """SURVEY.md s8(f) row 4, deterministic mode at scale: every grid vector with |m_d| <= 12 (P = 15 624:
+    several k-chunks in both kernels) with weights exp(-k^2/4alpha) on BASELINE config 1 reproduces the
+    full long-range force and energy of Eqs. (2.11) / (2.8), computed by oracle.ewald_full."""
+    cfg = inputs.CONFIGS["water_3k"]
+    atoms = inputs.make_atoms(cfg)
+    mmax = 12                                             # exp(-k^2/4alpha) < 3e-8 beyond it at L = 31 A
+    m = inputs.full_kgrid(mmax)
+    k2 = (2 * np.pi / cfg.L) ** 2 * (m.astype(np.float64) ** 2).sum(1)
+    w = np.exp(-k2 / (4 * cfg.alpha))
+    ctx, rho, F, U = gpu_step(atoms, cfg.L, cfg.alpha, m, w=w, with_energy=True)
+    Uref, _, Fl = oracle.ewald_full(atoms[:, :3].astype(np.float64), atoms[:, 3].astype(np.float64),
+                                    cfg.L, cfg.alpha, nreal=0, mmax=mmax)
+    assert np.linalg.norm(F[:, :3] - Fl) / np.linalg.norm(Fl) <= F_TOL
+    assert abs(U - Uref[1]) <= U_TOL * abs(Uref[1])
+    assert abs(F[:, 3].astype(np.float64).sum() - Uref[1]) <= 1e-4 * abs(Uref[1])
