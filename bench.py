@@ -353,17 +353,26 @@ def main():
         hx_np[:] = atoms
         hx, hf = torch.from_numpy(hx_np), torch.from_numpy(hf_np)
         k_e2e = max(3, min(args.steps, 20))
+        ms_e2e4 = None
         if world == 1:
-            for i in range(3):
-                ctx.rbe_step_host(hx, ksets[i % n_k], hf, with_energy=args.with_energy)
-            sync()
-            t0 = time.perf_counter()
-            e0.record()
-            for i in range(k_e2e):
-                ctx.rbe_step_host(hx, ksets[i % n_k], hf, with_energy=args.with_energy)
-            e1.record()
-            sync()
-            ms_e2e = e0.elapsed_time(e1) / k_e2e
+            def time_host(fn):
+                for i in range(3):
+                    fn(i)
+                sync()
+                e0.record()
+                for i in range(k_e2e):
+                    fn(i)
+                e1.record()
+                sync()
+                return e0.elapsed_time(e1) / k_e2e
+            # float4 {x,y,z,q} in / float4 {F,e} out: 32 B per atom over PCIe
+            ms_e2e4 = time_host(lambda i: ctx.rbe_step_host(hx, ksets[i % n_k], hf, with_energy=args.with_energy))
+            # the MD-loop form: charges resident on the device, positions in / force vectors out: 24 B per atom
+            hx3_np = rbe.rbe_host_alloc((n_local, 3), np.float32)
+            hf3_np = rbe.rbe_host_alloc((n_local, 3), np.float32)
+            hx3_np[:] = atoms[:, :3]
+            ctx.rbe_set_charges(torch.from_numpy(atoms[:, 3].copy()).cuda())
+            ms_e2e = time_host(lambda i: ctx.rbe_step_host_xyz(hx3_np, ksets[i % n_k], hf3_np))
         else:
             dx = torch.empty((n_local, 4), dtype=torch.float32, device="cuda")
             df = torch.empty((n_local, 4), dtype=torch.float32, device="cuda")
@@ -389,11 +398,14 @@ def main():
             t = torch.tensor([e0.elapsed_time(e1) / k_e2e], dtype=torch.float64, device="cuda")
             dist.all_reduce(t, op=dist.ReduceOp.MAX)
             ms_e2e = float(t.cpu()[0])
+        compact = world == 1
         e2e = {"value": ms_e2e * 1e6 / n_total, "unit": UNIT, "ms_per_step": ms_e2e, "steps": k_e2e,
-               "h2d_bytes_per_step": 16 * n_local + 16 * P, "d2h_bytes_per_step": 16 * n_local,
-               "path": "rbe_step_host: pinned host float4[N] in -> forces float4[N] out, "
-                       "copies chunked (<= 4) and overlapped with the kernels" if world == 1 else
-                       "H2D + rbe_* calls + all_gather + D2H per rank"}
+               "h2d_bytes_per_step": (12 if compact else 16) * n_local + 16 * P,
+               "d2h_bytes_per_step": (12 if compact else 16) * n_local,
+               "path": "rbe_step_host_xyz: pinned host positions float3[N] in -> forces float3[N] out (charges resident on "
+                       "the device), copies chunked (<= 4) and overlapped with the kernels" if compact else
+                       "H2D + rbe_* calls + exchange + D2H per rank",
+               "float4_ms_per_step": ms_e2e4}
 
     if rank != 0:
         if world > 1:

@@ -256,6 +256,19 @@ rbe_status rbe_step_host(rbe_ctx* ctx, const float* h_xyzq, const int32_t* h_m, 
                          float* h_force, int32_t with_energy, double* h_U, void* d_scratch,
                          size_t scratch_bytes, void* stream);
 
+/* Compact end-to-end step for MD loops, where the charges never change: only POSITIONS travel to the
+ * device (h_xyz float [N][3]) and only force vectors travel back (h_force3 float [N][3]): 24 B per
+ * atom over PCIe instead of 32.  The charges live on the device: rbe_set_charges(ctx, d_q) registers a
+ * caller-owned device array float [N] (retained until replaced; NULL unregisters).  Same chunked
+ * pipeline and the same two hot kernels as rbe_step_host, plus a pack and an unpack kernel per chunk;
+ * the forces are bitwise those of rbe_step_host.  d_scratch: at least 56 * N + 1024 bytes, 256-byte
+ * aligned.  Per-atom energies are not returned; h_U (optional) receives the k-space energy.
+ * Synchronises `stream`.  Errors: as rbe_step_host, plus RBE_ERR_NOT_READY without rbe_set_charges. */
+rbe_status rbe_set_charges(rbe_ctx* ctx, const void* d_q);
+rbe_status rbe_step_host_xyz(rbe_ctx* ctx, const float* h_xyz, const int32_t* h_m, const double* h_w,
+                             float* h_force3, double* h_U, void* d_scratch, size_t scratch_bytes,
+                             void* stream);
+
 /* Page-locked (pinned) HOST memory for the end-to-end path: cudaHostAlloc'ed, so that the copies of
  * rbe_step_host are asynchronous DMA transfers at full PCIe rate (measured on B200 hosts: 55 GB/s
  * from such a buffer, 15-40 GB/s and erratic from memory pinned after allocation).  The caller

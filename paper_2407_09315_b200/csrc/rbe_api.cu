@@ -78,6 +78,8 @@ struct rbe_ctx {
     unsigned char* xch_buf[rbe::MAX_WORLD] = {};
     size_t off_xch_err = 0;
 
+    const float* d_q = nullptr;   // charges on the device (rbe_set_charges), for the compact host step
+
     std::string err;
 };
 
@@ -767,18 +769,41 @@ rbe_status rbe_kspace_virial(rbe_ctx* c, double* h_W, void* stream) {
     return RBE_OK;
 }
 
-rbe_status rbe_step_host(rbe_ctx* c, const float* h_xyzq, const int32_t* h_m, const double* h_w, float* h_force,
-                         int32_t with_energy, double* h_U, void* d_scratch, size_t scratch_bytes, void* stream) {
+namespace {
+// The end-to-end step from host buffers.  compact = false: float4 {x,y,z,q} in, float4 {F, e} out.
+// compact = true: float3 positions in, float3 forces out, charges from rbe_set_charges; a pack and an
+// unpack kernel sit between the copies and the two hot kernels.
+rbe_status step_host_impl(rbe_ctx* c, const float* h_in, const int32_t* h_m, const double* h_w, float* h_out,
+                          int32_t with_energy, double* h_U, void* d_scratch, size_t scratch_bytes, void* stream, bool compact) {
     if (!c) return RBE_ERR_INVALID_ARG;
-    if ((c->N > 0 && (!h_xyzq || !h_force)) || !h_m) return fail(c, RBE_ERR_INVALID_ARG, "rbe_step_host: null argument");
-    const size_t nb = (size_t)c->N * sizeof(float4);
-    if (c->N > 0 && (!d_scratch || scratch_bytes < align_up(nb, 256) + nb || (reinterpret_cast<uintptr_t>(d_scratch) & 255u)))
-        return fail(c, RBE_ERR_WORKSPACE, "rbe_step_host: d_scratch must hold 32*N (+256) bytes, 256-byte aligned");
+    if ((c->N > 0 && (!h_in || !h_out)) || !h_m) return fail(c, RBE_ERR_INVALID_ARG, "rbe_step_host: null argument");
+    if (compact && c->N > 0 && !c->d_q) return fail(c, RBE_ERR_NOT_READY, "rbe_step_host_xyz needs rbe_set_charges");
+    const size_t nb = (size_t)c->N * sizeof(float4), nb3 = (size_t)c->N * 3 * sizeof(float);
+    const size_t need = align_up(nb, 256) + align_up(nb, 256) + (compact ? align_up(nb3, 256) + nb3 : 0);
+    if (c->N > 0 && (!d_scratch || scratch_bytes < need || (reinterpret_cast<uintptr_t>(d_scratch) & 255u)))
+        return fail(c, RBE_ERR_WORKSPACE, compact ? "rbe_step_host_xyz: d_scratch must hold 56*N (+1024) bytes, 256-byte aligned"
+                                                  : "rbe_step_host: d_scratch must hold 32*N (+512) bytes, 256-byte aligned");
     cudaStream_t st = static_cast<cudaStream_t>(stream);
-    float4* d_x = static_cast<float4*>(d_scratch);
-    float4* d_f = reinterpret_cast<float4*>(static_cast<unsigned char*>(d_scratch) + align_up(nb, 256));
-    const float4* h_x = reinterpret_cast<const float4*>(h_xyzq);
-    float4* h_f = reinterpret_cast<float4*>(h_force);
+    unsigned char* base = static_cast<unsigned char*>(d_scratch);
+    float4* d_x = reinterpret_cast<float4*>(base);
+    float4* d_f = reinterpret_cast<float4*>(base + align_up(nb, 256));
+    float* d_x3 = reinterpret_cast<float*>(base + 2 * align_up(nb, 256));
+    float* d_f3 = reinterpret_cast<float*>(base + 2 * align_up(nb, 256) + align_up(nb3, 256));
+    // bytes per atom on the wire and the two copy helpers (a chunk [lo, lo + n) of atoms)
+    auto copy_in = [&](int64_t lo, int64_t n, cudaStream_t s_) -> cudaError_t {
+        return compact ? cudaMemcpyAsync(d_x3 + 3 * lo, h_in + 3 * lo, (size_t)n * 3 * sizeof(float), cudaMemcpyHostToDevice, s_)
+                       : cudaMemcpyAsync(d_x + lo, reinterpret_cast<const float4*>(h_in) + lo, (size_t)n * sizeof(float4), cudaMemcpyHostToDevice, s_);
+    };
+    auto copy_out = [&](int64_t lo, int64_t n, cudaStream_t s_) -> cudaError_t {
+        return compact ? cudaMemcpyAsync(h_out + 3 * lo, d_f3 + 3 * lo, (size_t)n * 3 * sizeof(float), cudaMemcpyDeviceToHost, s_)
+                       : cudaMemcpyAsync(reinterpret_cast<float4*>(h_out) + lo, d_f + lo, (size_t)n * sizeof(float4), cudaMemcpyDeviceToHost, s_);
+    };
+    auto pack = [&](int64_t lo, int64_t n) {      // on st, after the chunk has arrived
+        if (compact && n > 0) rbe::pack_xyzq_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(d_x3 + 3 * lo, c->d_q + lo, n, d_x + lo);
+    };
+    auto unpack = [&](int64_t lo, int64_t n) {    // on st, after the chunk's forces
+        if (compact && n > 0) rbe::unpack_force_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(d_f + lo, n, d_f3 + 3 * lo);
+    };
     rbe_status s = rbe_set_kvectors(c, h_m, h_w, stream);
     if (s != RBE_OK) return s;
 
@@ -818,21 +843,24 @@ rbe_status rbe_step_host(rbe_ctx* c, const float* h_xyzq, const int32_t* h_m, co
         }
     }
     if (nchunk == 1) {
-        if (c->N > 0) RBE_CUDA(c, cudaMemcpyAsync(d_x, h_x, nb, cudaMemcpyHostToDevice, st));
+        if (c->N > 0) RBE_CUDA(c, copy_in(0, c->N, st));
+        pack(0, c->N);
         s = rbe_structure_factor(c, d_x, nullptr, stream);
         if (s != RBE_OK) return s;
         s = rbe_forces(c, d_x, d_f, with_energy, stream);
         if (s != RBE_OK) return s;
-        if (c->N > 0) RBE_CUDA(c, cudaMemcpyAsync(h_f, d_f, nb, cudaMemcpyDeviceToHost, st));
+        unpack(0, c->N);
+        if (c->N > 0) RBE_CUDA(c, copy_out(0, c->N, st));
     } else {
         RBE_CUDA(c, cudaEventRecord(c->ev_start, st));          // the copies start after the caller's earlier work
         RBE_CUDA(c, cudaStreamWaitEvent(c->s_h2d, c->ev_start, 0));
         RBE_CUDA(c, cudaStreamWaitEvent(c->s_d2h, c->ev_start, 0));
         for (int64_t i = 0; i < nchunk; ++i) {
             const int64_t lo = in_lo[i], n = in_lo[i + 1] - lo;
-            RBE_CUDA(c, cudaMemcpyAsync(d_x + lo, h_x + lo, (size_t)n * sizeof(float4), cudaMemcpyHostToDevice, c->s_h2d));
+            RBE_CUDA(c, copy_in(lo, n, c->s_h2d));
             RBE_CUDA(c, cudaEventRecord(c->ev_in[i], c->s_h2d));
             RBE_CUDA(c, cudaStreamWaitEvent(st, c->ev_in[i], 0));
+            pack(lo, n);
             s = launch_sf(c, d_x + lo, n, i > 0, i == nchunk - 1, nullptr, st);
             if (s != RBE_OK) return s;
         }
@@ -841,9 +869,10 @@ rbe_status rbe_step_host(rbe_ctx* c, const float* h_xyzq, const int32_t* h_m, co
             const int64_t lo = out_lo[i], n = out_lo[i + 1] - lo;
             s = launch_f(c, d_x + lo, d_f + lo, n, with_energy, st);
             if (s != RBE_OK) return s;
+            unpack(lo, n);
             RBE_CUDA(c, cudaEventRecord(c->ev_f[i], st));
             RBE_CUDA(c, cudaStreamWaitEvent(c->s_d2h, c->ev_f[i], 0));
-            RBE_CUDA(c, cudaMemcpyAsync(h_f + lo, d_f + lo, (size_t)n * sizeof(float4), cudaMemcpyDeviceToHost, c->s_d2h));
+            RBE_CUDA(c, copy_out(lo, n, c->s_d2h));
         }
         RBE_CUDA(c, cudaEventRecord(c->ev_done, c->s_d2h));
         RBE_CUDA(c, cudaStreamWaitEvent(st, c->ev_done, 0));
@@ -851,6 +880,24 @@ rbe_status rbe_step_host(rbe_ctx* c, const float* h_xyzq, const int32_t* h_m, co
     if (h_U) return rbe_kspace_energy(c, h_U, stream);
     RBE_CUDA(c, cudaStreamSynchronize(st));
     return RBE_OK;
+}
+}  // namespace
+
+rbe_status rbe_step_host(rbe_ctx* c, const float* h_xyzq, const int32_t* h_m, const double* h_w, float* h_force,
+                         int32_t with_energy, double* h_U, void* d_scratch, size_t scratch_bytes, void* stream) {
+    return step_host_impl(c, h_xyzq, h_m, h_w, h_force, with_energy, h_U, d_scratch, scratch_bytes, stream, false);
+}
+
+rbe_status rbe_set_charges(rbe_ctx* c, const void* d_q) {
+    if (!c) return RBE_ERR_INVALID_ARG;
+    if (d_q && (reinterpret_cast<uintptr_t>(d_q) & 3u)) return fail(c, RBE_ERR_INVALID_ARG, "rbe_set_charges: misaligned pointer");
+    c->d_q = static_cast<const float*>(d_q);
+    return RBE_OK;
+}
+
+rbe_status rbe_step_host_xyz(rbe_ctx* c, const float* h_xyz, const int32_t* h_m, const double* h_w, float* h_force3,
+                             double* h_U, void* d_scratch, size_t scratch_bytes, void* stream) {
+    return step_host_impl(c, h_xyz, h_m, h_w, h_force3, 0, h_U, d_scratch, scratch_bytes, stream, true);
 }
 
 rbe_status rbe_host_alloc(void** out, size_t bytes) {

@@ -788,4 +788,21 @@ __global__ void __launch_bounds__(1024) sample_kernel(const SampleParams p) {
     if (p.state && tid == 0) p.state[1] = step + 1;
 }
 
+// ---------------------------------------------------------------------------------------
+// Compact host step (rbe_step_host_xyz): only positions travel to the device and only force
+// vectors travel back (12 B per atom each way instead of 16); the charges stay on the device.
+// ---------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) pack_xyzq_kernel(const float* __restrict__ xyz, const float* __restrict__ q, int64_t n,
+                                                         float4* __restrict__ xyzq) {
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) xyzq[i] = make_float4(xyz[3 * i], xyz[3 * i + 1], xyz[3 * i + 2], q[i]);
+}
+__global__ void __launch_bounds__(256) unpack_force_kernel(const float4* __restrict__ f4, int64_t n, float* __restrict__ f3) {
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) {
+        const float4 f = f4[i];
+        f3[3 * i] = f.x; f3[3 * i + 1] = f.y; f3[3 * i + 2] = f.z;
+    }
+}
+
 }  // namespace rbe

@@ -95,6 +95,10 @@ def lib():
         L.rbe_kspace_energy.argtypes = [vp, ctypes.POINTER(dbl), vp]
         L.rbe_kspace_virial.restype = ctypes.c_int
         L.rbe_kspace_virial.argtypes = [vp, vp, vp]
+        L.rbe_set_charges.restype = ctypes.c_int
+        L.rbe_set_charges.argtypes = [vp, vp]
+        L.rbe_step_host_xyz.restype = ctypes.c_int
+        L.rbe_step_host_xyz.argtypes = [vp, vp, vp, vp, vp, ctypes.POINTER(dbl), vp, sz, vp]
         L.rbe_step_host.restype = ctypes.c_int
         L.rbe_step_host.argtypes = [vp, vp, vp, vp, vp, i32, ctypes.POINTER(dbl), vp, sz, vp]
         L.rbe_host_alloc.restype = ctypes.c_int
@@ -311,6 +315,32 @@ class Rbe:
         self._check(lib().rbe_kspace_virial(self._h, _np_ptr(W), _stream_ptr(stream)))
         return W
 
+    def rbe_set_charges(self, q):
+        """q: cuda float32 [N] (kept alive by this object) or None."""
+        if q is None:
+            self._check(lib().rbe_set_charges(self._h, None))
+        else:
+            _check_tensor(q, (self.N,), "float32")
+            self._check(lib().rbe_set_charges(self._h, ctypes.c_void_p(q.data_ptr())))
+        self._q = q
+
+    def rbe_step_host_xyz(self, h_xyz, m, h_force3, w=None, want_energy=False, stream=None):
+        """Compact end-to-end step: h_xyz / h_force3 are host float32 [N,3] (numpy or CPU torch)."""
+        import numpy as np
+        import torch
+        need = 56 * self.N + 1024
+        if getattr(self, "_scratch3", None) is None or self._scratch3.numel() < need:
+            self._scratch3 = torch.empty(max(1, need), dtype=torch.uint8, device="cuda")
+        mm = np.ascontiguousarray(m, dtype=np.int32)
+        assert mm.shape == (self.P, 3)
+        ww = None if w is None else np.ascontiguousarray(w, dtype=np.float64)
+        u = ctypes.c_double(0.0)
+        self._check(lib().rbe_step_host_xyz(
+            self._h, ctypes.c_void_p(_host_ptr3(h_xyz, self.N)), _np_ptr(mm), _np_ptr(ww),
+            ctypes.c_void_p(_host_ptr3(h_force3, self.N)), ctypes.byref(u) if want_energy else None,
+            ctypes.c_void_p(self._scratch3.data_ptr()), self._scratch3.numel(), _stream_ptr(stream)))
+        return float(u.value) if want_energy else None
+
     def rbe_step_host(self, h_xyzq, m, h_force, w=None, with_energy=False, want_energy=False, stream=None):
         """End-to-end step from HOST buffers: h_xyzq / h_force are CPU float32 [N,4] torch tensors
         (pinned for asynchronous copies) or numpy arrays; m numpy int32 [P,3]."""
@@ -328,6 +358,15 @@ class Rbe:
             ctypes.byref(u) if want_energy else None,
             ctypes.c_void_p(self._scratch.data_ptr()), self._scratch.numel(), _stream_ptr(stream)))
         return float(u.value) if want_energy else None
+
+
+def _host_ptr3(a, N):
+    import numpy as np
+    if isinstance(a, np.ndarray):
+        assert a.dtype == np.float32 and a.flags["C_CONTIGUOUS"] and a.shape == (N, 3)
+        return a.ctypes.data
+    assert (not a.is_cuda) and a.is_contiguous() and tuple(a.shape) == (N, 3)
+    return a.data_ptr()
 
 
 def _check_tensor(t, shape, dtype):

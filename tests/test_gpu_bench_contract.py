@@ -29,7 +29,8 @@ def test_bench_json_line_contract():
     c = d["cpu_baseline"]
     assert c["kind"] == "oracle" and c["cores"] >= 1 and c["value"] > d["value"] and "sample" in c
     e = d["e2e"]
-    assert e["value"] > d["value"] and e["h2d_bytes_per_step"] >= 16 * 96000 and e["d2h_bytes_per_step"] == 16 * 96000
+    assert e["value"] > d["value"] and e["h2d_bytes_per_step"] >= 12 * 96000 and e["d2h_bytes_per_step"] == 12 * 96000
+    assert e["float4_ms_per_step"] > 0
     assert d["gpu_launches"] == 2 * 5
     assert set(d["clocks"]) >= {"sm_mhz", "sm_max_mhz", "reasons"}
     assert d["graph_step"]["gpu_launches_per_step"] == 1 and d["short_range"]["ms_per_call"] > 0

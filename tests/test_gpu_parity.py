@@ -378,3 +378,25 @@ def test_deterministic_ewald_mode_with_a_large_k_grid():
     assert np.linalg.norm(F[:, :3] - Fl) / np.linalg.norm(Fl) <= F_TOL
     assert abs(U - Uref[1]) <= U_TOL * abs(Uref[1])
     assert abs(F[:, 3].astype(np.float64).sum() - Uref[1]) <= 1e-4 * abs(Uref[1])
+
+
+@pytest.mark.parametrize("N", [3000, 300_000])
+def test_compact_host_step_matches_the_float4_host_step(N):
+    """rbe_step_host_xyz (positions in, force vectors out, charges resident on the device) runs the same
+    kernels over the same chunks as rbe_step_host: bitwise the same forces and energy."""
+    cfg = inputs.ions_config(300_000)
+    atoms = inputs.make_atoms(cfg)[:N].copy()
+    m = inputs.sample_kset(cfg.L, cfg.alpha, 64, 41)
+    ctx = rbe.Rbe(N, cfg.L, cfg.alpha, 64)
+    h_x, h_f = rbe.rbe_host_alloc((N, 4)), rbe.rbe_host_alloc((N, 4))
+    h_x[:] = atoms
+    U4 = ctx.rbe_step_host(h_x, m, h_f, want_energy=True)
+    h_x3, h_f3 = rbe.rbe_host_alloc((N, 3)), rbe.rbe_host_alloc((N, 3))
+    h_x3[:] = atoms[:, :3]
+    h_f3[:] = np.nan
+    with pytest.raises(rbe.RbeError) as e:
+        ctx.rbe_step_host_xyz(h_x3, m, h_f3)
+    assert e.value.status == 3                                   # charges not registered yet
+    ctx.rbe_set_charges(torch.from_numpy(atoms[:, 3].copy()).cuda())
+    U3 = ctx.rbe_step_host_xyz(h_x3, m, h_f3, want_energy=True)
+    assert np.array_equal(h_f3, h_f[:, :3]) and U3 == U4
