@@ -38,7 +38,10 @@ namespace rbe {
 #ifndef RBE_F_CTAS_PER_SM
 #define RBE_F_CTAS_PER_SM 2
 #endif
-constexpr int SF_KPT = 4;        // wavevectors owned by one thread of the structure-factor kernel
+#ifndef RBE_SF_KPT
+#define RBE_SF_KPT 4
+#endif
+constexpr int SF_KPT = RBE_SF_KPT;   // wavevectors owned by one thread of the structure-factor kernel
 constexpr int SF_TMAX = RBE_SF_TMAX;    // max threads per CTA (structure-factor kernel): <= 64 registers
 constexpr int SF_CTAS_PER_SM = RBE_SF_CTAS_PER_SM;
 constexpr int SF_TILE_MAX = RBE_SF_TILE_MAX; // max atoms staged in shared memory at a time (structure-factor kernel)
