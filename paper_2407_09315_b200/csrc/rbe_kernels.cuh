@@ -45,6 +45,10 @@ constexpr int SF_KPT = RBE_SF_KPT;   // wavevectors owned by one thread of the s
 constexpr int SF_TMAX = RBE_SF_TMAX;    // max threads per CTA (structure-factor kernel): <= 64 registers
 constexpr int SF_CTAS_PER_SM = RBE_SF_CTAS_PER_SM;
 constexpr int SF_TILE_MAX = RBE_SF_TILE_MAX; // max atoms staged in shared memory at a time (structure-factor kernel)
+#ifndef RBE_SF_STAGE_UNROLL
+#define RBE_SF_STAGE_UNROLL 4
+#endif
+constexpr int SF_STAGE_UNROLL = RBE_SF_STAGE_UNROLL;   // unroll factor of the two staging loops over 32-atom windows
 constexpr int SF_DEPTH = 64;     // max atoms a thread accumulates in fp32 before the fp64 flush
 constexpr int F_THREADS = RBE_F_THREADS;   // threads per CTA (force kernel)
 constexpr int F_CTAS_PER_SM = RBE_F_CTAS_PER_SM;
@@ -432,6 +436,7 @@ __global__ void __launch_bounds__(SF_TMAX, SF_CTAS_PER_SM) sf_kernel(const SfPar
         RBE_STAMP();
 
         // ---- stage 1: per window (one warp each), classify by charge and count the records
+#pragma unroll SF_STAGE_UNROLL
         for (int w = warp; w < nwin; w += nwarps) {
             const int idx = (w << 5) + lane;
             const uint32_t qb = idx < cnt ? __float_as_uint(raw[idx].w) : 0u;
@@ -463,6 +468,7 @@ __global__ void __launch_bounds__(SF_TMAX, SF_CTAS_PER_SM) sf_kernel(const SfPar
         const int np = (int)(total & 0xffffu), ns = (int)(total >> 16);
 
         // ---- stage 2: convert to turns and write the records at their scanned positions
+#pragma unroll SF_STAGE_UNROLL
         for (int w = warp; w < nwin; w += nwarps) {
             const int idx = (w << 5) + lane;
             const uint32_t base = wbase[w];
