@@ -54,7 +54,10 @@ constexpr int F_THREADS = RBE_F_THREADS;   // threads per CTA (force kernel)
 constexpr int F_CTAS_PER_SM = RBE_F_CTAS_PER_SM;
 constexpr int F_RMAX = 4;        // max atoms per thread per pass (force kernel)
 constexpr int F_KCHUNK = 2048;   // wavevectors staged in shared memory at a time (force kernel)
-constexpr int SF_RED_GROUP = 16; // CTAs per group in the two-level reduction of the per-CTA rows
+#ifndef RBE_SF_RED_GROUP
+#define RBE_SF_RED_GROUP 16
+#endif
+constexpr int SF_RED_GROUP = RBE_SF_RED_GROUP; // CTAs per group in the two-level reduction of the per-CTA rows
 
 constexpr double TWO32 = 4294967296.0;
 constexpr double MAGIC = 6755399441055744.0;  // 2^52 + 2^51: low word of (d + MAGIC) = rint(d) mod 2^32
