@@ -201,9 +201,10 @@ rbe_status rbe_forces(rbe_ctx* ctx, const void* d_xyzq, void* d_force, int32_t w
  *   e_i = 1/2 q_i sum_{j != i, r < r_s} q_j erfc(sqrt(alpha) r) / r      (first term of Eq. 2.8)
  * with this context's L and alpha.  Coincident atoms (r = 0) are skipped.  Independent of the
  * k-set; needs no rbe_set_workspace.  fp32 arithmetic on cell-relative coordinates derived from exact
- * fixed-point separations; erfc by Abramowitz-Stegun 7.1.26 (|error| <= 1.5e-7).  Every unordered pair
+ * fixed-point separations; erfc by a degree-8 polynomial fit with 3.4e-7 RELATIVE error for x <= 10.  Every unordered pair
  * is evaluated once (Newton's third law); partial sums of different warps are combined in 64-bit
- * fixed point with integer atomics (scale 2^36: |F_i / q_i| must stay below 1.3e8 e/A^2), so the result
+ * fixed point with integer atomics (scale 2^40: |F_i / q_i| must stay below 8.4e6 e/A^2, and partial sums
+ * below 9e-13 e/A^2 are lost), so the result
  * is bitwise reproducible.
  *   d_xyzq      float4 [N] device;  rs  cutoff radius [A], 0 < rs <= L/3
  *   d_force     float4 [N] device: {F_x, F_y, F_z, e_i}; e_i = 0 unless with_energy != 0

@@ -18,7 +18,8 @@
 // Combining contributions that come from different warps.  A group receives partial forces from
 // ~20 other warps.  They are added in 64-bit FIXED POINT with integer atomics: integer addition is
 // associative, so the sum does not depend on the order in which the warps arrive -- no
-// floating-point atomics anywhere.  Scale 2^36 per e^2/A^2 (resolution 1.5e-11, range +-1.3e8).
+// floating-point atomics anywhere.  Scale 2^40 per e/A^2 of F_i / q_i (resolution 9e-13, range +-8.4e6:
+// two unit charges closer than 3.5e-4 A would overflow; contributions below the resolution are lost).
 // sr_finalize_kernel converts back to fp32, applies -q_i and scatters to the caller's atom order.
 #pragma once
 #include "sr_kernels.cuh"
@@ -26,7 +27,7 @@
 namespace rbe {
 
 constexpr int SR_GMAX = 8;                       // groups per cell that carry a bounding box (more: never skipped)
-constexpr double SR_FIXED_SCALE = 68719476736.0; // 2^36
+constexpr double SR_FIXED_SCALE = 1099511627776.0; // 2^40
 
 struct SrPairParams {
     const uint4* sorted;      // [N] {Sx, Sy, Sz, q} in cell order

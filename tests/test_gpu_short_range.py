@@ -87,6 +87,23 @@ def test_crowded_cell_more_atoms_than_threads_and_far_outside_box():
     check(atoms, L, alpha, rs)
 
 
+def test_sparse_system_where_every_pair_is_far():
+    """Found by a randomised sweep: when all neighbours sit at sqrt(alpha) r = 1.5 ... 4, erfc is 1e-2 ... 1e-8
+    and an erfc approximation that is only ABSOLUTELY accurate (Abramowitz-Stegun 7.1.26, 1.5e-7) fails
+    the relative bar; the kernel's fit is relatively accurate (csrc/fit_erfcx.py)."""
+    L, alpha, rs, n = 100.0, 0.1, 30.0, 400
+    rng = np.random.default_rng(12)
+    atoms = np.empty((n, 4), dtype=np.float32)
+    atoms[:, :3] = rng.random((n, 3)) * L
+    atoms[:, 3] = rng.choice(np.array([-0.8476, 0.4238, 0.4238], dtype=np.float32), n)
+    r = atoms[:, :3].astype(np.float64)
+    d = r[:, None, :] - r[None, :, :]
+    d -= L * np.rint(d / L)
+    dist = np.sqrt((d ** 2).sum(-1)) + np.eye(n) * 1e9
+    assert np.sqrt(alpha) * dist.min() > 0.3 and np.median(np.sqrt(alpha) * dist.min(1)) > 1.5     # the regime
+    check(atoms, L, alpha, rs)
+
+
 def test_accumulate_bitwise_reproducible_and_argument_checks():
     cfg = inputs.CONFIGS["water_3k"]
     atoms = inputs.make_atoms(cfg)
