@@ -204,8 +204,11 @@ rbe_status init_device(rbe_ctx* c) {
     li.f_atoms_per_thread = rbe::F_RMAX;
     const int nk = c->P < rbe::F_KCHUNK ? c->P : rbe::F_KCHUNK;
     li.f_smem_bytes = (int32_t)((size_t)nk * (sizeof(int4) + sizeof(float4)));
-    RBE_CUDA(c, cudaFuncSetAttribute(rbe::f_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, li.f_smem_bytes));
-    RBE_CUDA(c, cudaFuncSetAttribute(rbe::f_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, li.f_smem_bytes));
+    // The attribute belongs to the FUNCTION, not to this context: contexts of different sizes live in one
+    // process, so it is always raised to the most any context can ask for, never set to this context's need.
+    const int f_smem_max = rbe::F_KCHUNK * (int)(sizeof(int4) + sizeof(float4));
+    RBE_CUDA(c, cudaFuncSetAttribute(rbe::f_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, f_smem_max));
+    RBE_CUDA(c, cudaFuncSetAttribute(rbe::f_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, f_smem_max));
     int occ0 = 0, occ1 = 0;  // resident CTAs per SM: the grid is exactly one wave
     RBE_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ0, rbe::f_kernel<false>, rbe::F_THREADS, li.f_smem_bytes));
     RBE_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ1, rbe::f_kernel<true>, rbe::F_THREADS, li.f_smem_bytes));
@@ -218,8 +221,10 @@ rbe_status init_device(rbe_ctx* c) {
     if (f_grid > max_f) f_grid = max_f;
     li.f_grid = (int32_t)f_grid;
 
-    RBE_CUDA(c, cudaFuncSetAttribute(rbe::sf_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, li.sf_smem_bytes));
-    RBE_CUDA(c, cudaFuncSetAttribute(rbe::sf_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, li.sf_smem_bytes));
+    const int sf_smem_max = (int)prop.sharedMemPerBlockOptin - 12 * 1024;   // (static shared memory of the kernel: < 12 KB)
+    if (li.sf_smem_bytes > sf_smem_max) return fail(c, RBE_ERR_CUDA, "structure-factor kernel needs more shared memory than the device offers");
+    RBE_CUDA(c, cudaFuncSetAttribute(rbe::sf_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, sf_smem_max));
+    RBE_CUDA(c, cudaFuncSetAttribute(rbe::sf_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, sf_smem_max));
 
     // ---- workspace layout
     size_t off = 0;

@@ -400,3 +400,22 @@ def test_compact_host_step_matches_the_float4_host_step(N):
     ctx.rbe_set_charges(torch.from_numpy(atoms[:, 3].copy()).cuda())
     U3 = ctx.rbe_step_host_xyz(h_x3, m, h_f3, want_energy=True)
     assert np.array_equal(h_f3, h_f[:, :3]) and U3 == U4
+
+
+def test_contexts_of_different_sizes_coexist():
+    """Found by a randomised sweep: the dynamic-shared-memory limit is an attribute of the kernel FUNCTION; a
+    small context created after a large one must not lower it under the large one's launches."""
+    big_cfg, small_cfg = inputs.CONFIGS["water_96k"], inputs.CONFIGS["water_3k"]
+    big_atoms, small_atoms = inputs.make_atoms(big_cfg), inputs.make_atoms(small_cfg)
+    big = rbe.Rbe(big_cfg.N, big_cfg.L, big_cfg.alpha, big_cfg.P)
+    small = rbe.Rbe(64, small_cfg.L, small_cfg.alpha, 3)                # created second: tiny tile, tiny k-table
+    xb, xs = torch.from_numpy(big_atoms).cuda(), torch.from_numpy(small_atoms[:64].copy()).cuda()
+    Fb, Fs = torch.empty_like(xb), torch.empty_like(xs)
+    mb = inputs.sample_kset(big_cfg.L, big_cfg.alpha, big_cfg.P, 1, 0)
+    ms = inputs.sample_kset(small_cfg.L, small_cfg.alpha, 3, 1, 0)
+    for _ in range(2):                                                   # alternate the two contexts
+        small.rbe_set_kvectors(ms); small.rbe_structure_factor(xs); small.rbe_forces(xs, Fs)
+        big.rbe_set_kvectors(mb); big.rbe_structure_factor(xb); big.rbe_forces(xb, Fb)
+    S = oracle.S(big_cfg.L, big_cfg.alpha)
+    F_o = oracle.force(big_atoms, big_cfg.L, mb, S, oracle.rho(big_atoms, big_cfg.L, mb))
+    assert np.linalg.norm(Fb.cpu().numpy()[:, :3] - F_o) / np.linalg.norm(F_o) <= F_TOL
