@@ -74,34 +74,59 @@ def test_config_small(name, with_energy):
     assert np.abs(F.sum(0)).max() <= 1e-6 * np.abs(F).max(1).sum()
 
 
-def test_config_1m_full_size_bench_configuration():
-    """Config 3 (N = 999 999, P = 200) in the launch configuration bench.py times: rho against
-    the full oracle, forces on 20 000 sampled atoms, sum F = 0 over all atoms."""
-    cfg = inputs.CONFIGS["water_nacl_1m"]
-    atoms = inputs.make_atoms(cfg)
-    m = inputs.sample_kset(cfg.L, cfg.alpha, cfg.P, cfg.seed, 0)
-    sel = np.sort(np.random.default_rng(0).choice(cfg.N, 20_000, replace=False)).astype(np.int64)
-    sel[-3:] = [cfg.N - 3, cfg.N - 2, cfg.N - 1]  # the ragged tail and the ions
-    r = check(atoms, cfg.L, cfg.alpha, m, with_energy=False, sel=sel)
-    F = r["F_gpu"][:, :3].astype(np.float64)
+def _momentum_ok(F_gpu):
+    F = F_gpu[:, :3].astype(np.float64)
     assert np.abs(F.sum(0)).max() <= 1e-6 * np.abs(F).max(1).sum()
 
 
-def test_config_10m_sampled():
+def test_config_1m_full_size_bench_configuration():
+    """Config 3 (N = 999 999, P = 200) in the launch configuration bench.py times: rho and ALL 3N
+    force components against the full oracle (Eq. 2.9, Eq. 2.12), sum F = 0."""
+    cfg = inputs.CONFIGS["water_nacl_1m"]
+    atoms = inputs.make_atoms(cfg)
+    m = inputs.sample_kset(cfg.L, cfg.alpha, cfg.P, cfg.seed, 0)
+    r = check(atoms, cfg.L, cfg.alpha, m, with_energy=False)
+    _momentum_ok(r["F_gpu"])
+
+
+def test_config_10m_full():
+    """Config 4 (N = 9 999 999, P = 200): every force component against the oracle (~7 s of oracle time)."""
     cfg = inputs.CONFIGS["water_10m"]
     atoms = inputs.make_atoms(cfg)
     m = inputs.sample_kset(cfg.L, cfg.alpha, cfg.P, cfg.seed, 0)
-    sel = np.sort(np.random.default_rng(1).choice(cfg.N, 5_000, replace=False)).astype(np.int64)
-    check(atoms, cfg.L, cfg.alpha, m, sel=sel)
+    r = check(atoms, cfg.L, cfg.alpha, m)
+    _momentum_ok(r["F_gpu"])
 
 
-def test_ions_1e8_max_size_small_batch():
-    """The largest sweep point (N = 1e8, L = 1000 A: the hardest case for fp32 phases).  The
-    oracle cannot do P = 200 here in minutes, so the batch is P = 8 and forces are sampled."""
-    cfg = inputs.ions_config(10 ** 8, P=8)
+@pytest.mark.parametrize("P", [50, 100, 200, 400, 800, 1600])
+def test_ion_sweep_batch_sizes_at_1m(P):
+    """Config 5, the P sweep at its own N = 1e6: rho and all 3N force components against the oracle."""
+    cfg = inputs.ions_config(10 ** 6, P=P)
     atoms = inputs.make_atoms(cfg)
     m = inputs.sample_kset(cfg.L, cfg.alpha, cfg.P, cfg.seed, 0)
-    sel = np.sort(np.random.default_rng(2).choice(cfg.N, 2_000, replace=False)).astype(np.int64)
+    r = check(atoms, cfg.L, cfg.alpha, m, with_energy=(P == 100))
+    _momentum_ok(r["F_gpu"])
+
+
+@pytest.mark.parametrize("N", [10 ** 4, 10 ** 5, 10 ** 7])
+def test_ion_sweep_sizes_at_p200(N):
+    """Config 5, the N sweep at P = 200 (N = 1e6 is in the P sweep above, 1e8 below): full oracle."""
+    cfg = inputs.ions_config(N, P=200)
+    atoms = inputs.make_atoms(cfg)
+    m = inputs.sample_kset(cfg.L, cfg.alpha, cfg.P, cfg.seed, 0)
+    r = check(atoms, cfg.L, cfg.alpha, m)
+    _momentum_ok(r["F_gpu"])
+
+
+def test_ions_1e8_max_size_at_p200():
+    """The largest sweep point at its own batch size (N = 1e8, L = 1000 A, P = 200: the hardest case
+    for fp32 phases), as SURVEY.md s8(d) prescribes: oracle rho for all 200 wavevectors once, oracle
+    forces on a seeded subset of 1e5 atoms (plus the ragged tail)."""
+    cfg = inputs.ions_config(10 ** 8, P=200)
+    atoms = inputs.make_atoms(cfg)
+    m = inputs.sample_kset(cfg.L, cfg.alpha, cfg.P, cfg.seed, 0)
+    sel = np.sort(np.random.default_rng(2).choice(cfg.N, 100_000, replace=False)).astype(np.int64)
+    sel[-2:] = [cfg.N - 2, cfg.N - 1]
     check(atoms, cfg.L, cfg.alpha, m, sel=sel)
 
 
