@@ -25,8 +25,10 @@
  *    after the call returns (except the workspace, retained until rbe_destroy or the next
  *    rbe_set_workspace).  `h_*` pointers are HOST memory owned by the caller.
  *  - `stream` is a cudaStream_t passed as void* (0 = the legacy default stream).  Every call
- *    that takes a stream only enqueues work on it and returns; the exceptions are
- *    rbe_kspace_energy and rbe_step_host, which synchronise that stream before returning.
+ *    that takes a stream only enqueues work on it and returns; the exceptions, which synchronise
+ *    that stream (or, where they take none, the device) before returning, are rbe_kspace_energy,
+ *    rbe_kspace_virial, rbe_get_kvectors, rbe_exchange_check, rbe_step_host, rbe_step_host_xyz,
+ *    rbe_probe_pipe_rates, rbe_set_workspace and rbe_graph_capture.
  *  - The library allocates no device memory.  Host memory: the context and a small pinned
  *    staging ring for the k-vectors, both freed by rbe_destroy.
  *  - Every function returns an rbe_status (or a value documented below); nothing aborts,
@@ -66,6 +68,7 @@ typedef struct {
     int32_t sf_k_per_thread, sf_atom_groups, sf_tile_atoms;
     int32_t sf_red_group, sf_red_groups;                     /* in-kernel two-level fixed-order reduction */
     int32_t f_grid, f_threads, f_smem_bytes, f_atoms_per_thread; /* force kernel */
+    int32_t step_fused, step_smem_bytes;                     /* rbe_step runs as ONE cooperative launch (grid sf_grid_x) */
 } rbe_launch_info;
 
 /* Create a context for N atoms (on this GPU), box side L [A], splitting parameter alpha [A^-2]
@@ -83,7 +86,7 @@ double rbe_normaliser_S(const rbe_ctx* ctx);
 
 /* Bytes of device scratch the context needs (per-CTA fp64 partials, rho, the k-set).
  * Queries the current CUDA device on first use.  Returns 0 on error (see rbe_last_error). */
-size_t rbe_workspace_bytes(rbe_ctx* ctx);
+size_t rbe_workspace_bytes(const rbe_ctx* ctx);
 
 /* Hand the context a device buffer of at least rbe_workspace_bytes bytes, 256-byte aligned,
  * allocated on the current CUDA device.  Caller keeps ownership and must keep it alive.
@@ -176,6 +179,9 @@ rbe_status rbe_set_rho(rbe_ctx* ctx, const void* d_rho, void* stream);
  * that rbe_exchange_check reports (it never hangs the GPU).
  *   d_bufs  host array of `world` device pointers, d_bufs[r] = rank r's buffer as mapped in THIS
  *           process (d_bufs[rank] is the local one), each 256-byte aligned, `bytes` long.
+ * Every rbe_set_exchange restarts the step epoch at zero: the buffers of ALL ranks must be zero-filled again
+ * (and the ranks synchronised) before the first step after it.  A consumer that gives up waiting writes NaN
+ * forces / energy, so a missed rbe_exchange_check cannot pass silently.
  * rbe_set_exchange with world < 1 or d_bufs == NULL switches the exchange off.  Not combinable with
  * rbe_set_rho or rbe_graph_capture (RBE_ERR_INVALID_ARG).
  * Errors: RBE_ERR_INVALID_ARG, RBE_ERR_WORKSPACE (bytes too small), RBE_ERR_CUDA. */
@@ -185,7 +191,10 @@ rbe_status rbe_exchange_check(rbe_ctx* ctx, void* stream);   /* synchronises `st
 
 /* Algorithm 1 step 4, Eq. (2.12): forces on this context's N atoms from the
  * current k-set and structure factors.
- *   d_xyzq   float4 [N], device: the same positions the structure factor was computed from.
+ *   d_xyzq   float4 [N], device: the same positions the structure factor was computed from.  The kernel is
+ *            launched with programmatic stream serialisation; before it waits for the preceding kernel of the
+ *            stream it only issues L2 prefetches for d_xyzq (no value is consumed early), so a preceding
+ *            kernel may still be writing the positions.
  *   d_force  float4 [N], device: {F_x, F_y, F_z, e_i}; e_i = 0 unless with_energy != 0, then
  *            e_i = (2 pi q_i / V) sum_l w_l Re(exp(-i k_l . r_i) rho(k_l)) / k_l^2 (sum_i e_i = U).
  * Errors: RBE_ERR_NOT_READY (no structure factor since the last rbe_set_kvectors),
@@ -193,9 +202,28 @@ rbe_status rbe_exchange_check(rbe_ctx* ctx, void* stream);   /* synchronises `st
 rbe_status rbe_forces(rbe_ctx* ctx, const void* d_xyzq, void* d_force, int32_t with_energy,
                       void* stream);
 
+/* Algorithm 1 steps 2-4 -- Eq. (2.9) P:117 then Eq. (2.12) P:131 -- as ONE cooperative kernel launch:
+ * structure-factor phase, a grid-wide barrier, a fixed-order reduction of the per-CTA fp64 rows distributed
+ * over the CTAs (which also builds every wavevector's force record once), a second barrier, force phase.
+ *   h_m, h_w   as rbe_set_kvectors, or h_m == NULL: keep the k-set already on the device (rbe_set_kvectors /
+ *              rbe_sample_kvectors).  With h_w == NULL and P <= 512 the wavevectors travel in the kernel
+ *              parameters: the step is one launch and no host-to-device copy.
+ *   d_xyzq     float4 [N] device;  d_force  float4 [N] device (as rbe_forces);  with_energy as rbe_forces
+ *   d_rho      double2 [P] device, or NULL
+ * Equivalent to rbe_set_kvectors + rbe_structure_factor + rbe_forces: the same arithmetic per (atom, k) pair,
+ * the same tolerances against the definitions; rho differs from rbe_structure_factor's in the last bits only
+ * (another fixed order of the per-CTA rows).  Bitwise reproducible.  Afterwards rbe_kspace_energy /
+ * rbe_kspace_virial / rbe_forces refer to this step.  Falls back to the two launches when P > 4096, when a
+ * multi-GPU exchange is configured, or when the device cannot launch cooperatively (rbe_launch_info.step_fused).
+ * d_xyzq must not be written by other work while the launch runs; no other kernel may share the GPU's SMs with
+ * it in a way that keeps part of the grid from becoming resident (the cooperative launch fails rather than hangs).
+ * Errors: RBE_ERR_NOT_READY, RBE_ERR_BAD_KVECTOR, RBE_ERR_INVALID_ARG, RBE_ERR_CUDA. */
+rbe_status rbe_step(rbe_ctx* ctx, const int32_t* h_m, const double* h_w, const void* d_xyzq, void* d_force,
+                    int32_t with_energy, void* d_rho, void* stream);
+
 /* Real-space partner of the RBE force: the short-range part of the Ewald-split Coulomb force,
  * Eq. (2.10), truncated at the cutoff radius r_s, over a linked-cell list of cubic
- * cells of side >= r_s (the cell list of Algorithm 2):
+ * cells of side >= r_s (a one-shot cell list; Algorithm 2's own list has cells of side r_c):
  *   F_i = - q_i sum_{j != i, r < r_s} q_j ( erfc(sqrt(alpha) r) / r^2
  *            + 2 sqrt(alpha) exp(-alpha r^2) / (sqrt(pi) r) ) d / r,   d = nearest image of r_j - r_i
  *   e_i = 1/2 q_i sum_{j != i, r < r_s} q_j erfc(sqrt(alpha) r) / r      (first term of Eq. 2.8)
@@ -247,12 +275,14 @@ rbe_status rbe_kspace_virial(rbe_ctx* ctx, double* h_W, void* stream);
 /* One whole step from HOST buffers (the end-to-end path): copies h_xyzq (float [N][4]) to the
  * device, uploads the k-set, runs rbe_structure_factor and rbe_forces, copies the forces back
  * into h_force (float [N][4]) and, if h_U != NULL, the energy into *h_U; synchronises `stream`.
- * d_scratch: caller-owned device buffer of at least 32 * N bytes (positions + forces).
+ * d_scratch: caller-owned device buffer of at least rbe_step_host_bytes(ctx, 0) bytes (positions + forces:
+ * about 32 B per atom), 256-byte aligned.
  * With N >= 131 072 the atoms travel in up to 4 chunks on two internal copy streams so that the
  * transfers overlap the kernels (every chunk adds to the same per-CTA fp64 partial rows in stream
  * order: the result stays bitwise reproducible).  Pinned host buffers (rbe_host_alloc) make the
  * copies asynchronous; pageable ones work but are slower.
  * Errors: as the calls it is made of, plus RBE_ERR_WORKSPACE if d_scratch is too small. */
+size_t     rbe_step_host_bytes(const rbe_ctx* ctx, int32_t compact);   /* d_scratch size: compact = 0 rbe_step_host, 1 rbe_step_host_xyz */
 rbe_status rbe_step_host(rbe_ctx* ctx, const float* h_xyzq, const int32_t* h_m, const double* h_w,
                          float* h_force, int32_t with_energy, double* h_U, void* d_scratch,
                          size_t scratch_bytes, void* stream);
@@ -262,13 +292,21 @@ rbe_status rbe_step_host(rbe_ctx* ctx, const float* h_xyzq, const int32_t* h_m, 
  * atom over PCIe instead of 32.  The charges live on the device: rbe_set_charges(ctx, d_q) registers a
  * caller-owned device array float [N] (retained until replaced; NULL unregisters).  Same chunked
  * pipeline and the same two hot kernels as rbe_step_host, plus a pack and an unpack kernel per chunk;
- * the forces are bitwise those of rbe_step_host.  d_scratch: at least 56 * N + 1024 bytes, 256-byte
- * aligned.  Per-atom energies are not returned; h_U (optional) receives the k-space energy.
+ * the forces are bitwise those of rbe_step_host.  d_scratch: at least rbe_step_host_bytes(ctx, 1)
+ * bytes (about 56 B per atom), 256-byte aligned.  Per-atom energies are not returned; h_U (optional) receives the k-space energy.
  * Synchronises `stream`.  Errors: as rbe_step_host, plus RBE_ERR_NOT_READY without rbe_set_charges. */
 rbe_status rbe_set_charges(rbe_ctx* ctx, const void* d_q);
 rbe_status rbe_step_host_xyz(rbe_ctx* ctx, const float* h_xyz, const int32_t* h_m, const double* h_w,
                              float* h_force3, double* h_U, void* d_scratch, size_t scratch_bytes,
                              void* stream);
+
+/* Measure, on this device and now, the issue rates that bound this path (there is no vendor-stated figure to
+ * take them from): h_out double [5] (host) = thread-instructions per SM per clock of FFMA, IMAD, I2FP.F32.S32
+ * and MUFU.SIN (dependent-free chains, 32 warps per SM, in-kernel clock64), and the SM clock in MHz observed
+ * while the MUFU probe ran (its cycles / its CUDA-event time).  Four short launches (~0.2 ms in all) that use the
+ * workspace as scratch: call it between steps (it invalidates the per-CTA rows of a chunked host step in
+ * flight, nothing else).  Synchronises `stream`.  Errors: RBE_ERR_NOT_READY, RBE_ERR_INVALID_ARG, RBE_ERR_CUDA. */
+rbe_status rbe_probe_pipe_rates(rbe_ctx* ctx, double* h_out, void* stream);
 
 /* Page-locked (pinned) HOST memory for the end-to-end path: cudaHostAlloc'ed, so that the copies of
  * rbe_step_host are asynchronous DMA transfers at full PCIe rate (measured on B200 hosts: 55 GB/s

@@ -1,6 +1,5 @@
-"""Build csrc/ -> paper_2407_09315_b200/librbe.so (the C-ABI library) and
-paper_2407_09315_b200/pipe_probe (the stand-alone pipe-rate / MUFU-accuracy probe) with nvcc
-for sm_100a, in-tree, so that both travel with the repository snapshot to the GPU box."""
+"""Build csrc/ -> paper_2407_09315_b200/librbe.so (the C-ABI library) with nvcc for sm_100a,
+in-tree, so that it travels with the repository snapshot to the GPU box."""
 from __future__ import annotations
 
 import os
@@ -13,9 +12,6 @@ CSRC = os.path.join(HERE, "csrc")
 SO = os.path.join(HERE, "librbe.so")
 SOURCES = [os.path.join(CSRC, "rbe_api.cu")]
 DEPS = SOURCES + [os.path.join(CSRC, f) for f in sorted(os.listdir(CSRC)) if f.endswith(".cuh")] + [os.path.join(ROOT, "include", "rbe.h")]
-PROBE = os.path.join(HERE, "pipe_probe")
-PROBE_SRC = os.path.join(CSRC, "pipe_probe.cu")
-
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a",
     "-O3", "-lineinfo", "-std=c++17",
@@ -31,22 +27,7 @@ def is_stale() -> bool:
     return any(os.path.getmtime(d) > t for d in DEPS)
 
 
-def build_probe(force: bool = False) -> str:
-    if not force and os.path.exists(PROBE) and os.path.getmtime(PROBE) >= os.path.getmtime(PROBE_SRC):
-        return PROBE
-    nvcc = os.environ.get("NVCC", "nvcc")
-    tmp = PROBE + f".tmp{os.getpid()}"
-    cmd = [nvcc, "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17", "-o", tmp, PROBE_SRC]
-    res = subprocess.run(cmd, capture_output=True, text=True)
-    if res.returncode != 0:
-        sys.stderr.write(res.stdout + res.stderr)
-        raise RuntimeError("nvcc failed: " + " ".join(cmd))
-    os.replace(tmp, PROBE)
-    return PROBE
-
-
 def build(force: bool = False, verbose: bool = False) -> str:
-    build_probe(force)
     if not (force or is_stale()):
         return SO
     nvcc = os.environ.get("NVCC", "nvcc")

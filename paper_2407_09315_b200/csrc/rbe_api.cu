@@ -2,6 +2,7 @@
 // upload and kernel launches.  No torch types, no device allocation, no CPU fallback.
 #include "rbe.h"
 
+#include <algorithm>
 #include <cmath>
 #include <cstdio>
 #include <cstring>
@@ -13,10 +14,6 @@
 #include "sr_kernels.cuh"
 #include "sr_pair_kernels.cuh"
 #include "rbl_kernels.cuh"
-
-#ifdef RBE_SF_PROFILE
-static long long* g_rbe_prof = nullptr;
-#endif
 
 namespace {
 
@@ -44,6 +41,10 @@ struct rbe_ctx {
     int sf_ngroups = 1;
     size_t ws_bytes = 0;
     size_t off_kvec = 0, off_w = 0, off_part = 0, off_rho = 0, off_grow = 0, off_U = 0, off_ticket = 0;
+    size_t off_ka = 0, off_kb = 0, off_bar = 0;
+    bool sf_deep = false;       // a thread takes more than SF_DEPTH atoms from one tile: flush inside the loops
+    bool step_fused = false;    // the one-launch cooperative step kernel is usable for this context
+    size_t step_smem = 0;
 
     // workspace
     unsigned char* ws = nullptr;
@@ -137,24 +138,6 @@ bool build_sampler_table(double L, double alpha, std::vector<uint32_t>& T, int32
     return true;
 }
 
-// Shared-memory tile of the structure-factor kernel for a launch over n atoms: up to 4 windows of
-// 32 atoms per warp (amortises the staging barriers), but no more than one CTA's share needs.
-struct SfTile { int tile, flush_every; bool deep; };
-SfTile sf_tile(const rbe_ctx* c, int64_t n) {
-    const int gx = c->li.sf_grid_x, threads = c->li.sf_threads, ng = c->sf_ng;
-    const int64_t share = n > 0 ? ((n + gx - 1) / gx + 31) / 32 * 32 : 32;
-    int tile = 4 * threads;
-    if (tile > rbe::SF_TILE_MAX) tile = rbe::SF_TILE_MAX;
-    if ((int64_t)tile > share) tile = (int)share;
-    if (tile < 32) tile = 32;
-    const int per_group = (tile + ng - 1) / ng;   // atoms a group takes from one tile
-    SfTile t;
-    t.tile = tile;
-    t.flush_every = per_group >= rbe::SF_DEPTH ? 1 : rbe::SF_DEPTH / per_group;
-    t.deep = per_group + 1 > rbe::SF_DEPTH;       // more than SF_DEPTH atoms from one tile: flush inside the loops
-    return t;
-}
-
 // Choose the launch geometry for this context on the current device.
 rbe_status init_device(rbe_ctx* c) {
     if (c->dev_ready) return RBE_OK;
@@ -173,27 +156,27 @@ rbe_status init_device(rbe_ctx* c) {
     rbe_launch_info& li = c->li;
     li.num_sms = prop.multiProcessorCount;
 
-    // ---- SF kernel: a thread owns SF_KPT wavevectors; gs threads cover one k-chunk, ng atom
-    // groups share a CTA of up to SF_TMAX threads (one CTA per SM); tile = blockDim.x atoms.
+    // ---- SF phase: a thread owns SF_KPT wavevectors; gs threads cover one k-chunk, ng atom
+    // groups share a CTA of up to SF_TMAX threads (one CTA per SM).
     const int slots = (c->P + rbe::SF_KPT - 1) / rbe::SF_KPT;
     int gy = (slots + rbe::SF_TMAX - 1) / rbe::SF_TMAX;
     int gs = (slots + gy - 1) / gy;
     int ng = rbe::SF_TMAX / gs;
     if (ng < 1) ng = 1;
     int threads = (int)align_up((size_t)gs * ng, 32);
-    int gx = rbe::SF_CTAS_PER_SM * li.num_sms / gy;
+    int gx = li.num_sms / gy;
     if (gx < 1) gx = 1;
     // never more CTAs than 32-atom windows to feed them
     const int64_t max_gx = c->N > 0 ? (c->N + 31) / 32 : 1;
     if ((int64_t)gx > max_gx) gx = (int)max_gx;
     c->sf_gs = gs; c->sf_ng = ng;
     li.sf_threads = threads; li.sf_grid_x = gx;
-    const SfTile tl = sf_tile(c, c->N);
-    const int tile = tl.tile;
+    const int tile = (threads / 32) * rbe::SF_WPT * 32;     // atoms per tile: SF_WPT windows per warp
+    c->sf_deep = (tile + ng - 1) / ng + 2 > rbe::SF_DEPTH;
     li.sf_grid_y = gy;
     li.sf_k_per_thread = rbe::SF_KPT; li.sf_atom_groups = ng; li.sf_tile_atoms = tile;
-    // raw tile + record arena (16 B per atom each) + fp64 accumulators [SF_KPT][threads]
-    li.sf_smem_bytes = (int32_t)((size_t)tile * 2 * sizeof(uint4) + (size_t)threads * rbe::SF_KPT * sizeof(double2));
+    // two record arenas (16 B per atom each) + fp64 accumulators [SF_KPT][threads]
+    li.sf_smem_bytes = (int32_t)rbe::sf_smem_bytes(threads);
 
     c->sf_ngroups = (gx + rbe::SF_RED_GROUP - 1) / rbe::SF_RED_GROUP;
     li.sf_red_group = rbe::SF_RED_GROUP;
@@ -221,10 +204,28 @@ rbe_status init_device(rbe_ctx* c) {
     if (f_grid > max_f) f_grid = max_f;
     li.f_grid = (int32_t)f_grid;
 
-    const int sf_smem_max = (int)prop.sharedMemPerBlockOptin - 12 * 1024;   // (static shared memory of the kernel: < 12 KB)
+    const int sf_smem_max = (int)prop.sharedMemPerBlockOptin - 4 * 1024;   // (static shared memory of the kernels: < 4 KB)
     if (li.sf_smem_bytes > sf_smem_max) return fail(c, RBE_ERR_CUDA, "structure-factor kernel needs more shared memory than the device offers");
     RBE_CUDA(c, cudaFuncSetAttribute(rbe::sf_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, sf_smem_max));
     RBE_CUDA(c, cudaFuncSetAttribute(rbe::sf_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, sf_smem_max));
+
+    // ---- one-launch step kernel (cooperative: one CTA per SM, all co-resident): one k-chunk only
+    c->step_smem = (size_t)li.sf_smem_bytes;
+    if ((size_t)c->P * (sizeof(int4) + sizeof(float4)) > c->step_smem) c->step_smem = (size_t)c->P * (sizeof(int4) + sizeof(float4));
+    int coop = 0;
+    RBE_CUDA(c, cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, c->device));
+    c->step_fused = coop && gy == 1 && c->P <= rbe::STEP_PMAX && c->step_smem <= (size_t)sf_smem_max && gx <= li.num_sms;
+    if (c->step_fused) {
+        RBE_CUDA(c, cudaFuncSetAttribute(rbe::step_kernel<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, sf_smem_max));
+        RBE_CUDA(c, cudaFuncSetAttribute(rbe::step_kernel<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, sf_smem_max));
+        RBE_CUDA(c, cudaFuncSetAttribute(rbe::step_kernel<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, sf_smem_max));
+        RBE_CUDA(c, cudaFuncSetAttribute(rbe::step_kernel<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, sf_smem_max));
+        int occ = 0;
+        RBE_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, rbe::step_kernel<true, true>, threads, c->step_smem));
+        if (occ < 1) c->step_fused = false;
+    }
+    li.step_fused = c->step_fused ? 1 : 0;
+    li.step_smem_bytes = (int32_t)c->step_smem;
 
     // ---- workspace layout
     size_t off = 0;
@@ -239,6 +240,9 @@ rbe_status init_device(rbe_ctx* c) {
     c->off_T = off;    off = align_up(off + c->sampler_T.size() * sizeof(uint32_t) + 4, 256);
     c->off_state = off; off = align_up(off + 2 * sizeof(unsigned long long), 256);
     c->off_xch_err = off; off = align_up(off + sizeof(int32_t), 256);
+    c->off_ka = off;   off = align_up(off + P * sizeof(int4), 256);      // per-k force records of the step kernel
+    c->off_kb = off;   off = align_up(off + P * sizeof(float4), 256);
+    c->off_bar = off;  off = align_up(off + sizeof(unsigned long long), 256);   // grid-barrier arrival counter
     c->ws_bytes = off;
 
     c->stage_bytes = P * (sizeof(int4) + sizeof(double));
@@ -288,21 +292,27 @@ rbe_status launch_sampler(rbe_ctx* c, bool from_state, uint64_t seed, uint64_t s
     return RBE_OK;
 }
 
+rbe::SfArgs sf_args(rbe_ctx* c, const void* d_xyzq, int64_t n, int accumulate) {
+    rbe::SfArgs a;
+    a.xyzq = static_cast<const float4*>(d_xyzq);
+    a.N = n;
+    a.part = ws_ptr<double2>(c, c->off_part);
+    a.two32_over_L = rbe::TWO32 / c->L;
+    a.P = c->P; a.gs = c->sf_gs; a.ng = c->sf_ng;
+    a.pairing = c->sf_pairing;
+    a.accumulate = accumulate;
+    return a;
+}
+
 // One launch of the structure-factor kernel over n atoms.  accumulate: add to the per-CTA rows
 // already in the workspace; finalise: run the fixed-order second pass (rows -> rho) in this launch.
 rbe_status launch_sf(rbe_ctx* c, const void* d_xyzq, int64_t n, int accumulate, int finalise, void* d_rho,
                      cudaStream_t st) {
-    const SfTile tl = sf_tile(c, n);
     rbe::SfParams sp;
-    sp.xyzq = static_cast<const float4*>(d_xyzq);
-    sp.N = n;
+    sp.a = sf_args(c, d_xyzq, n, accumulate);
     sp.kvec = ws_ptr<int4>(c, c->off_kvec);
-    sp.part = ws_ptr<double2>(c, c->off_part);
-    sp.two32_over_L = rbe::TWO32 / c->L;
-    sp.P = c->P; sp.gs = c->sf_gs; sp.ng = c->sf_ng; sp.flush_every = tl.flush_every; sp.tile_atoms = tl.tile;
-    sp.pairing = c->sf_pairing;
-    sp.accumulate = accumulate; sp.finalise = finalise;
-    sp.red.part = sp.part;
+    sp.finalise = finalise;
+    sp.red.part = sp.a.part;
     sp.red.grow = ws_ptr<double2>(c, c->off_grow);
     sp.red.rho = ws_ptr<double2>(c, c->off_rho);
     sp.red.rho_user = static_cast<double2*>(d_rho);
@@ -321,16 +331,9 @@ rbe_status launch_sf(rbe_ctx* c, const void* d_xyzq, int64_t n, int accumulate, 
             sp.red.xch.flag[r] = reinterpret_cast<uint32_t*>(c->xch_buf[r] + fo) + parity * c->xch_world + c->xch_rank;
         }
     }
-#ifdef RBE_SF_PROFILE
-    static long long* d_prof = nullptr;
-    if (!d_prof) cudaMalloc(&d_prof, 4096 * 64 * sizeof(long long));
-    cudaMemsetAsync(d_prof, 0, 4096 * 64 * sizeof(long long), st);
-    sp.prof = d_prof;
-    g_rbe_prof = d_prof;
-#endif
-    const size_t smem = (size_t)tl.tile * 2 * sizeof(uint4) + (size_t)c->li.sf_threads * rbe::SF_KPT * sizeof(double2);
+    const size_t smem = (size_t)c->li.sf_smem_bytes;
     dim3 grid(c->li.sf_grid_x, c->li.sf_grid_y);
-    if (tl.deep) rbe::sf_kernel<true><<<grid, c->li.sf_threads, smem, st>>>(sp);
+    if (c->sf_deep) rbe::sf_kernel<true><<<grid, c->li.sf_threads, smem, st>>>(sp);
     else rbe::sf_kernel<false><<<grid, c->li.sf_threads, smem, st>>>(sp);
     RBE_CUDA(c, cudaGetLastError());
     return RBE_OK;
@@ -341,11 +344,11 @@ rbe_status launch_sf(rbe_ctx* c, const void* d_xyzq, int64_t n, int accumulate, 
 // reads anything that grid wrote).
 rbe_status launch_f(rbe_ctx* c, const void* d_xyzq, void* d_force, int64_t n, int with_energy, cudaStream_t st) {
     rbe::FParams fp;
-    fp.xyzq = static_cast<const float4*>(d_xyzq);
-    fp.force = static_cast<float4*>(d_force);
-    fp.N = n;
+    fp.a.xyzq = static_cast<const float4*>(d_xyzq);
+    fp.a.force = static_cast<float4*>(d_force);
+    fp.a.N = n;
+    fp.a.two32_over_L = rbe::TWO32 / c->L;
     fp.kt = k_table(c);
-    fp.two32_over_L = rbe::TWO32 / c->L;
     fp.P = c->P;
     fp.pdl = 1;
     const int64_t units = (n + 31) / 32, wpc = rbe::F_THREADS / 32;
@@ -368,13 +371,61 @@ rbe_status launch_f(rbe_ctx* c, const void* d_xyzq, void* d_force, int64_t n, in
     return RBE_OK;
 }
 
-}  // namespace
-
-#ifdef RBE_SF_PROFILE
-extern "C" int rbe_debug_prof(long long* h_out, int nrows) {
-    return (int)cudaMemcpy(h_out, g_rbe_prof, (size_t)nrows * 64 * sizeof(long long), cudaMemcpyDeviceToHost);
+// The whole k-space step as ONE cooperative launch (step_kernel).  h_m != nullptr: the wavevectors ride in
+// the kernel parameters (P <= STEP_KPARAM_MAX, uniform weights); else they are read from the workspace.
+rbe_status launch_step(rbe_ctx* c, const int32_t* h_m, const void* d_xyzq, void* d_force, int with_energy, void* d_rho,
+                       cudaStream_t st) {
+    rbe::StepParams sp;
+    sp.sf = sf_args(c, d_xyzq, c->N, 0);
+    sp.f.xyzq = static_cast<const float4*>(d_xyzq);
+    sp.f.force = static_cast<float4*>(d_force);
+    sp.f.N = c->N;
+    sp.f.two32_over_L = rbe::TWO32 / c->L;
+    sp.kvec = ws_ptr<int4>(c, c->off_kvec);
+    sp.w = c->have_w ? ws_ptr<double>(c, c->off_w) : nullptr;
+    sp.w_uniform = c->S / (double)c->P;
+    sp.L = c->L;
+    sp.rho = ws_ptr<double2>(c, c->off_rho);
+    sp.rho_user = static_cast<double2*>(d_rho);
+    sp.ka = ws_ptr<int4>(c, c->off_ka);
+    sp.kb = ws_ptr<float4>(c, c->off_kb);
+    sp.bar = ws_ptr<unsigned long long>(c, c->off_bar);
+    sp.kparam = h_m ? 1 : 0;
+    if (h_m)
+        for (int32_t i = 0; i < 3 * c->P; ++i) sp.km[i] = (int16_t)h_m[i];   // validated: |m_d| < 2^15
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((unsigned)c->li.sf_grid_x);
+    cfg.blockDim = dim3((unsigned)c->li.sf_threads);
+    cfg.dynamicSmemBytes = c->step_smem;
+    cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeCooperative;
+    attr[0].val.cooperative = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    if (c->sf_deep) {
+        if (with_energy) RBE_CUDA(c, cudaLaunchKernelEx(&cfg, rbe::step_kernel<true, true>, sp));
+        else RBE_CUDA(c, cudaLaunchKernelEx(&cfg, rbe::step_kernel<true, false>, sp));
+    } else {
+        if (with_energy) RBE_CUDA(c, cudaLaunchKernelEx(&cfg, rbe::step_kernel<false, true>, sp));
+        else RBE_CUDA(c, cudaLaunchKernelEx(&cfg, rbe::step_kernel<false, false>, sp));
+    }
+    return RBE_OK;
 }
-#endif
+
+rbe_status check_kvectors(rbe_ctx* c, const int32_t* h_m, const double* h_w) {
+    for (int32_t l = 0; l < c->P; ++l) {
+        const int32_t a = h_m[3 * l], b = h_m[3 * l + 1], d = h_m[3 * l + 2];
+        if ((a == 0 && b == 0 && d == 0) || a <= -32768 || a >= 32768 || b <= -32768 || b >= 32768 ||
+            d <= -32768 || d >= 32768)
+            return fail(c, RBE_ERR_BAD_KVECTOR, "k-vector " + std::to_string(l) + " is zero or out of range (|m_d| < 2^15)");
+        if (h_w && !std::isfinite(h_w[l]))
+            return fail(c, RBE_ERR_BAD_KVECTOR, "weight " + std::to_string(l) + " is not finite");
+    }
+    return RBE_OK;
+}
+
+}  // namespace
 
 extern "C" {
 
@@ -417,8 +468,9 @@ rbe_status rbe_destroy(rbe_ctx* c) {
 
 double rbe_normaliser_S(const rbe_ctx* c) { return c ? c->S : 0.0; }
 
-size_t rbe_workspace_bytes(rbe_ctx* c) {
-    if (!c) return 0;
+size_t rbe_workspace_bytes(const rbe_ctx* cc) {
+    if (!cc) return 0;
+    rbe_ctx* c = const_cast<rbe_ctx*>(cc);   // the launch geometry is a lazily filled cache of the context
     if (init_device(c) != RBE_OK) return 0;
     return c->ws_bytes;
 }
@@ -437,6 +489,7 @@ rbe_status rbe_set_workspace(rbe_ctx* c, void* d_ws, size_t bytes) {
         RBE_CUDA(c, cudaMemcpy(c->ws + c->off_T, c->sampler_T.data(), c->sampler_T.size() * sizeof(uint32_t), cudaMemcpyHostToDevice));
     RBE_CUDA(c, cudaMemset(c->ws + c->off_state, 0, 2 * sizeof(unsigned long long)));
     RBE_CUDA(c, cudaMemset(c->ws + c->off_xch_err, 0, sizeof(int32_t)));
+    RBE_CUDA(c, cudaMemset(c->ws + c->off_bar, 0, sizeof(unsigned long long)));
     if (c->graph_exec) { cudaGraphExecDestroy(c->graph_exec); c->graph_exec = nullptr; }   // bound to the old workspace
     if (c->graph) { cudaGraphDestroy(c->graph); c->graph = nullptr; }
     RBE_CUDA(c, cudaDeviceSynchronize());
@@ -460,14 +513,8 @@ rbe_status rbe_get_launch_info(const rbe_ctx* c, rbe_launch_info* out) {
 rbe_status rbe_set_kvectors(rbe_ctx* c, const int32_t* h_m, const double* h_w, void* stream) {
     if (!c || !h_m) return fail(c, RBE_ERR_INVALID_ARG, "rbe_set_kvectors: null argument");
     // validate first: independent of the device state
-    for (int32_t l = 0; l < c->P; ++l) {
-        const int32_t a = h_m[3 * l], b = h_m[3 * l + 1], d = h_m[3 * l + 2];
-        if ((a == 0 && b == 0 && d == 0) || a <= -32768 || a >= 32768 || b <= -32768 || b >= 32768 ||
-            d <= -32768 || d >= 32768)
-            return fail(c, RBE_ERR_BAD_KVECTOR, "k-vector " + std::to_string(l) + " is zero or out of range (|m_d| < 2^15)");
-        if (h_w && !std::isfinite(h_w[l]))
-            return fail(c, RBE_ERR_BAD_KVECTOR, "weight " + std::to_string(l) + " is not finite");
-    }
+    const rbe_status vs = check_kvectors(c, h_m, h_w);
+    if (vs != RBE_OK) return vs;
     if (!c->ws) return fail(c, RBE_ERR_NOT_READY, "rbe_set_kvectors before rbe_set_workspace");
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     const int slot = c->stage_next;
@@ -526,6 +573,42 @@ rbe_status rbe_forces(rbe_ctx* c, const void* d_xyzq, void* d_force, int32_t wit
     if (!d_xyzq || !d_force || (reinterpret_cast<uintptr_t>(d_xyzq) & 15u) || (reinterpret_cast<uintptr_t>(d_force) & 15u))
         return fail(c, RBE_ERR_INVALID_ARG, "rbe_forces: null or misaligned pointer");
     return launch_f(c, d_xyzq, d_force, c->N, with_energy, static_cast<cudaStream_t>(stream));
+}
+
+rbe_status rbe_step(rbe_ctx* c, const int32_t* h_m, const double* h_w, const void* d_xyzq, void* d_force, int32_t with_energy,
+                    void* d_rho, void* stream) {
+    if (!c) return RBE_ERR_INVALID_ARG;
+    if (!c->ws) return fail(c, RBE_ERR_NOT_READY, "rbe_step before rbe_set_workspace");
+    if (!h_m && h_w) return fail(c, RBE_ERR_INVALID_ARG, "rbe_step: weights without wavevectors");
+    if (!h_m && !c->have_k) return fail(c, RBE_ERR_NOT_READY, "rbe_step: no k-set (pass h_m, or call rbe_set_kvectors / rbe_sample_kvectors first)");
+    if ((c->N > 0 && (!d_xyzq || !d_force)) || (reinterpret_cast<uintptr_t>(d_xyzq) & 15u) || (reinterpret_cast<uintptr_t>(d_force) & 15u) ||
+        (reinterpret_cast<uintptr_t>(d_rho) & 15u))
+        return fail(c, RBE_ERR_INVALID_ARG, "rbe_step: null or misaligned pointer");
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    const bool fused = c->step_fused && c->xch_world == 0;
+    rbe_status s = RBE_OK;
+    if (h_m) {
+        if (fused && !h_w && c->P <= rbe::STEP_KPARAM_MAX) {
+            // the wavevectors travel in the kernel parameters: validate here, no copy, no staging
+            s = check_kvectors(c, h_m, nullptr);
+            if (s != RBE_OK) return s;
+            c->have_k = true; c->have_w = false; c->have_rho = false;
+            s = launch_step(c, h_m, d_xyzq, d_force, with_energy, d_rho, st);
+            if (s == RBE_OK) c->have_rho = true;
+            return s;
+        }
+        s = rbe_set_kvectors(c, h_m, h_w, stream);
+        if (s != RBE_OK) return s;
+    }
+    if (fused) {
+        s = launch_step(c, nullptr, d_xyzq, d_force, with_energy, d_rho, st);
+        if (s == RBE_OK) c->have_rho = true;
+        return s;
+    }
+    // several k-chunks (P > 4096), a multi-GPU exchange, or no cooperative launch: the two-launch path
+    s = rbe_structure_factor(c, d_xyzq, d_rho, stream);
+    if (s != RBE_OK) return s;
+    return rbe_forces(c, d_xyzq, d_force, with_energy, stream);
 }
 
 rbe_status rbe_kspace_energy(rbe_ctx* c, double* h_U, void* stream) {
@@ -774,6 +857,12 @@ rbe_status rbe_kspace_virial(rbe_ctx* c, double* h_W, void* stream) {
     return RBE_OK;
 }
 
+size_t rbe_step_host_bytes(const rbe_ctx* c, int32_t compact) {
+    if (!c) return 0;
+    const size_t nb = (size_t)c->N * sizeof(float4), nb3 = (size_t)c->N * 3 * sizeof(float);
+    return align_up(nb, 256) + align_up(nb, 256) + (compact ? align_up(nb3, 256) + align_up(nb3, 256) : 0);
+}
+
 namespace {
 // The end-to-end step from host buffers.  compact = false: float4 {x,y,z,q} in, float4 {F, e} out.
 // compact = true: float3 positions in, float3 forces out, charges from rbe_set_charges; a pack and an
@@ -784,10 +873,9 @@ rbe_status step_host_impl(rbe_ctx* c, const float* h_in, const int32_t* h_m, con
     if ((c->N > 0 && (!h_in || !h_out)) || !h_m) return fail(c, RBE_ERR_INVALID_ARG, "rbe_step_host: null argument");
     if (compact && c->N > 0 && !c->d_q) return fail(c, RBE_ERR_NOT_READY, "rbe_step_host_xyz needs rbe_set_charges");
     const size_t nb = (size_t)c->N * sizeof(float4), nb3 = (size_t)c->N * 3 * sizeof(float);
-    const size_t need = align_up(nb, 256) + align_up(nb, 256) + (compact ? align_up(nb3, 256) + nb3 : 0);
+    const size_t need = rbe_step_host_bytes(c, compact ? 1 : 0);
     if (c->N > 0 && (!d_scratch || scratch_bytes < need || (reinterpret_cast<uintptr_t>(d_scratch) & 255u)))
-        return fail(c, RBE_ERR_WORKSPACE, compact ? "rbe_step_host_xyz: d_scratch must hold 56*N (+1024) bytes, 256-byte aligned"
-                                                  : "rbe_step_host: d_scratch must hold 32*N (+512) bytes, 256-byte aligned");
+        return fail(c, RBE_ERR_WORKSPACE, "rbe_step_host: d_scratch must hold rbe_step_host_bytes bytes, 256-byte aligned");
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     unsigned char* base = static_cast<unsigned char*>(d_scratch);
     float4* d_x = reinterpret_cast<float4*>(base);
@@ -903,6 +991,49 @@ rbe_status rbe_set_charges(rbe_ctx* c, const void* d_q) {
 rbe_status rbe_step_host_xyz(rbe_ctx* c, const float* h_xyz, const int32_t* h_m, const double* h_w, float* h_force3,
                              double* h_U, void* d_scratch, size_t scratch_bytes, void* stream) {
     return step_host_impl(c, h_xyz, h_m, h_w, h_force3, 0, h_U, d_scratch, scratch_bytes, stream, true);
+}
+
+rbe_status rbe_probe_pipe_rates(rbe_ctx* c, double* h_out, void* stream) {
+    if (!c || !h_out) return fail(c, RBE_ERR_INVALID_ARG, "rbe_probe_pipe_rates: null argument");
+    if (!c->ws) return fail(c, RBE_ERR_NOT_READY, "rbe_probe_pipe_rates before rbe_set_workspace");
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    const int sms = c->li.num_sms, iters = 2048, chains = 8;
+    // scratch: the grid-barrier-free tail of the workspace is not touched; the group rows are (>= 16 B * P per group)
+    if ((size_t)sms * sizeof(long long) > (size_t)c->li.sf_grid_x * c->P * sizeof(double2) + (c->off_rho - c->off_part))
+        return fail(c, RBE_ERR_WORKSPACE, "rbe_probe_pipe_rates: workspace too small");
+    long long* d_cyc = ws_ptr<long long>(c, c->off_part);
+    std::vector<long long> cyc((size_t)sms);
+    cudaEvent_t e0, e1;
+    RBE_CUDA(c, cudaEventCreate(&e0));
+    RBE_CUDA(c, cudaEventCreate(&e1));
+    double clock_mhz = 0.0;
+    for (int mode = 0; mode < 4; ++mode) {
+        for (int rep = 0; rep < 2; ++rep) {   // rep 0 warms up
+            RBE_CUDA(c, cudaEventRecord(e0, st));
+            switch (mode) {
+                case 0: rbe::probe_kernel<0><<<sms, 1024, 0, st>>>(d_cyc, iters, 1.0001f, 0.5f, 3, 7); break;
+                case 1: rbe::probe_kernel<1><<<sms, 1024, 0, st>>>(d_cyc, iters, 1.0001f, 0.5f, 3, 7); break;
+                case 2: rbe::probe_kernel<2><<<sms, 1024, 0, st>>>(d_cyc, iters, 1.0001f, 0.5f, 3, 7); break;
+                default: rbe::probe_kernel<3><<<sms, 1024, 0, st>>>(d_cyc, iters, 1.0001f, 0.5f, 3, 7); break;
+            }
+            RBE_CUDA(c, cudaEventRecord(e1, st));
+            RBE_CUDA(c, cudaGetLastError());
+        }
+        RBE_CUDA(c, cudaMemcpyAsync(cyc.data(), d_cyc, cyc.size() * sizeof(long long), cudaMemcpyDeviceToHost, st));
+        RBE_CUDA(c, cudaStreamSynchronize(st));
+        std::sort(cyc.begin(), cyc.end());
+        const double med = (double)cyc[cyc.size() / 2];
+        h_out[mode] = 1024.0 * chains * iters / med;          // lanes (thread-instructions) per SM per clock
+        if (mode == 3) {                                       // the longest kernel: clock = cycles / elapsed time
+            float ms = 0.f;
+            RBE_CUDA(c, cudaEventElapsedTime(&ms, e0, e1));
+            clock_mhz = (double)cyc.back() / (ms * 1e3);
+        }
+    }
+    h_out[4] = clock_mhz;
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    return RBE_OK;
 }
 
 rbe_status rbe_host_alloc(void** out, size_t bytes) {

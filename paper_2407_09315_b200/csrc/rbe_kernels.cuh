@@ -11,7 +11,7 @@
 // scaled so that the FMUL by fl(1/2pi) inside sin.approx/cos.approx lands on turns; MUFU.SIN /
 // MUFU.COS then evaluate sin/cos(2 pi t), |t| <= 1/2.
 //
-// Measured on B200 (csrc/pipe_probe.cu, profiles/): MUFU 16 lanes/SM/clk, IMAD and I2FP 64,
+// Measured on B200 (rbe_probe_pipe_rates, profiles/): MUFU 16 lanes/SM/clk, IMAD and I2FP 64,
 // FFMA 128; a MUFU also costs ~3 issue slots.  Both hot kernels are bound by MUFU + issue.
 #pragma once
 #include <cstdint>
@@ -20,44 +20,20 @@
 namespace rbe {
 
 // ---------------------------------------------------------------------------------------
-// tunables (compile time)
+// tunables (compile time; the values are the measured optima, see profiles/)
 // ---------------------------------------------------------------------------------------
-// (each may be overridden with -DRBE_<NAME>=value when sweeping; the defaults are the tuned ones)
-#ifndef RBE_SF_TMAX
-#define RBE_SF_TMAX 1024
-#endif
-#ifndef RBE_SF_CTAS_PER_SM
-#define RBE_SF_CTAS_PER_SM 1
-#endif
-#ifndef RBE_SF_TILE_MAX
-#define RBE_SF_TILE_MAX 4096
-#endif
-#ifndef RBE_F_THREADS
-#define RBE_F_THREADS 512
-#endif
-#ifndef RBE_F_CTAS_PER_SM
-#define RBE_F_CTAS_PER_SM 2
-#endif
-#ifndef RBE_SF_KPT
-#define RBE_SF_KPT 4
-#endif
-constexpr int SF_KPT = RBE_SF_KPT;   // wavevectors owned by one thread of the structure-factor kernel
-constexpr int SF_TMAX = RBE_SF_TMAX;    // max threads per CTA (structure-factor kernel): <= 64 registers
-constexpr int SF_CTAS_PER_SM = RBE_SF_CTAS_PER_SM;
-constexpr int SF_TILE_MAX = RBE_SF_TILE_MAX; // max atoms staged in shared memory at a time (structure-factor kernel)
-#ifndef RBE_SF_STAGE_UNROLL
-#define RBE_SF_STAGE_UNROLL 4
-#endif
-constexpr int SF_STAGE_UNROLL = RBE_SF_STAGE_UNROLL;   // unroll factor of the two staging loops over 32-atom windows
-constexpr int SF_DEPTH = 64;     // max atoms a thread accumulates in fp32 before the fp64 flush
-constexpr int F_THREADS = RBE_F_THREADS;   // threads per CTA (force kernel)
-constexpr int F_CTAS_PER_SM = RBE_F_CTAS_PER_SM;
+constexpr int SF_KPT = 4;        // wavevectors owned by one thread of the structure-factor phase
+constexpr int SF_TMAX = 1024;    // max threads per CTA (structure-factor / step kernels): <= 64 registers
+constexpr int SF_WPT = 2;        // 32-atom windows a warp stages per tile
+constexpr int SF_TILE_MAX = (SF_TMAX / 32) * SF_WPT * 32;   // atoms per tile (one record arena): 2048
+constexpr int SF_DEPTH = 128;    // max atoms a thread accumulates in fp32 before the fp64 flush
+constexpr int STEP_PMAX = SF_TMAX * SF_KPT;   // largest batch the one-launch step kernel takes (one k-chunk)
+constexpr int STEP_KPARAM_MAX = 512;          // largest batch whose wavevectors ride in the kernel parameters
+constexpr int F_THREADS = 512;   // threads per CTA (force kernel)
+constexpr int F_CTAS_PER_SM = 2;
 constexpr int F_RMAX = 4;        // max atoms per thread per pass (force kernel)
 constexpr int F_KCHUNK = 2048;   // wavevectors staged in shared memory at a time (force kernel)
-#ifndef RBE_SF_RED_GROUP
-#define RBE_SF_RED_GROUP 16
-#endif
-constexpr int SF_RED_GROUP = RBE_SF_RED_GROUP; // CTAs per group in the two-level reduction of the per-CTA rows
+constexpr int SF_RED_GROUP = 16; // CTAs per group in the two-level reduction of the per-CTA rows (two-launch path)
 
 constexpr double TWO32 = 4294967296.0;
 constexpr double MAGIC = 6755399441055744.0;  // 2^52 + 2^51: low word of (d + MAGIC) = rint(d) mod 2^32
@@ -85,12 +61,6 @@ __device__ __forceinline__ float fast_cos(float x) {
     return r;
 }
 __device__ __forceinline__ float phase_to_arg(uint32_t ph, float K) { return (float)(int32_t)ph * K; }
-
-__device__ __forceinline__ void cp_async16(void* smem_dst, const void* gmem_src) {
-    const uint32_t d = (uint32_t)__cvta_generic_to_shared(smem_dst);
-    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(d), "l"(gmem_src) : "memory");
-}
-__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
 
 // Programmatic dependent launch (PDL): the force kernel may start while the structure-factor
 // kernel drains; it waits here before touching anything that kernel writes.
@@ -176,6 +146,10 @@ struct KTable {
 
 __device__ __forceinline__ double2 k_rho(const KTable& t, int k) {
     if (t.xch.world < 1) return t.rho[k];
+    if (*reinterpret_cast<volatile const int32_t*>(t.xch.error)) {   // a peer never arrived: poison, do not pass silently
+        const double nan = __longlong_as_double(0x7ff8000000000000ll);
+        return make_double2(nan, nan);
+    }
     double re = 0.0, im = 0.0;
     for (int r = 0; r < t.xch.world; ++r) {
         const double2 v = __ldcg(&t.xch.slots[(int64_t)r * t.P + k]);   // written by a peer: not through L1
@@ -184,17 +158,33 @@ __device__ __forceinline__ double2 k_rho(const KTable& t, int k) {
     return make_double2(re, im);
 }
 
-__device__ __forceinline__ void k_record(const KTable& t, int k, int4& ka, float4& kb) {
-    const int4 m = t.kvec[k];
-    const double2 r = k_rho(t, k);
-    const double w = t.w ? t.w[k] : t.w_uniform;
+__device__ __forceinline__ void k_record_from(int4 m, double2 r, double w, double L, int4& ka, float4& kb) {
     const double m2 = (double)m.x * m.x + (double)m.y * m.y + (double)m.z * m.z;
     const double mag = sqrt(r.x * r.x + r.y * r.y);
     const double theta = atan2(r.y, r.x) * (1.0 / (2.0 * PI_D));      // turns, [-1/2, 1/2]
-    const double gs = -2.0 * w / (t.L * t.L * m2) * mag;
-    const double el = w / (2.0 * PI_D * t.L * m2);
+    const double gs = -2.0 * w / (L * L * m2) * mag;
+    const double el = w / (2.0 * PI_D * L * m2);
     ka = make_int4(-m.x, -m.y, -m.z, __double2loint(fma(theta, TWO32, MAGIC)));   // {-m, theta in 2^-32 turns}
     kb = make_float4((float)(gs * m.x), (float)(gs * m.y), (float)(gs * m.z), (float)(el * mag));  // {G, e_l |rho_l|}
+}
+// The same record with |rho| and arg rho taken in fp32 (sqrtf, atan2f: ~1e-7 relative, far inside the 2e-5
+// force tolerance; the products around them stay fp64).  The step kernel builds every record on its critical
+// path between two grid barriers, where the fp64 atan2 chain alone costs over a microsecond.
+__device__ __forceinline__ void k_record_fast(int4 m, double2 r, double w, double L, int4& ka, float4& kb) {
+    const double m2 = (double)m.x * m.x + (double)m.y * m.y + (double)m.z * m.z;
+    // scale first: |rho|^2 of a large system overflows nothing in fp32, but tiny ones would underflow
+    const double big = fmax(fabs(r.x), fabs(r.y));
+    const double inv = big > 0.0 ? 1.0 / big : 0.0;
+    const float xr = (float)(r.x * inv), yr = (float)(r.y * inv);
+    const double mag = big * (double)sqrtf(fmaf(xr, xr, yr * yr));
+    const double theta = (double)atan2f(yr, xr) * (1.0 / (2.0 * PI_D));   // turns, [-1/2, 1/2]
+    const double gs = -2.0 * w / (L * L * m2) * mag;
+    const double el = w / (2.0 * PI_D * L * m2);
+    ka = make_int4(-m.x, -m.y, -m.z, __double2loint(fma(theta, TWO32, MAGIC)));
+    kb = make_float4((float)(gs * m.x), (float)(gs * m.y), (float)(gs * m.z), (float)(el * mag));
+}
+__device__ __forceinline__ void k_record(const KTable& t, int k, int4& ka, float4& kb) {
+    k_record_from(t.kvec[k], k_rho(t, k), t.w ? t.w[k] : t.w_uniform, t.L, ka, kb);
 }
 
 // U = sum_l e_l |rho_l|^2 in a fixed order (thread-strided partials, then a fixed tree).
@@ -297,55 +287,46 @@ __device__ __forceinline__ void reduce_rows(const double2* src, int nrows, int P
 }
 
 // ---------------------------------------------------------------------------------------
-// SF kernel -- Algorithm 1 steps 2+3 fused, Eq. (2.9) P:117.
+// SF phase -- Algorithm 1 steps 2+3 fused, Eq. (2.9) P:117.  Shared by the two-launch
+// structure-factor kernel (sf_kernel) and the one-launch step kernel (step_kernel).
 //
 // Mapping: a thread OWNS SF_KPT wavevectors (their m in registers) and one of `ng` atom
-// groups.  The CTA streams its contiguous atom range through shared memory in tiles of
-// blockDim.x atoms (cp.async prefetch of the raw float4 records); the N x P array of Fourier
-// modes the paper materialises before its Reduce-by-Key never exists, and there is no
-// cross-lane reduction: each thread sums its own (cos, sin) in fp32 over at most ~SF_DEPTH
-// atoms, then in fp64 (shared-memory accumulators).  Groups are combined in group order and
-// one fp64 row of P complex partials per CTA goes to global memory.  No atomics on data.
+// groups.  The CTA walks its contiguous atom range in tiles of nwarps * SF_WPT windows of 32 atoms;
+// the N x P array of Fourier modes the paper materialises before its Reduce-by-Key never
+// exists, and there is no cross-lane reduction: each thread sums its own (cos, sin) in fp32 over at
+// most ~SF_DEPTH atoms, then in fp64 (shared-memory accumulators).  Groups are combined in group
+// order and one fp64 row of P complex partials per CTA goes to global memory.  No atomics on data.
 //
-// Equal-|q| pairing (what makes this kernel 3 MUFU per TWO pairs instead of 4).  For two atoms
+// Equal-|q| pairing (what makes this phase 3 MUFU per TWO pairs instead of 4).  For two atoms
 // with q_2 = +-q_1 and turns S_1, S_2 let S_d = (S_1 - S_2)/2, S_a = S_2 + S_d.  Then exactly
 //   q_1 e^{i phi_1} + q_2 e^{i phi_2} = 2 q_1 cos(2 pi m.S_d - o) e^{i (2 pi m.S_a + o)},
 // o = 0 for equal charges, a quarter turn for opposite ones (2i sin d = 2 cos(d - pi/2) e^{i pi/2}).
-// While staging a tile each warp matches the 32 atoms of its window by |q| bit pattern
-// (MATCH.ANY) and emits pair records {S_a, o}{S_d, 2 q_1} and single records {S, q} for the
-// leftovers, so ANY charge assignment is handled (all-distinct charges fall back to 2 MUFU per
-// pair).  MD systems have a handful of distinct charge magnitudes, so nearly all atoms pair up.
-// Compaction of the records is by warp counts + a prefix scan: deterministic order.
+// Staging a tile, each warp matches the 32 atoms of a window by |q| bit pattern (MATCH.ANY) and
+// emits pair records {S_a, o}{S_d, 2 q_1} and single records {S, q} for the leftovers, so ANY charge
+// assignment is handled (all-distinct charges fall back to 2 MUFU per pair).  MD systems have a
+// handful of distinct charge magnitudes, so nearly all atoms pair up.
 //
-// The last CTAs to finish (atomicInc tickets; data order never depends on them) run the second
-// pass: the fixed-order two-level sum of the per-CTA rows into rho (reduce_rows), and, with a
-// multi-GPU exchange configured, the push of rho into every rank's exchange buffer.
+// Staging is warp-local and overlapped.  A warp loads its SF_WPT windows of the NEXT tile straight
+// from global memory into registers (lane = atom: one coalesced 512-byte request per window; no raw
+// tile in shared memory, no cp.async), classifies and converts them and writes the records into the
+// other half of a double-buffered record arena.  It does so in the middle of its accumulation loop
+// over the CURRENT tile, at a point that depends on the warp index, so that at any moment about one
+// warp per SM is staging (and waiting on HBM) while the other 31 keep the MUFU pipe busy.  Record
+// positions are the exclusive prefix over the warps' counts (published through shared-memory flags;
+// a warp only ever waits for warps that staged earlier), so the record order -- and with it every
+// floating-point sum -- is deterministic.  One __syncthreads per tile.
 // ---------------------------------------------------------------------------------------
-struct SfParams {
+struct SfArgs {
     const float4* xyzq;
     int64_t N;
-    const int4* kvec;  // [P] {mx, my, mz, 0}
-    double2* part;     // [gridDim.x][P]
+    double2* part;     // [gridDim.x][P] per-CTA rows
     double two32_over_L;
     int32_t P;
     int32_t gs;        // threads per atom group in this CTA = k-slots / SF_KPT
     int32_t ng;        // atom groups per CTA
-    int32_t tile_atoms;   // atoms staged per tile: a multiple of 32, <= SF_TILE_MAX
-    int32_t flush_every;  // tiles between fp64 flushes (keeps the fp32 depth <= ~SF_DEPTH atoms)
-    int32_t pairing;      // bit 0: pair equal charges, bit 1: pair opposite charges (3 = both)
+    int32_t pairing;   // bit 0: pair equal charges, bit 1: pair opposite charges (3 = both)
     int32_t accumulate;   // add this launch's per-CTA rows to what `part` holds (chunked host step: one launch per chunk)
-    int32_t finalise;     // run the second pass (rows -> rho) at the end of this launch
-    RedParams red;
-#ifdef RBE_SF_PROFILE
-    long long* prof;      // [gridDim.x][64] globaltimer stamps of thread 0 (sweep builds only)
-#endif
 };
-
-#ifdef RBE_SF_PROFILE
-#define RBE_STAMP() do { if (tid == 0 && prof_n < 64) { long long t_; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t_)); p.prof[blockIdx.x * 64 + prof_n++] = t_; } } while (0)
-#else
-#define RBE_STAMP() do { } while (0)
-#endif
 
 // acc points at this thread's slot of component 0; component r lives `stride` entries further
 // (layout [SF_KPT][blockDim.x]: conflict-free).
@@ -382,154 +363,162 @@ __device__ __forceinline__ SfWindow sf_classify(uint32_t qbits, bool in_range, i
     return w;
 }
 
+// Shared-memory control words of the staging protocol (one set per CTA).
+struct SfCtl {
+    volatile uint32_t cnt[32];    // per warp: pair records | single records << 16 of the tile being staged
+    volatile uint32_t flag[32];   // per warp: sequence number (tile index + 1) of the tile whose counts are published
+    uint32_t tot[2];              // per arena half: total pair | single << 16 records of the tile
+};
+
+// Stage this warp's SF_WPT windows of one tile: atoms [a0, a0 + 32 * SF_WPT) clipped to `hi`.  All 32 lanes.
+// FIRST: the tile every warp stages at once when the kernel starts -- the counts meet at a __syncthreads
+// (called by ALL threads of the CTA); otherwise through the per-warp flags (a warp stages tile t + 1 in the
+// middle of its loop over tile t and waits only for warps whose turn came earlier).
+template <bool FIRST>
+__device__ __forceinline__ void sf_stage(const SfArgs& p, int64_t a0, int64_t hi, int warp, int lane, int nwarps, uint4* A,
+                                         SfCtl& ctl, uint32_t* tot, uint32_t seq) {
+    const uint32_t lt_mask = (1u << lane) - 1u;
+    float4 a[SF_WPT];
+    SfWindow cw[SF_WPT];
+    uint32_t mine = 0;    // this warp's pair | single << 16 counts
+#pragma unroll
+    for (int j = 0; j < SF_WPT; ++j) {
+        const int64_t i = a0 + j * 32 + lane;
+        a[j] = i < hi ? __ldg(&p.xyzq[i]) : make_float4(0.f, 0.f, 0.f, 0.f);
+    }
+#pragma unroll
+    for (int j = 0; j < SF_WPT; ++j) {
+        cw[j] = sf_classify(__float_as_uint(a[j].w), a0 + j * 32 + lane < hi, p.pairing, lane);
+        mine += (uint32_t)__popc(cw[j].lmask) | ((uint32_t)__popc(cw[j].smask) << 16);
+    }
+    // publish the counts, then take the exclusive prefix over the warps before this one
+    uint32_t base = 0;
+    if (FIRST) {
+        if (lane == 0) ctl.cnt[warp] = mine;
+        __syncthreads();
+        if (lane < warp) base = ctl.cnt[lane];
+    } else {
+        if (lane == 0) {
+            ctl.cnt[warp] = mine;
+            __threadfence_block();
+            ctl.flag[warp] = seq;
+        }
+        if (lane < warp) {
+            while (ctl.flag[lane] != seq) __nanosleep(40);
+            __threadfence_block();
+            base = ctl.cnt[lane];
+        }
+    }
+#pragma unroll
+    for (int d = 16; d > 0; d >>= 1) base += __shfl_xor_sync(FULL_MASK, base, d);   // fields cannot carry: <= 2048 each
+    if (warp == nwarps - 1 && lane == 0) *tot = base + mine;
+    uint32_t bp = base & 0xffffu, bs = base >> 16;
+#pragma unroll
+    for (int j = 0; j < SF_WPT; ++j) {
+        const uint32_t Sx = to_turns(a[j].x, p.two32_over_L);
+        const uint32_t Sy = to_turns(a[j].y, p.two32_over_L);
+        const uint32_t Sz = to_turns(a[j].z, p.two32_over_L);
+        const uint32_t Px = __shfl_sync(FULL_MASK, Sx, cw[j].partner);
+        const uint32_t Py = __shfl_sync(FULL_MASK, Sy, cw[j].partner);
+        const uint32_t Pz = __shfl_sync(FULL_MASK, Sz, cw[j].partner);
+        const uint32_t Pq = __shfl_sync(FULL_MASK, __float_as_uint(a[j].w), cw[j].partner);
+        if (cw[j].leader) {
+            // S_d = (S_1 - S_2) / 2 (arithmetic shift of the wrapped difference), S_a = S_2 + S_d
+            const uint32_t e = bp + (uint32_t)__popc(cw[j].lmask & lt_mask);
+            const uint32_t dx = (uint32_t)((int32_t)(Sx - Px) >> 1);
+            const uint32_t dy = (uint32_t)((int32_t)(Sy - Py) >> 1);
+            const uint32_t dz = (uint32_t)((int32_t)(Sz - Pz) >> 1);
+            // o: a quarter turn for opposite charges; plus half a turn on every other pair, which leaves
+            // cos(d - o) e^{i(a + o)} unchanged but alternates the sign of the evaluated amplitude, so
+            // the +1.7e-8 mean error of MUFU.COS (measured) cannot add up coherently over the pairs
+            // (for single atoms it cancels by neutrality; the sum of pair amplitudes is not neutral)
+            const uint32_t off = (((__float_as_uint(a[j].w) ^ Pq) >> 31) ? QUARTER_TURN : 0u) + (e << 31);
+            A[2 * e] = make_uint4(Px + dx, Py + dy, Pz + dz, off);
+            A[2 * e + 1] = make_uint4(dx, dy, dz, __float_as_uint(2.0f * a[j].w));
+        } else if (cw[j].single) {
+            const uint32_t e = bs + (uint32_t)__popc(cw[j].smask & lt_mask);
+            A[SF_TILE_MAX - 1 - e] = make_uint4(Sx, Sy, Sz, __float_as_uint(a[j].w));   // singles from the back
+        }
+        bp += (uint32_t)__popc(cw[j].lmask);
+        bs += (uint32_t)__popc(cw[j].smask);
+    }
+}
+
+// Shared-memory footprint of the SF phase: two record arenas + the fp64 accumulators [SF_KPT][threads].
+__host__ __device__ constexpr size_t sf_smem_bytes(int threads) {
+    return (size_t)2 * SF_TILE_MAX * sizeof(uint4) + (size_t)threads * SF_KPT * sizeof(double2);
+}
+
+// The accumulation over this CTA's atoms.  On return the fp64 accumulators in shared memory hold every
+// thread's sums (call sf_write_row next).  bx / gx: this CTA's index among the CTAs that share the atoms.
 template <bool DEEP>
-__global__ void __launch_bounds__(SF_TMAX, SF_CTAS_PER_SM) sf_kernel(const SfParams p) {
-    extern __shared__ __align__(16) unsigned char smem_raw[];
+__device__ __forceinline__ void sf_accumulate(const SfArgs& p, const int (&mx)[SF_KPT], const int (&my)[SF_KPT],
+                                              const int (&mz)[SF_KPT], unsigned char* smem_raw, SfCtl& ctl, int bx, int gx) {
     const int tid = threadIdx.x, T = blockDim.x, lane = tid & 31, warp = tid >> 5, nwarps = T >> 5;
-    const int TA = p.tile_atoms;                                      // multiple of 32, <= SF_TILE_MAX
-    float4* raw = reinterpret_cast<float4*>(smem_raw);               // [TA] raw atom records of the tile
-    uint4* arena = reinterpret_cast<uint4*>(smem_raw) + TA;          // [TA] pair records from the front, singles from the back
-    double2* acc_all = reinterpret_cast<double2*>(arena + TA);       // [SF_KPT][T] fp64 accumulators
-    constexpr int WIN_MAX = 128;   // the one-warp scan below covers 4 windows per lane
-    static_assert(SF_TILE_MAX / 32 <= WIN_MAX, "tile too large for the window scan");
-    __shared__ uint32_t wcount[WIN_MAX], wbase[WIN_MAX + 1];
-    __shared__ uint16_t roles[SF_TILE_MAX];
-    __shared__ uint32_t s_last;
+    uint4* arena = reinterpret_cast<uint4*>(smem_raw);                           // [2][SF_TILE_MAX] records
+    double2* acc_all = reinterpret_cast<double2*>(arena + 2 * SF_TILE_MAX);      // [SF_KPT][T] fp64 accumulators
+    // this CTA's atom range, aligned to 32-atom windows, in tiles of nwarps * SF_WPT windows
+    const int64_t units = (p.N + 31) >> 5;
+    const int64_t lo = (units * bx / gx) << 5;
+    int64_t hi = (units * (bx + 1) / gx) << 5;
+    if (hi > p.N) hi = p.N;
+    const int tile_atoms = nwarps * SF_WPT * 32;
+    const int ntiles = hi > lo ? (int)((hi - lo + tile_atoms - 1) / tile_atoms) : 0;
+    // tile 0 first: its loads are the longest latency of the prologue (every thread calls: it has a barrier inside)
+    sf_stage<true>(p, lo + (int64_t)warp * (SF_WPT * 32), hi, warp, lane, nwarps, arena, ctl, &ctl.tot[0], 1u);
 
     const bool active = tid < p.gs * p.ng;
-    const int g = active ? tid / p.gs : (1 << 28);  // inactive threads: group index past every list -> empty loops
-    const int j = active ? tid % p.gs : 0;
-    const int kbase = (blockIdx.y * p.gs + j) * SF_KPT;
+    const int g = active ? tid / p.gs : (1 << 28);  // inactive threads: cursor past every list -> empty loops
     double2* acc = acc_all + tid;
-
-    int mx[SF_KPT], my[SF_KPT], mz[SF_KPT];
     float c[SF_KPT], s[SF_KPT];
 #pragma unroll
     for (int r = 0; r < SF_KPT; ++r) {
-        int4 m = make_int4(0, 0, 0, 0);
-        if (active && kbase + r < p.P) m = __ldg(&p.kvec[kbase + r]);
-        mx[r] = m.x; my[r] = m.y; mz[r] = m.z;
         c[r] = s[r] = 0.f;
         acc[r * T] = make_double2(0.0, 0.0);
     }
-
-    // this CTA's atom range, aligned to 32-atom windows
-    const int64_t units = (p.N + 31) >> 5;
-    const int64_t lo = (units * blockIdx.x / gridDim.x) << 5;
-    int64_t hi = (units * (blockIdx.x + 1) / gridDim.x) << 5;
-    if (hi > p.N) hi = p.N;
+    if (tid < 32) ctl.flag[tid] = 0u;
     const float K = phase_scale();
-    const uint32_t lt_mask = (1u << lane) - 1u;
+    __syncthreads();   // records of tile 0, tot[0], zeroed flags and accumulators                           // @stamp
 
-    // a short first tile gets the MUFU-bound loop going early; later tiles are full size
-    int tl = (TA >> 7) << 5;
-    if (tl < 32) tl = 32;
-    for (int i = tid; i < tl && lo + i < hi; i += T) cp_async16(&raw[i], &p.xyzq[lo + i]);
-    int since_flush = 0;
-#ifdef RBE_SF_PROFILE
-    int prof_n = 0;
-#endif
-    RBE_STAMP();
-
-    for (int64_t t0 = lo; t0 < hi; t0 += tl, tl = TA) {
-        const int cnt = (int)((hi - t0 < tl) ? (hi - t0) : tl);
-        const int nwin = (cnt + 31) >> 5;
-        cp_async_wait_all();
-        __syncthreads();  // raw holds the tile; everyone is done with the previous arena
-        RBE_STAMP();
-
-        // ---- stage 1: per window (one warp each), classify by charge and count the records
-#pragma unroll SF_STAGE_UNROLL
-        for (int w = warp; w < nwin; w += nwarps) {
-            const int idx = (w << 5) + lane;
-            const uint32_t qb = idx < cnt ? __float_as_uint(raw[idx].w) : 0u;
-            const SfWindow cw = sf_classify(qb, idx < cnt, p.pairing, lane);
-            // role word: bits 0-4 partner lane, bit 5 leader, bit 6 single, bits 8.. index in the window's list
-            roles[idx] = (uint16_t)(cw.partner | (cw.leader ? 32 : 0) | (cw.single ? 64 : 0) |
-                                    (__popc((cw.leader ? cw.lmask : cw.smask) & lt_mask) << 8));
-            if (lane == 0) wcount[w] = (uint32_t)__popc(cw.lmask) | ((uint32_t)__popc(cw.smask) << 16);
-        }
-        __syncthreads();
-        // exclusive scan of the window counts (<= SF_TILE_MAX/32 = 128 of them) by one warp: record positions
-        if (warp == 0) {
-            uint32_t v[4], run = 0;
-#pragma unroll
-            for (int i = 0; i < 4; ++i) { v[i] = (4 * lane + i < nwin) ? wcount[4 * lane + i] : 0u; run += v[i]; }
-            uint32_t incl = run;
-#pragma unroll
-            for (int d = 1; d < 32; d <<= 1) {
-                const uint32_t n = __shfl_up_sync(FULL_MASK, incl, d);
-                if (lane >= d) incl += n;
-            }
-            uint32_t ex = incl - run;
-#pragma unroll
-            for (int i = 0; i < 4; ++i) { wbase[4 * lane + i] = ex; ex += v[i]; }
-            if (lane == 31) wbase[WIN_MAX] = incl;
-        }
-        __syncthreads();
-        const uint32_t total = wbase[WIN_MAX];
+    int ep = g, es = g;    // round-robin cursors into the pair / single lists, carried across tiles
+    int depth = 0;
+#pragma unroll 1
+    for (int t = 0; t < ntiles; ++t) {
+        const int buf = t & 1;
+        const uint4* A = arena + buf * SF_TILE_MAX;
+        const uint32_t total = ctl.tot[buf];
         const int np = (int)(total & 0xffffu), ns = (int)(total >> 16);
-
-        // ---- stage 2: convert to turns and write the records at their scanned positions
-#pragma unroll SF_STAGE_UNROLL
-        for (int w = warp; w < nwin; w += nwarps) {
-            const int idx = (w << 5) + lane;
-            const uint32_t base = wbase[w];
-            const float4 a = idx < cnt ? raw[idx] : make_float4(0.f, 0.f, 0.f, 0.f);
-            const uint32_t role = roles[idx];
-            const int partner = role & 31, e_in = role >> 8;
-            const uint32_t Sx = to_turns(a.x, p.two32_over_L);
-            const uint32_t Sy = to_turns(a.y, p.two32_over_L);
-            const uint32_t Sz = to_turns(a.z, p.two32_over_L);
-            const uint32_t Px = __shfl_sync(FULL_MASK, Sx, partner);
-            const uint32_t Py = __shfl_sync(FULL_MASK, Sy, partner);
-            const uint32_t Pz = __shfl_sync(FULL_MASK, Sz, partner);
-            const uint32_t Pq = __shfl_sync(FULL_MASK, __float_as_uint(a.w), partner);
-            if (role & 32) {
-                // S_d = (S_1 - S_2) / 2 (arithmetic shift of the wrapped difference), S_a = S_2 + S_d
-                const int e = (int)(base & 0xffffu) + e_in;
-                const uint32_t dx = (uint32_t)((int32_t)(Sx - Px) >> 1);
-                const uint32_t dy = (uint32_t)((int32_t)(Sy - Py) >> 1);
-                const uint32_t dz = (uint32_t)((int32_t)(Sz - Pz) >> 1);
-                // o: a quarter turn for opposite charges; plus half a turn on every other pair, which leaves
-                // cos(d - o) e^{i(a + o)} unchanged but alternates the sign of the evaluated amplitude, so
-                // the +1.7e-8 mean error of MUFU.COS (measured) cannot add up coherently over the pairs
-                // (for single atoms it cancels by neutrality; the sum of pair amplitudes is not neutral)
-                const uint32_t off = (((__float_as_uint(a.w) ^ Pq) >> 31) ? QUARTER_TURN : 0u) + ((uint32_t)e << 31);
-                arena[2 * e] = make_uint4(Px + dx, Py + dy, Pz + dz, off);
-                arena[2 * e + 1] = make_uint4(dx, dy, dz, __float_as_uint(2.0f * a.w));
-            } else if (role & 64) {
-                const int e = (int)(base >> 16) + e_in;
-                arena[TA - 1 - e] = make_uint4(Sx, Sy, Sz, __float_as_uint(a.w));
-            }
-        }
-        __syncthreads();  // records visible; raw fully consumed
-        RBE_STAMP();
-
-        // prefetch the next tile while this one is processed
-        for (int i = tid; i < TA && t0 + tl + i < hi; i += T) cp_async16(&raw[i], &p.xyzq[t0 + tl + i]);
-
-        // ---- accumulate: pair records g, g+ng, ... then single records g, g+ng, ...
-        int depth = 0;
+        const bool more = t + 1 < ntiles;
+        // this warp stages its windows of tile t + 1 after the first `split` pair records of tile t: the
+        // warps take turns over the first three quarters of the tile
+        const int split = more ? (np * 3 * warp) / (4 * nwarps) : np;
 #pragma unroll 1
-        for (int e = g; e < np; e += p.ng) {
-            const uint4 ra = arena[2 * e];
-            const uint4 rd = arena[2 * e + 1];
-            const float w2 = __uint_as_float(rd.w);
+        for (int part = 0; part < 2; ++part) {
+            const int end = part == 0 ? split : np;
+#pragma unroll 1
+            for (; ep < end; ep += p.ng) {
+                const uint4 ra = A[2 * ep];
+                const uint4 rd = A[2 * ep + 1];
+                const float w2 = __uint_as_float(rd.w);
 #pragma unroll
-            for (int r = 0; r < SF_KPT; ++r) {
-                const uint32_t pa = (uint32_t)mx[r] * ra.x + ((uint32_t)my[r] * ra.y + ((uint32_t)mz[r] * ra.z + ra.w));
-                const uint32_t pd = (uint32_t)mx[r] * rd.x + ((uint32_t)my[r] * rd.y + ((uint32_t)mz[r] * rd.z - ra.w));
-                const float xa = phase_to_arg(pa, K);
-                const float amp = w2 * fast_cos(phase_to_arg(pd, K));
-                c[r] = fmaf(amp, fast_cos(xa), c[r]);
-                s[r] = fmaf(amp, fast_sin(xa), s[r]);
+                for (int r = 0; r < SF_KPT; ++r) {
+                    const uint32_t pa = (uint32_t)mx[r] * ra.x + ((uint32_t)my[r] * ra.y + ((uint32_t)mz[r] * ra.z + ra.w));
+                    const uint32_t pd = (uint32_t)mx[r] * rd.x + ((uint32_t)my[r] * rd.y + ((uint32_t)mz[r] * rd.z - ra.w));
+                    const float xa = phase_to_arg(pa, K);
+                    const float amp = w2 * fast_cos(phase_to_arg(pd, K));
+                    c[r] = fmaf(amp, fast_cos(xa), c[r]);
+                    s[r] = fmaf(amp, fast_sin(xa), s[r]);
+                }
+                if (DEEP) { depth += 2; if (depth >= SF_DEPTH) { sf_flush(acc, T, c, s); depth = 0; } }
             }
-            if (DEEP) { depth += 2; if (depth >= SF_DEPTH) { sf_flush(acc, T, c, s); depth = 0; } }
+            if (part == 0 && more)
+                sf_stage<false>(p, lo + (int64_t)(t + 1) * tile_atoms + (int64_t)warp * (SF_WPT * 32), hi, warp, lane, nwarps,
+                                arena + (buf ^ 1) * SF_TILE_MAX, ctl, &ctl.tot[buf ^ 1], (uint32_t)t + 2u);
         }
+        ep -= np;
 #pragma unroll 1
-        for (int e = g; e < ns; e += p.ng) {
-            const uint4 at = arena[TA - 1 - e];
+        for (; es < ns; es += p.ng) {
+            const uint4 at = A[SF_TILE_MAX - 1 - es];
             const float q = __uint_as_float(at.w);
 #pragma unroll
             for (int r = 0; r < SF_KPT; ++r) {
@@ -540,33 +529,71 @@ __global__ void __launch_bounds__(SF_TMAX, SF_CTAS_PER_SM) sf_kernel(const SfPar
             }
             if (DEEP) { depth += 1; if (depth >= SF_DEPTH) { sf_flush(acc, T, c, s); depth = 0; } }
         }
-        if (++since_flush >= p.flush_every) { sf_flush(acc, T, c, s); since_flush = 0; }
+        es -= ns;
+        if (!DEEP) sf_flush(acc, T, c, s);   // a thread takes at most SF_DEPTH atoms from one tile
+        __syncthreads();   // tile t is consumed (its arena half may be overwritten), tile t + 1 is staged   // @stamp
     }
-    sf_flush(acc, T, c, s);
-    RBE_STAMP();
-
-    // let the dependent (force) kernel start launching; it waits for this grid's completion
-    grid_launch_dependents();
-
-    // combine the atom groups in group order, one fp64 row per CTA
-    const int kslots = p.gs * SF_KPT;
+    if (DEEP) sf_flush(acc, T, c, s);
     __syncthreads();
+}
+
+// Combine the atom groups in group order: one fp64 row of this CTA's k-slots.  by: k-chunk index.
+__device__ __forceinline__ void sf_write_row(const SfArgs& p, unsigned char* smem_raw, int bx, int by) {
+    const int tid = threadIdx.x, T = blockDim.x;
+    const double2* acc_all = reinterpret_cast<const double2*>(reinterpret_cast<uint4*>(smem_raw) + 2 * SF_TILE_MAX);
+    const int kslots = p.gs * SF_KPT;
     for (int idx = tid; idx < kslots; idx += T) {
-        const int k = blockIdx.y * kslots + idx;
+        const int k = by * kslots + idx;
         if (k < p.P) {
             double re = 0.0, im = 0.0;
             for (int gg = 0; gg < p.ng; ++gg) {
                 const double2 v = acc_all[(idx % SF_KPT) * T + gg * p.gs + idx / SF_KPT];
                 re += v.x; im += v.y;
             }
-            double2* row = &p.part[(int64_t)blockIdx.x * p.P + k];
+            double2* row = &p.part[(int64_t)bx * p.P + k];
             if (p.accumulate) { const double2 old = *row; re += old.x; im += old.y; }   // chunks arrive in stream order
             *row = make_double2(re, im);
         }
     }
+}
+
+// ---------------------------------------------------------------------------------------
+// sf_kernel -- the structure factors as their own launch (rbe_structure_factor; the chunked host
+// step; the multi-GPU exchange).  The last CTAs to finish (atomicInc tickets; data order never
+// depends on them) run the second pass: the fixed-order two-level sum of the per-CTA rows into rho
+// (reduce_rows), and, with a multi-GPU exchange configured, the push of rho into every rank's buffer.
+// ---------------------------------------------------------------------------------------
+struct SfParams {
+    SfArgs a;
+    const int4* kvec;  // [P] {mx, my, mz, 0}
+    int32_t finalise;  // run the second pass (rows -> rho) at the end of this launch
+    RedParams red;
+};
+
+template <bool DEEP>
+__global__ void __launch_bounds__(SF_TMAX, 1) sf_kernel(const SfParams p) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    __shared__ SfCtl ctl;
+    __shared__ uint32_t s_last;
+    const int tid = threadIdx.x, T = blockDim.x;
+    const bool active = tid < p.a.gs * p.a.ng;
+    const int kbase = (blockIdx.y * p.a.gs + (active ? tid % p.a.gs : 0)) * SF_KPT;
+    int mx[SF_KPT], my[SF_KPT], mz[SF_KPT];
+#pragma unroll
+    for (int r = 0; r < SF_KPT; ++r) {
+        int4 m = make_int4(0, 0, 0, 0);
+        if (active && kbase + r < p.a.P) m = __ldg(&p.kvec[kbase + r]);
+        mx[r] = m.x; my[r] = m.y; mz[r] = m.z;
+    }
+    sf_accumulate<DEEP>(p.a, mx, my, mz, smem_raw, ctl, blockIdx.x, gridDim.x);
+
+    // let the dependent (force) kernel start launching; it waits for this grid's completion
+    grid_launch_dependents();
+    sf_write_row(p.a, smem_raw, blockIdx.x, blockIdx.y);
     if (!p.finalise) return;
 
     // ---- second pass: the last CTA of each group sums the group, the last group sums the groups
+    double2* scratch = reinterpret_cast<double2*>(reinterpret_cast<uint4*>(smem_raw) + 2 * SF_TILE_MAX);
     const RedParams& rp = p.red;
     const int grp = blockIdx.x / rp.group_size, first = grp * rp.group_size;
     const int members = ((int)gridDim.x - first < rp.group_size) ? (int)gridDim.x - first : rp.group_size;
@@ -578,9 +605,8 @@ __global__ void __launch_bounds__(SF_TMAX, SF_CTAS_PER_SM) sf_kernel(const SfPar
         __threadfence();
     }
     __syncthreads();
-    RBE_STAMP();
     if (!s_last) return;
-    reduce_rows(rp.part + (int64_t)first * p.P, members, p.P, rp.grow + (int64_t)grp * p.P, nullptr, acc_all, tid, T);
+    reduce_rows(rp.part + (int64_t)first * p.a.P, members, p.a.P, rp.grow + (int64_t)grp * p.a.P, nullptr, scratch, tid, T);
     __syncthreads();
     if (tid == 0) {
         __threadfence();
@@ -589,15 +615,13 @@ __global__ void __launch_bounds__(SF_TMAX, SF_CTAS_PER_SM) sf_kernel(const SfPar
     }
     __syncthreads();
     if (!s_last) return;
-    RBE_STAMP();
-    reduce_rows(rp.grow, rp.ngroups, p.P, rp.rho, rp.rho_user, acc_all, tid, T);
-    RBE_STAMP();
+    reduce_rows(rp.grow, rp.ngroups, p.a.P, rp.rho, rp.rho_user, scratch, tid, T);
     if (rp.xch.world > 0) {
         // fused exchange: this CTA (the last one of the grid) writes the partial rho into its slot on
         // every rank over NVLink, then releases the per-rank flags (stores, fence, flag)
         __syncthreads();
         for (int r = 0; r < rp.xch.world; ++r)
-            for (int k = tid; k < p.P; k += T) rp.xch.slot[r][k] = __ldcg(&rp.rho[k]);
+            for (int k = tid; k < p.a.P; k += T) rp.xch.slot[r][k] = __ldcg(&rp.rho[k]);
         __threadfence_system();
         __syncthreads();
         if (tid < rp.xch.world) st_release_sys(rp.xch.flag[tid], rp.xch.epoch);
@@ -605,7 +629,7 @@ __global__ void __launch_bounds__(SF_TMAX, SF_CTAS_PER_SM) sf_kernel(const SfPar
 }
 
 // ---------------------------------------------------------------------------------------
-// F kernel -- Algorithm 1 step 4, Eq. (2.12) P:131.
+// F phase -- Algorithm 1 step 4, Eq. (2.12) P:131.  Shared by f_kernel and step_kernel.
 //
 // Mapping: a thread owns R atoms (coordinates as fixed-point turns in registers) and loops
 // over the wavevectors, whose {-m, theta} and {G, E} records are broadcast from shared memory.
@@ -614,39 +638,34 @@ __global__ void __launch_bounds__(SF_TMAX, SF_CTAS_PER_SM) sf_kernel(const SfPar
 // same number of (atom, k) pairs to within one unit.
 // Per pair: 3 IMAD (phase), I2FP, 2 FMUL, 1 MUFU.SIN, 3 FFMA (+ MUFU.COS, FFMA with energy).
 // ---------------------------------------------------------------------------------------
-struct FParams {
+struct FArgs {
     const float4* xyzq;
     float4* force;
     int64_t N;
-    KTable kt;     // rho and the k-set: every CTA builds its {-m, theta}, {G, E} records from these
     double two32_over_L;
-    int32_t P;
-    int32_t pdl;   // launched with programmatic stream serialisation: wait before reading rho
 };
 
-__device__ __forceinline__ float4 f_fetch(const FParams& p, int64_t unit, int lane) {
+__device__ __forceinline__ float4 f_fetch(const FArgs& p, int64_t unit, int lane) {
     const int64_t i = unit * 32 + lane;
     return i < p.N ? __ldg(&p.xyzq[i]) : make_float4(0.f, 0.f, 0.f, 0.f);
 }
 
 // One pass: R units (R atoms per thread) against the nk wavevector records in shared memory.
-// `pre` != nullptr: the atom records were fetched earlier (prologue overlap), else fetch here.
 template <int R, bool ENERGY, bool ACCUM>
-__device__ __forceinline__ void f_pass(const FParams& p, const int4* s_ka, const float4* s_kb, int nk, int64_t unit0,
-                                       int lane, const float4* pre) {
+__device__ __forceinline__ void f_pass(const FArgs& p, const int4* s_ka, const float4* s_kb, int nk, int64_t unit0, int lane) {
     uint32_t sx[R], sy[R], sz[R];
     float q[R], fx[R], fy[R], fz[R], en[R];
     const float K = phase_scale();
 #pragma unroll
     for (int r = 0; r < R; ++r) {
-        const float4 a = pre ? pre[r] : f_fetch(p, unit0 + r, lane);
+        const float4 a = f_fetch(p, unit0 + r, lane);
         sx[r] = to_turns(a.x, p.two32_over_L);
         sy[r] = to_turns(a.y, p.two32_over_L);
         sz[r] = to_turns(a.z, p.two32_over_L);
         q[r] = a.w;
         fx[r] = fy[r] = fz[r] = en[r] = 0.f;
     }
-#pragma unroll 4
+#pragma unroll 2
     for (int k = 0; k < nk; ++k) {
         const int4 a = s_ka[k];
         const float4 b = s_kb[k];
@@ -675,28 +694,42 @@ __device__ __forceinline__ void f_pass(const FParams& p, const int4* s_ka, const
     }
 }
 
-// n units in ceil(n / F_RMAX) passes of nearly equal size (e.g. 9 -> 3+3+3, not 4+4+1)
-__device__ __forceinline__ int f_first_pass(int n) {
-    const int passes = (n + F_RMAX - 1) / F_RMAX;
-    return passes ? (n + passes - 1) / passes : 0;
+// The units [c0, c1) of a CTA dealt to its warps so that the four SM sub-partitions (warp index mod 4) get the
+// same number of units to within one: the warps of a sub-partition take CONSECUTIVE shares of the even split.
+// (With the plain split by warp index, 212 units over 32 warps give the pattern 7,6,7,7,6,7,6,7 of period 8, and
+// one sub-partition gets 56 units against 53 on average: measured 6 % on the CTAs that have 212 units.)
+__device__ __forceinline__ void f_warp_share(int64_t c0, int64_t c1, int warp, int nwarps, int64_t& u0, int& n) {
+    int pos = warp;
+    if ((nwarps & 3) == 0) pos = (warp & 3) * (nwarps >> 2) + (warp >> 2);
+    u0 = c0 + (c1 - c0) * pos / nwarps;
+    n = (int)(c0 + (c1 - c0) * (pos + 1) / nwarps - u0);
 }
 
 template <bool ENERGY, bool ACCUM>
-__device__ __forceinline__ void f_run(const FParams& p, const int4* s_ka, const float4* s_kb, int nk, int64_t u, int n,
-                                      int lane, const float4* pre) {
-    int passes = (n + F_RMAX - 1) / F_RMAX;
+__device__ __forceinline__ void f_run(const FArgs& p, const int4* s_ka, const float4* s_kb, int nk, int64_t u, int n, int lane) {
+    int passes = (n + F_RMAX - 1) / F_RMAX;   // n units in passes of nearly equal size (e.g. 9 -> 3+3+3, not 4+4+1)
     while (n > 0) {
         const int r = (n + passes - 1) / passes;
         switch (r) {
-            case 4: f_pass<4, ENERGY, ACCUM>(p, s_ka, s_kb, nk, u, lane, pre); break;
-            case 3: f_pass<3, ENERGY, ACCUM>(p, s_ka, s_kb, nk, u, lane, pre); break;
-            case 2: f_pass<2, ENERGY, ACCUM>(p, s_ka, s_kb, nk, u, lane, pre); break;
-            default: f_pass<1, ENERGY, ACCUM>(p, s_ka, s_kb, nk, u, lane, pre); break;
+            case 4: f_pass<4, ENERGY, ACCUM>(p, s_ka, s_kb, nk, u, lane); break;
+            case 3: f_pass<3, ENERGY, ACCUM>(p, s_ka, s_kb, nk, u, lane); break;
+            case 2: f_pass<2, ENERGY, ACCUM>(p, s_ka, s_kb, nk, u, lane); break;
+            default: f_pass<1, ENERGY, ACCUM>(p, s_ka, s_kb, nk, u, lane); break;
         }
         u += r; n -= r; --passes;
-        pre = nullptr;
     }
 }
+
+// ---------------------------------------------------------------------------------------
+// f_kernel -- the forces as their own launch (rbe_forces; the chunked host step; the multi-GPU
+// exchange).  Every CTA builds the per-k records for its shared-memory tile from rho (k_record).
+// ---------------------------------------------------------------------------------------
+struct FParams {
+    FArgs a;
+    KTable kt;     // rho and the k-set: every CTA builds its {-m, theta}, {G, E} records from these
+    int32_t P;
+    int32_t pdl;   // launched with programmatic stream serialisation: wait before reading rho
+};
 
 template <bool ENERGY>
 __global__ void __launch_bounds__(F_THREADS, F_CTAS_PER_SM) f_kernel(const FParams p) {
@@ -705,18 +738,17 @@ __global__ void __launch_bounds__(F_THREADS, F_CTAS_PER_SM) f_kernel(const FPara
     int4* s_ka = reinterpret_cast<int4*>(smem_raw);
     float4* s_kb = reinterpret_cast<float4*>(smem_raw + (size_t)nkmax * sizeof(int4));
     const int lane = threadIdx.x & 31;
-    const int64_t nwarps = (int64_t)gridDim.x * (F_THREADS / 32);
-    const int64_t gw = (int64_t)blockIdx.x * (F_THREADS / 32) + (threadIdx.x >> 5);
-    const int64_t units = (p.N + 31) / 32;
-    const int64_t u0 = units * gw / nwarps, u1 = units * (gw + 1) / nwarps;
-    const int n = (int)(u1 - u0);
+    const int64_t units = (p.a.N + 31) / 32;
+    int64_t u0;
+    int n;
+    f_warp_share(units * blockIdx.x / gridDim.x, units * (blockIdx.x + 1) / gridDim.x, threadIdx.x >> 5, F_THREADS / 32, u0, n);
 
-    // fetch the first pass's atoms before waiting for the structure factors: the loads (and, with
-    // PDL, this grid's launch) overlap the tail of the preceding grid
-    float4 pre[F_RMAX];
-    const int r0 = f_first_pass(n);
-#pragma unroll
-    for (int r = 0; r < F_RMAX; ++r) pre[r] = r < r0 ? f_fetch(p, u0 + r, lane) : make_float4(0.f, 0.f, 0.f, 0.f);
+    // pull this warp's atoms into L2 before waiting for the structure factors: the requests (and, with PDL,
+    // this grid's launch) overlap the tail of the preceding grid, and hold no registers across the wait
+    for (int r = 0; r < n && r < 2 * F_RMAX; ++r) {
+        const int64_t i = (u0 + r) * 32 + lane;
+        if (i < p.a.N) asm volatile("prefetch.global.L2 [%0];" ::"l"(p.a.xyzq + i));
+    }
 
     if (p.pdl) grid_dependency_wait();   // rho comes from the preceding grid
     xch_wait(p.kt.xch);                  // ... and, with a multi-GPU exchange, from the peers' grids
@@ -726,9 +758,145 @@ __global__ void __launch_bounds__(F_THREADS, F_CTAS_PER_SM) f_kernel(const FPara
         if (k0 > 0) __syncthreads();
         for (int t = threadIdx.x; t < nk; t += F_THREADS) k_record(p.kt, k0 + t, s_ka[t], s_kb[t]);
         __syncthreads();
-        if (k0 == 0) f_run<ENERGY, false>(p, s_ka, s_kb, nk, u0, n, lane, pre);
-        else f_run<ENERGY, true>(p, s_ka, s_kb, nk, u0, n, lane, nullptr);
+        if (k0 == 0) f_run<ENERGY, false>(p.a, s_ka, s_kb, nk, u0, n, lane);
+        else f_run<ENERGY, true>(p.a, s_ka, s_kb, nk, u0, n, lane);
     }
+}
+
+// ---------------------------------------------------------------------------------------
+// step_kernel -- Algorithm 1 steps 2-4 in ONE cooperative launch (rbe_step), one CTA per
+// SM, all CTAs co-resident:
+//   1. SF phase over the CTA's atoms -> one fp64 row of P partial sums per CTA (global memory);
+//   2. grid barrier;
+//   3. distributed fixed-order reduction: the P wavevectors are dealt to the CTAs; one warp per
+//      wavevector sums the gridDim.x rows (lane l takes rows l, l+32, ... in order, then a fixed
+//      butterfly over the lanes), writes rho(k) and builds that wavevector's force record ONCE
+//      (k_record_from: fp64 atan2 / sqrt) -- no serial tail, no ticket, no per-CTA rebuild;
+//   4. grid barrier;
+//   5. F phase over the same atoms with the P records in shared memory.
+// Which CTA does what is fixed by blockIdx, so the result is bitwise reproducible.  The grid barrier
+// is a 64-bit arrival counter in the workspace that only ever grows (a launch adds 2 * gridDim.x).
+// For small batches without weights the wavevectors ride in the kernel parameters (int16 triples), so
+// a step is one launch and nothing else: no host-to-device copy.
+// ---------------------------------------------------------------------------------------
+struct StepParams {
+    SfArgs sf;
+    FArgs f;
+    const int4* kvec;          // [P] wavevectors in the workspace (read unless kparam, written if kparam)
+    const double* w;           // [P] weights or nullptr
+    double w_uniform, L;
+    double2* rho;              // [P] out
+    double2* rho_user;         // [P] out or nullptr
+    int4* ka;                  // [P] force records, built in step 3
+    float4* kb;
+    unsigned long long* bar;   // grid-barrier arrival counter
+    int32_t kparam;            // wavevectors are in km (P <= STEP_KPARAM_MAX), else in kvec
+    int16_t km[STEP_KPARAM_MAX * 3];
+};
+
+__device__ __forceinline__ unsigned long long ld_acquire_gpu_u64(const unsigned long long* p) {
+    unsigned long long v;
+    asm volatile("ld.acquire.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(p) : "memory");
+    return v;
+}
+
+// All threads of all CTAs of a cooperative launch.  Release: barrier + fence by thread 0 before its
+// arrival; acquire: its polling load + fence before the barrier that lets the CTA continue.
+__device__ __forceinline__ void grid_barrier(unsigned long long* ctr) {
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        __threadfence();
+        const unsigned long long n = gridDim.x;
+        const unsigned long long old = atomicAdd(ctr, 1ull);
+        const unsigned long long target = (old / n + 1ull) * n;
+        while (ld_acquire_gpu_u64(ctr) < target) { }
+        __threadfence();
+    }
+    __syncthreads();
+}
+
+__device__ __forceinline__ int4 step_kvec(const StepParams& p, const int16_t* s_km, int k) {
+    if (p.kparam) return make_int4(s_km[3 * k], s_km[3 * k + 1], s_km[3 * k + 2], 0);
+    return __ldg(&p.kvec[k]);
+}
+
+template <bool DEEP, bool ENERGY>
+__global__ void __launch_bounds__(SF_TMAX, 1) step_kernel(const __grid_constant__ StepParams p) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    __shared__ SfCtl ctl;
+    const int tid = threadIdx.x, T = blockDim.x, lane = tid & 31, warp = tid >> 5, nwarps = T >> 5;
+    const int bx = blockIdx.x, G = gridDim.x, P = p.sf.P;
+
+    // ---- 1. SF phase                                                                   // @stamp
+    // wavevectors from the kernel parameters: the constant bank serves one address per request, so every warp
+    // reads a run of consecutive words with all its lanes on the SAME word (a broadcast) and parks them in
+    // shared memory; per-thread indexing of the parameter array would serialise 32 ways (measured: 11 us)
+    __shared__ int16_t s_km[STEP_KPARAM_MAX * 3];
+    if (p.kparam) {
+        const int n3 = 3 * P, per = (n3 + nwarps - 1) / nwarps;
+        const int i1 = (warp + 1) * per < n3 ? (warp + 1) * per : n3;
+        for (int i = warp * per; i < i1; ++i) {
+            const int16_t v = p.km[i];
+            if (lane == 0) s_km[i] = v;
+        }
+        __syncthreads();
+    }
+    {
+        const bool active = tid < p.sf.gs * p.sf.ng;
+        const int kbase = (active ? tid % p.sf.gs : 0) * SF_KPT;
+        int mx[SF_KPT], my[SF_KPT], mz[SF_KPT];
+#pragma unroll
+        for (int r = 0; r < SF_KPT; ++r) {
+            int4 m = make_int4(0, 0, 0, 0);
+            if (active && kbase + r < P) m = step_kvec(p, s_km, kbase + r);
+            mx[r] = m.x; my[r] = m.y; mz[r] = m.z;
+        }
+        if (p.kparam && bx == 0)   // keep the workspace copy current for the energy / virial / read-back calls
+            for (int k = tid; k < P; k += T) const_cast<int4*>(p.kvec)[k] = step_kvec(p, s_km, k);
+        sf_accumulate<DEEP>(p.sf, mx, my, mz, smem_raw, ctl, bx, G);                    // @stamp
+        sf_write_row(p.sf, smem_raw, bx, 0);                                              // @stamp
+    }
+    grid_barrier(p.bar);                                                                  // @stamp
+
+    // ---- 3. distributed fixed-order reduction + the per-k force records
+    {
+        const int k_lo = (int)((int64_t)P * bx / G), k_hi = (int)((int64_t)P * (bx + 1) / G);
+        for (int k = k_lo + warp; k < k_hi; k += nwarps) {
+            double re = 0.0, im = 0.0;
+#pragma unroll 5
+            for (int row = lane; row < G; row += 32) {     // (148 rows: five independent loads per lane in flight)
+                const double2 v = __ldcg(&p.sf.part[(int64_t)row * P + k]);
+                re += v.x; im += v.y;
+            }
+#pragma unroll
+            for (int d = 16; d > 0; d >>= 1) {
+                re += __shfl_xor_sync(FULL_MASK, re, d);
+                im += __shfl_xor_sync(FULL_MASK, im, d);
+            }
+            if (lane == 0) {
+                const double2 r = make_double2(re, im);
+                p.rho[k] = r;
+                if (p.rho_user) p.rho_user[k] = r;
+                int4 a; float4 b;
+                k_record_fast(step_kvec(p, s_km, k), r, p.w ? p.w[k] : p.w_uniform, p.L, a, b);
+                p.ka[k] = a; p.kb[k] = b;
+            }
+        }
+    }
+                                                                                          // @stamp
+    grid_barrier(p.bar);                                                                  // @stamp
+
+    // ---- 5. F phase: this CTA's warps take the same atom range the CTA had in the SF phase
+    if (p.f.force == nullptr) return;
+    int4* s_ka = reinterpret_cast<int4*>(smem_raw);
+    float4* s_kb = reinterpret_cast<float4*>(smem_raw + (size_t)P * sizeof(int4));
+    for (int t = tid; t < P; t += T) { s_ka[t] = __ldcg(&p.ka[t]); s_kb[t] = __ldcg(&p.kb[t]); }
+    __syncthreads();
+    const int64_t units = (p.f.N + 31) / 32;
+    int64_t u0;
+    int n;
+    f_warp_share(units * bx / G, units * (bx + 1) / G, warp, nwarps, u0, n);   // the CTA's units (as in the SF phase)
+    f_run<ENERGY, false>(p.f, s_ka, s_kb, P, u0, n, lane);                            // @stamp @stamp_sync
 }
 
 // ---------------------------------------------------------------------------------------
@@ -815,6 +983,40 @@ __global__ void __launch_bounds__(256) unpack_force_kernel(const float4* __restr
         const float4 f = f4[i];
         f3[3 * i] = f.x; f3[3 * i + 1] = f.y; f3[3 * i + 2] = f.z;
     }
+}
+
+// ---------------------------------------------------------------------------------------
+// Pipe-rate probe (rbe_probe_pipe_rates): the roofline of this path is set by the FP32-FMA, IMAD,
+// I2FP and MUFU issue rates, which MEASURED_PEAKS.json does not hold (SURVEY.md s7 stage 6).  One CTA
+// of 1024 threads per SM runs 8 dependent-free chains per thread of one instruction kind; thread 0 of
+// every CTA reports the SM cycles (clock64) its CTA took, so the rates are per clock, whatever the clock.
+// MODE 0: FFMA, 1: IMAD, 2: I2FP.F32.S32, 3: FMUL.RZ + MUFU.SIN (sin.approx).
+// ---------------------------------------------------------------------------------------
+template <int MODE>
+__global__ void __launch_bounds__(1024, 1) probe_kernel(long long* cycles, int iters, float fa, float fb, int ia, int ib) {
+    constexpr int C = 8;
+    float v[C];
+    int w[C];
+#pragma unroll
+    for (int c = 0; c < C; ++c) { v[c] = threadIdx.x * 0.001f + c; w[c] = threadIdx.x + c; }
+    __syncthreads();
+    const long long t0 = clock64();
+    for (int it = 0; it < iters; ++it) {
+#pragma unroll
+        for (int c = 0; c < C; ++c) {
+            if (MODE == 0) v[c] = fmaf(v[c], fa, fb);
+            if (MODE == 1) w[c] = w[c] * ia + ib;
+            if (MODE == 2) w[c] = __float_as_int((float)w[c]);
+            if (MODE == 3) v[c] = fast_sin(v[c]);
+        }
+    }
+    float s = 0.f;
+    int t = 0;
+#pragma unroll
+    for (int c = 0; c < C; ++c) { s += v[c]; t += w[c]; }
+    __syncthreads();
+    const long long t1 = clock64();
+    if (threadIdx.x == 0) cycles[blockIdx.x] = (s + (float)t == 123.456f) ? 0 : t1 - t0;
 }
 
 }  // namespace rbe

@@ -29,7 +29,7 @@ class LaunchInfo(ctypes.Structure):
     _fields_ = [(n, ctypes.c_int32) for n in (
         "num_sms", "sf_grid_x", "sf_grid_y", "sf_threads", "sf_smem_bytes", "sf_k_per_thread",
         "sf_atom_groups", "sf_tile_atoms", "sf_red_group", "sf_red_groups", "f_grid", "f_threads",
-        "f_smem_bytes", "f_atoms_per_thread")]
+        "f_smem_bytes", "f_atoms_per_thread", "step_fused", "step_smem_bytes")]
 
     def as_dict(self):
         return {n: int(getattr(self, n)) for n, _ in self._fields_}
@@ -91,6 +91,12 @@ def lib():
         L.rbe_set_rho.argtypes = [vp, vp, vp]
         L.rbe_forces.restype = ctypes.c_int
         L.rbe_forces.argtypes = [vp, vp, vp, i32, vp]
+        L.rbe_step.restype = ctypes.c_int
+        L.rbe_step.argtypes = [vp, vp, vp, vp, vp, i32, vp, vp]
+        L.rbe_step_host_bytes.restype = sz
+        L.rbe_step_host_bytes.argtypes = [vp, i32]
+        L.rbe_probe_pipe_rates.restype = ctypes.c_int
+        L.rbe_probe_pipe_rates.argtypes = [vp, vp, vp]
         L.rbe_kspace_energy.restype = ctypes.c_int
         L.rbe_kspace_energy.argtypes = [vp, ctypes.POINTER(dbl), vp]
         L.rbe_kspace_virial.restype = ctypes.c_int
@@ -272,6 +278,33 @@ class Rbe:
                                      ctypes.c_void_p(force.data_ptr()), int(bool(with_energy)),
                                      _stream_ptr(stream)))
 
+    def rbe_step(self, m, xyzq, force, w=None, with_energy: bool = False, rho=None, stream=None):
+        """Algorithm 1 steps 2-4 in one cooperative launch.  m: numpy int32 [P,3] (host) or None (keep the
+        k-set on the device); xyzq, force: cuda float32 [N,4]; rho: cuda float64 [P,2] or None."""
+        import numpy as np
+        _check_tensor(xyzq, (self.N, 4), "float32")
+        _check_tensor(force, (self.N, 4), "float32")
+        if rho is not None:
+            _check_tensor(rho, (self.P, 2), "float64")
+        mm = None if m is None else np.ascontiguousarray(m, dtype=np.int32)
+        assert mm is None or mm.shape == (self.P, 3), mm.shape
+        ww = None if w is None else np.ascontiguousarray(w, dtype=np.float64)
+        assert ww is None or ww.shape == (self.P,)
+        self._check(lib().rbe_step(self._h, _np_ptr(mm), _np_ptr(ww), ctypes.c_void_p(xyzq.data_ptr()),
+                                   ctypes.c_void_p(force.data_ptr()), int(bool(with_energy)),
+                                   None if rho is None else ctypes.c_void_p(rho.data_ptr()), _stream_ptr(stream)))
+
+    def rbe_step_host_bytes(self, compact: bool) -> int:
+        return int(lib().rbe_step_host_bytes(self._h, int(bool(compact))))
+
+    def rbe_probe_pipe_rates(self, stream=None) -> dict:
+        """Measured issue rates (thread-instructions per SM per clock) and the SM clock seen (synchronises)."""
+        import numpy as np
+        out = np.zeros(5, dtype=np.float64)
+        self._check(lib().rbe_probe_pipe_rates(self._h, _np_ptr(out), _stream_ptr(stream)))
+        return {"ffma": float(out[0]), "imad": float(out[1]), "i2fp": float(out[2]), "mufu": float(out[3]),
+                "sm_mhz": float(out[4])}
+
     def rbe_short_range_bytes(self, rs: float) -> int:
         return int(lib().rbe_short_range_bytes(self._h, float(rs)))
 
@@ -328,7 +361,7 @@ class Rbe:
         """Compact end-to-end step: h_xyz / h_force3 are host float32 [N,3] (numpy or CPU torch)."""
         import numpy as np
         import torch
-        need = 56 * self.N + 1024
+        need = self.rbe_step_host_bytes(True)
         if getattr(self, "_scratch3", None) is None or self._scratch3.numel() < need:
             self._scratch3 = torch.empty(max(1, need), dtype=torch.uint8, device="cuda")
         mm = np.ascontiguousarray(m, dtype=np.int32)
@@ -347,7 +380,7 @@ class Rbe:
         import numpy as np
         import torch
         if self._scratch is None:
-            self._scratch = torch.empty(max(1, 32 * self.N + 512), dtype=torch.uint8, device="cuda")
+            self._scratch = torch.empty(max(1, self.rbe_step_host_bytes(False)), dtype=torch.uint8, device="cuda")
         mm = np.ascontiguousarray(m, dtype=np.int32)
         assert mm.shape == (self.P, 3)
         ww = None if w is None else np.ascontiguousarray(w, dtype=np.float64)

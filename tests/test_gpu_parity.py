@@ -32,15 +32,40 @@ def gpu_step(atoms, L, alpha, m, w=None, with_energy=False):
     return ctx, rho.cpu().numpy(), force.cpu().numpy(), U
 
 
+def gpu_fused_step(atoms, L, alpha, m, w=None, with_energy=False):
+    """The same step through rbe_step: ONE cooperative launch (SF phase, grid barrier, distributed
+    fixed-order reduction, grid barrier, F phase)."""
+    N, P = atoms.shape[0], m.shape[0]
+    ctx = rbe.Rbe(N, L, alpha, P)
+    xyzq = torch.from_numpy(atoms).cuda()
+    rho = torch.full((P, 2), float("nan"), dtype=torch.float64, device="cuda")
+    force = torch.full((N, 4), float("nan"), dtype=torch.float32, device="cuda")
+    ctx.rbe_step(m, xyzq, force, w=w, with_energy=with_energy, rho=rho)
+    U = ctx.rbe_kspace_energy()
+    torch.cuda.synchronize()
+    return ctx, rho.cpu().numpy(), force.cpu().numpy(), U
+
+
 def check(atoms, L, alpha, m, w=None, with_energy=False, sel=None, f_tol=F_TOL):
-    ctx, rho_g, F_g, U_g = gpu_step(atoms, L, alpha, m, w, with_energy)
+    """Both product paths against the oracle: the two launches (rbe_structure_factor + rbe_forces) and the
+    one-launch rbe_step.  Returns the errors of the one-launch path (what bench.py times)."""
+    cache = {}
+    _check_path(gpu_step, cache, atoms, L, alpha, m, w, with_energy, sel, f_tol)
+    return _check_path(gpu_fused_step, cache, atoms, L, alpha, m, w, with_energy, sel, f_tol)
+
+
+def _check_path(run, cache, atoms, L, alpha, m, w, with_energy, sel, f_tol):
+    ctx, rho_g, F_g, U_g = run(atoms, L, alpha, m, w, with_energy)
     S = oracle.S(L, alpha)
     assert abs(ctx.rbe_normaliser_S() - S) <= 1e-13 * S
-    rho_o = oracle.rho(atoms, L, m)
+    if "rho" not in cache:
+        cache["rho"] = oracle.rho(atoms, L, m)
+        cache["F"] = oracle.force(atoms, L, m, S, cache["rho"], w=w, sel=sel, with_energy=with_energy)
+    rho_o = cache["rho"]
     qsum = np.abs(atoms[:, 3].astype(np.float64)).sum()
     err_rho = np.abs(rho_g - rho_o).max() if len(m) else 0.0
     assert err_rho <= RHO_TOL * max(qsum, 1e-300), (err_rho, qsum)
-    out = oracle.force(atoms, L, m, S, rho_o, w=w, sel=sel, with_energy=with_energy)
+    out = cache["F"]
     F_o, e_o = out if with_energy else (out, None)
     Fg = F_g[:, :3].astype(np.float64)
     if sel is not None:
