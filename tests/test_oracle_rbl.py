@@ -64,3 +64,59 @@ def test_unbiased_mean_over_steps_converges_to_the_deterministic_force():
     assert 1.5 <= res[16] / res[64] <= 2.7 and 1.5 <= res[64] / res[256] <= 2.7, res
     one = np.linalg.norm(rbl.rbl_forces(a, L, alpha, rc, rs, p, seed=9, step=1, correction=False)[0] - Fd)
     assert res[256] <= 0.15 * one
+
+
+def _fmix32_inverse(h):
+    """Inverse of fmix32 from the mathematics, not from its code: x ^= x >> s is undone by repeating the shift-xor
+    until the shift passes 32 bits; a multiplication by an odd constant mod 2^32 by its modular inverse."""
+    h = int(h)
+    h ^= h >> 16
+    h = (h * pow(0xC2B2AE35, -1, 1 << 32)) & 0xFFFFFFFF
+    h ^= (h >> 13) ^ (h >> 26)
+    h = (h * pow(0x85EBCA6B, -1, 1 << 32)) & 0xFFFFFFFF
+    h ^= h >> 16
+    return h
+
+
+def test_pair_key_is_a_bijective_well_mixed_hash():
+    rng = np.random.default_rng(3)
+    x = rng.integers(0, 1 << 32, 2000, dtype=np.uint64)
+    y = rbl.fmix32(x)
+    assert all(_fmix32_inverse(v) == int(u) for u, v in zip(x, y))          # a bijection, with exactly these steps
+    assert int(rbl.fmix32(np.array([0], dtype=np.uint64))[0]) == 0          # fixed point of shift-xor and multiply
+    # avalanche: flipping any single input bit flips half of the output bits on average
+    for bit in (0, 7, 15, 16, 24, 31):
+        flips = np.bitwise_xor(y, rbl.fmix32(x ^ np.uint64(1 << bit)))
+        n = np.array([bin(int(v)).count("1") for v in flips])
+        assert 15.0 <= n.mean() <= 17.0, (bit, n.mean())
+    # for a fixed i the keys of distinct partners are distinct (j -> u_ij is a bijection), and the salt matters
+    k = rbl.pair_keys(5, np.arange(50_000), 9, 4)
+    assert np.unique(k).shape[0] == 50_000
+    assert not np.array_equal(k[:100], rbl.pair_keys(5, np.arange(100), 9, 5))
+    assert not np.array_equal(k[:100], rbl.pair_keys(5, np.arange(100), 10, 4))
+    assert rbl.step_salt(9, 4) != rbl.step_salt(9, (1 << 32) + 4)                  # the high word of the step counts
+
+
+def test_batch_is_a_uniform_p_subset_of_the_shell():
+    """Every member of S(i) is chosen with probability p / N_s (chi-square over many steps), whatever its index
+    or its position in the list -- a selection that favoured low keys' owners, low j, or near neighbours fails."""
+    p, T = 6, 3000
+    for i, shell in ((0, np.arange(100, 140)), (77, np.array([3, 4, 5, 6, 1000, 1001, 70_000, 2 ** 20 + 1, 12, 13, 14, 15, 16, 17, 18, 19]))):
+        counts = np.zeros(shell.shape[0])
+        pairs = np.zeros((shell.shape[0], shell.shape[0]))
+        for t in range(T):
+            keys = rbl.pair_keys(i, shell, 123, t).astype(np.uint64)
+            chosen = np.lexsort((shell, keys))[:p]
+            counts[chosen] += 1
+            pairs[np.ix_(chosen, chosen)] += 1
+        n = shell.shape[0]
+        expect = T * p / n
+        # marginal counts: hypergeometric-like, variance T q (1 - q) with q = p/n; the counts sum to T p exactly
+        # (one linear constraint), so sum z^2 has about n - 1 degrees of freedom
+        z = (counts - expect) / np.sqrt(T * (p / n) * (1 - p / n))
+        assert (z ** 2).sum() <= 2.2 * n, (z ** 2).sum()
+        # pair inclusion: P(j and k both in B) = p (p - 1) / (n (n - 1)) for a uniform subset
+        off = pairs[~np.eye(n, dtype=bool)]
+        q2 = p * (p - 1) / (n * (n - 1))
+        assert abs(off.mean() - T * q2) <= 1e-9 * T          # exact: every batch has p (p - 1) ordered pairs
+        assert off.std() <= 1.6 * np.sqrt(T * q2 * (1 - q2)), (off.std(), np.sqrt(T * q2))
