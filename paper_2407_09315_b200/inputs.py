@@ -118,6 +118,29 @@ def make_atoms(cfg: Config) -> np.ndarray:
     return np.ascontiguousarray(a.astype(np.float32))
 
 
+MASS_NA, MASS_CL = 22.98977, 35.453  # amu
+
+
+def rocksalt(ncells: int, a: float = 5.64, seed: int = 7, jitter: float = 0.05, v_rms: float = 0.0):
+    """A perturbed rock-salt (NaCl) crystal for the NVE loop: ncells^3 conventional cells of
+    side a [A] (8 ions each: Na+ on the fcc sites, Cl- shifted by a/2 along x), every ion displaced by a normal
+    deviate of standard deviation `jitter` [A], velocities normal with per-component deviation v_rms / sqrt(m)
+    [A / tau] minus the centre-of-mass drift.  Returns (x fp64 [N,3], v fp64 [N,3], q fp32 [N], mass fp64 [N], L)."""
+    rng = np.random.default_rng(seed)
+    fcc = np.array([[0.0, 0.0, 0.0], [0.0, 0.5, 0.5], [0.5, 0.0, 0.5], [0.5, 0.5, 0.0]])
+    cells = np.stack(np.meshgrid(*[np.arange(ncells)] * 3, indexing="ij"), axis=-1).reshape(-1, 1, 3)
+    na = (cells + fcc[None]).reshape(-1, 3)
+    cl = na + np.array([0.5, 0.0, 0.0])
+    x = np.concatenate([na, cl]) * a
+    n = x.shape[0]
+    q = np.concatenate([np.ones(n // 2), -np.ones(n // 2)]).astype(np.float32)
+    mass = np.concatenate([np.full(n // 2, MASS_NA), np.full(n // 2, MASS_CL)])
+    x = x + jitter * rng.standard_normal((n, 3))
+    v = v_rms * rng.standard_normal((n, 3)) / np.sqrt(mass)[:, None]
+    v -= (mass[:, None] * v).sum(0) / mass.sum()
+    return x, v, q, mass, float(ncells * a)
+
+
 def pmf_1d(L: float, alpha: float):
     """(support m = -M..M, probabilities) of the 1-D discrete Gaussian exp(-pi^2 m^2/(alpha L^2))."""
     c = np.pi ** 2 / (alpha * L * L)
