@@ -213,8 +213,9 @@ rbe_status rbe_forces(rbe_ctx* ctx, const void* d_xyzq, void* d_force, int32_t w
  * Equivalent to rbe_set_kvectors + rbe_structure_factor + rbe_forces: the same arithmetic per (atom, k) pair,
  * the same tolerances against the definitions; rho differs from rbe_structure_factor's in the last bits only
  * (another fixed order of the per-CTA rows).  Bitwise reproducible.  Afterwards rbe_kspace_energy /
- * rbe_kspace_virial / rbe_forces refer to this step.  Falls back to the two launches when P > 4096, when a
- * multi-GPU exchange is configured, or when the device cannot launch cooperatively (rbe_launch_info.step_fused).
+ * rbe_kspace_virial / rbe_forces refer to this step.  Takes the two launches instead when P > 4096, when a
+ * multi-GPU exchange is configured, when the device cannot launch cooperatively, or when the system is so large
+ * (N * P > 4e6 per SM) that the two-launch kernels are the faster form (rbe_launch_info.step_fused tells).
  * d_xyzq must not be written by other work while the launch runs; no other kernel may share the GPU's SMs with
  * it in a way that keeps part of the grid from becoming resident (the cooperative launch fails rather than hangs).
  * Errors: RBE_ERR_NOT_READY, RBE_ERR_BAD_KVECTOR, RBE_ERR_INVALID_ARG, RBE_ERR_CUDA. */
@@ -248,13 +249,19 @@ rbe_status rbe_short_range(rbe_ctx* ctx, const void* d_xyzq, double rs, void* d_
 /* Random batch list (RBL) estimate of the same short-range force: section 2.3, Eqs. (2.13)-(2.16)
  * P:145-166, Algorithm 2, with F_ij the electrostatic pair force of Eq. (2.10):
  *   F_i = sum_{j: r < r_c} F_ij + (N_s / p) sum_{j in B(i)} F_ij + F^corr,  F^corr = -(1/N) sum_i (...)
- * where N_s counts the shell r_c <= r < r_s of atom i and B(i) holds the min(p, N_s) shell members with
- * the smallest (u_ij, j), u_ij = first output word of Philox4x32-10 with counter (i, j, step mod 2^32,
- * step >> 32) and key (seed mod 2^32, seed >> 32), i and j being atom indices: a uniformly random
- * p-subset, a pure function of (seed, step).  N_s <= p: the whole shell, scale 1.  Forces only
- * (d_force[i].w = 0, or unchanged with accumulate).  1 <= p <= 32, 0 < rc < rs <= L/3.  d_ws as for
- * rbe_short_range (rbe_short_range_bytes(ctx, rs)).  Bitwise reproducible.
+ * where N_s counts the shell r_c <= r < r_s of atom i and B(i) holds the min(p, N_s) shell members with the
+ * smallest keys u_ij.  The paper does not say how the p members are drawn; here (reading Q20)
+ *   (s0, s1) = first two words of Philox4x32-10 with counter (step mod 2^32, step >> 32, 0, 0) and key
+ *              (seed mod 2^32, seed >> 32)                       [once per call, on the host]
+ *   u_ij     = fmix32( (i * 0x9E3779B1 + s0) xor (j * 0x85EBCA77 + s1) )   mod 2^32, i and j atom indices,
+ *   fmix32(h): h ^= h >> 16; h *= 0x85EBCA6B; h ^= h >> 13; h *= 0xC2B2AE35; h ^= h >> 16
+ * -- a uniformly random p-subset, a pure function of (seed, step), distinct keys for distinct j.  N_s <= p:
+ * the whole shell, scale 1.  Cell list with cells of side max(r_c, r_s / 4) (Algorithm 2: side r_c),
+ * one CTA per cell, a warp per atom.  Forces only (d_force[i].w = 0, or unchanged with accumulate).
+ * 1 <= p <= 32, 0 < rc < rs <= L/3.  d_ws: caller-owned scratch of rbe_rbl_bytes(ctx, rc, rs) bytes (~76 B per atom
+ * + 204 B per cell), 256-byte aligned; rbe_rbl_bytes returns 0 for invalid radii.  Bitwise reproducible.
  * Errors: RBE_ERR_INVALID_ARG, RBE_ERR_WORKSPACE, RBE_ERR_NO_DEVICE, RBE_ERR_CUDA. */
+size_t     rbe_rbl_bytes(const rbe_ctx* ctx, double rc, double rs);
 rbe_status rbe_rbl_forces(rbe_ctx* ctx, const void* d_xyzq, double rc, double rs, int32_t p, uint64_t seed,
                           uint64_t step, void* d_force, int32_t accumulate, void* d_ws, size_t ws_bytes,
                           void* stream);
@@ -299,6 +306,37 @@ rbe_status rbe_set_charges(rbe_ctx* ctx, const void* d_q);
 rbe_status rbe_step_host_xyz(rbe_ctx* ctx, const float* h_xyz, const int32_t* h_m, const double* h_w,
                              float* h_force3, double* h_U, void* d_scratch, size_t scratch_bytes,
                              void* stream);
+
+/* NVE velocity-Verlet loop (the paper integrates with velocity-Verlet, and runs the NVE ensemble among
+ * others).  State in fp64, owned by the caller, on the device: positions
+ * d_pos double [N][3], velocities d_vel double [N][3], inverse masses d_inv_mass double [N]; the force kernels
+ * read d_xyzq float4 [N] = positions rounded to fp32 + charges, which rbe_nve_kick keeps in step.  Units: A, e,
+ * amu, hence times in tau = sqrt(amu A^3 / e^2) = 2.68285 fs (reading Q21).
+ *
+ * rbe_nve_kick:  v += half_dt * F / m  from d_force float4 [N] (.w ignored); then, if d_pos != NULL, the drift
+ *   x += dt * v and d_xyzq[i].xyz = (float) x[i] (d_xyzq[i].w, the charge, is kept).  One step of the scheme is
+ *   kick(dt/2, drift dt) -> forces at the new positions -> kick(dt/2, no drift).  Enqueues one kernel.
+ * rbe_nve_energies:  h_out double [2] (host) = { sum_i 1/2 m_i v_i^2 (0 if d_vel == NULL), sum_i d_force[i].w
+ *   (0 if d_force == NULL: with_energy forces carry the per-atom potential energies there) }, fp64, fixed order;
+ *   synchronises `stream`; needs the workspace.
+ * rbe_md_capture:  one whole MD step -- kick + drift, [a fresh batch from the device sampler if sampled != 0:
+ *   (seed, step) as rbe_graph_capture; else the k-set and weights already on the device, e.g. the full grid with
+ *   w_l = exp(-k_l^2 / 4 alpha): deterministic Ewald], the k-space step (rbe_step's kernels), rbe_short_range
+ *   with accumulate = 1 and cutoff rs (d_sr_ws of rbe_short_range_bytes(ctx, rs) bytes), kick -- captured ONCE as
+ *   a CUDA graph bound to these arrays and replayed by rbe_graph_launch with one launch per step, positions and
+ *   velocities resident on the device.  Before the first replay d_force must hold the forces of the current
+ *   positions (rbe_step + rbe_short_range(accumulate)).  with_energy != 0: d_force[i].w carries the per-atom
+ *   k-space + short-range potential energy after every step.  Synchronises; replaces any rbe_graph_capture graph.
+ * Nothing on this path keeps unlike charges apart (the paper's Lennard-Jones term, Eq. 2.2, is out of scope):
+ * meant for short horizons from a perturbed crystal.
+ * Errors: RBE_ERR_INVALID_ARG, RBE_ERR_NOT_READY, RBE_ERR_WORKSPACE, RBE_ERR_CUDA. */
+rbe_status rbe_nve_kick(rbe_ctx* ctx, void* d_vel, const void* d_inv_mass, const void* d_force, double half_dt,
+                        void* d_pos, void* d_xyzq, double dt, void* stream);
+rbe_status rbe_nve_energies(rbe_ctx* ctx, const void* d_vel, const void* d_inv_mass, const void* d_force,
+                            double* h_out, void* stream);
+rbe_status rbe_md_capture(rbe_ctx* ctx, void* d_pos, void* d_vel, const void* d_inv_mass, void* d_xyzq, void* d_force,
+                          double rs, double dt, void* d_sr_ws, size_t sr_bytes, int32_t sampled, uint64_t seed,
+                          uint64_t first_step, int32_t with_energy);
 
 /* Measure, on this device and now, the issue rates that bound this path (there is no vendor-stated figure to
  * take them from): h_out double [5] (host) = thread-instructions per SM per clock of FFMA, IMAD, I2FP.F32.S32

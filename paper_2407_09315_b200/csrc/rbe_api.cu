@@ -14,6 +14,7 @@
 #include "sr_kernels.cuh"
 #include "sr_pair_kernels.cuh"
 #include "rbl_kernels.cuh"
+#include "nve_kernels.cuh"
 
 namespace {
 
@@ -41,7 +42,7 @@ struct rbe_ctx {
     int sf_ngroups = 1;
     size_t ws_bytes = 0;
     size_t off_kvec = 0, off_w = 0, off_part = 0, off_rho = 0, off_grow = 0, off_U = 0, off_ticket = 0;
-    size_t off_ka = 0, off_kb = 0, off_bar = 0;
+    size_t off_ka = 0, off_kb = 0, off_bar = 0, off_nve = 0;
     bool sf_deep = false;       // a thread takes more than SF_DEPTH atoms from one tile: flush inside the loops
     bool step_fused = false;    // the one-launch cooperative step kernel is usable for this context
     size_t step_smem = 0;
@@ -100,6 +101,17 @@ rbe_status cuda_fail(rbe_ctx* c, const char* what, cudaError_t e) {
         cudaError_t e__ = (call);                             \
         if (e__ != cudaSuccess) return cuda_fail(ctx, #call, e__); \
     } while (0)
+
+// Philox4x32-10 (Salmon et al., SC'11) on the host, for the one call per step that salts the RBL pair keys
+void philox4x32_10_host(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3, uint32_t k0, uint32_t k1, uint32_t out[4]) {
+    for (int r = 0; r < 10; ++r) {
+        const uint64_t p0 = (uint64_t)0xD2511F53u * c0, p1 = (uint64_t)0xCD9E8D57u * c2;
+        const uint32_t n0 = (uint32_t)(p1 >> 32) ^ c1 ^ k0, n1 = (uint32_t)p1, n2 = (uint32_t)(p0 >> 32) ^ c3 ^ k1, n3 = (uint32_t)p0;
+        c0 = n0; c1 = n1; c2 = n2; c3 = n3;
+        k0 += 0x9E3779B9u; k1 += 0xBB67AE85u;
+    }
+    out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
+}
 
 double normaliser_S(double L, double alpha) {
     // S = H^3 - 1, H = sum_{m in Z} exp(-pi^2 m^2 / (alpha L^2))   (k = 2 pi m / L P:115)
@@ -215,6 +227,10 @@ rbe_status init_device(rbe_ctx* c) {
     int coop = 0;
     RBE_CUDA(c, cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, c->device));
     c->step_fused = coop && gy == 1 && c->P <= rbe::STEP_PMAX && c->step_smem <= (size_t)sf_smem_max && gx <= li.num_sms;
+    // Beyond ~4e6 (atom, k) pairs per SM the fixed costs the single launch removes (~8 us) are under 0.5 % of the
+    // step, while the two-launch force kernel (2 CTAs x 512 threads per SM) runs its loop 4 % faster than the force
+    // phase of the 1024-thread step kernel (measured, N = 1e7, P = 200: 1540 against 1592 us per step).
+    if ((double)c->N * (double)c->P > 4.0e6 * (double)li.num_sms) c->step_fused = false;
     if (c->step_fused) {
         RBE_CUDA(c, cudaFuncSetAttribute(rbe::step_kernel<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, sf_smem_max));
         RBE_CUDA(c, cudaFuncSetAttribute(rbe::step_kernel<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, sf_smem_max));
@@ -243,6 +259,7 @@ rbe_status init_device(rbe_ctx* c) {
     c->off_ka = off;   off = align_up(off + P * sizeof(int4), 256);      // per-k force records of the step kernel
     c->off_kb = off;   off = align_up(off + P * sizeof(float4), 256);
     c->off_bar = off;  off = align_up(off + sizeof(unsigned long long), 256);   // grid-barrier arrival counter
+    c->off_nve = off;  off = align_up(off + (size_t)(rbe::NVE_RED_CTAS + 1) * sizeof(double2), 256);   // partials + result of the NVE sums
     c->ws_bytes = off;
 
     c->stage_bytes = P * (sizeof(int4) + sizeof(double));
@@ -411,6 +428,14 @@ rbe_status launch_step(rbe_ctx* c, const int32_t* h_m, const void* d_xyzq, void*
         else RBE_CUDA(c, cudaLaunchKernelEx(&cfg, rbe::step_kernel<false, false>, sp));
     }
     return RBE_OK;
+}
+
+// Algorithm 1 steps 2-4 on the k-set in the workspace: the one-launch step kernel where it applies, else two launches
+rbe_status launch_kspace(rbe_ctx* c, const void* d_xyzq, void* d_force, int with_energy, cudaStream_t st) {
+    if (c->step_fused && c->xch_world == 0) return launch_step(c, nullptr, d_xyzq, d_force, with_energy, nullptr, st);
+    rbe_status s = launch_sf(c, d_xyzq, c->N, 0, 1, nullptr, st);
+    if (s == RBE_OK && c->N > 0) s = launch_f(c, d_xyzq, d_force, c->N, with_energy, st);
+    return s;
 }
 
 rbe_status check_kvectors(rbe_ctx* c, const int32_t* h_m, const double* h_w) {
@@ -661,8 +686,7 @@ rbe_status rbe_graph_capture(rbe_ctx* c, const void* d_xyzq, void* d_force, int3
     RBE_CUDA(c, cudaStreamBeginCapture(c->s_cap, cudaStreamCaptureModeThreadLocal));
     rbe_status s = launch_sampler(c, true, 0, 0, c->s_cap);
     c->have_w = false;   // the graph's batch carries the uniform weights S / P
-    if (s == RBE_OK) s = launch_sf(c, d_xyzq, c->N, 0, 1, nullptr, c->s_cap);
-    if (s == RBE_OK && c->N > 0) s = launch_f(c, d_xyzq, d_force, c->N, with_energy, c->s_cap);
+    if (s == RBE_OK) s = launch_kspace(c, d_xyzq, d_force, with_energy, c->s_cap);
     cudaGraph_t g = nullptr;
     const cudaError_t e = cudaStreamEndCapture(c->s_cap, &g);
     if (s != RBE_OK) { if (g) cudaGraphDestroy(g); return s; }
@@ -723,11 +747,12 @@ struct SrLayout {
     size_t off_acc = 0, off_gbox = 0;
     size_t bytes = 0;
 };
-bool sr_layout(const rbe_ctx* c, double rs, SrLayout& l) {
-    if (!c || !(rs > 0.0) || !std::isfinite(rs) || c->N >= ((int64_t)1 << 32)) return false;
-    const double ncd = std::floor(c->L / rs);
-    if (ncd < 3.0) return false;                       // the 27-cell stencil needs 3 distinct cells per dimension
-    l.nc = ncd > 512.0 ? 512 : (int)ncd;               // larger cells are still correct (side >= r_s)
+// cells of side >= cell_min; `need` distinct cells per dimension (the stencil must not meet itself around the box)
+bool sr_layout(const rbe_ctx* c, double cell_min, int need, SrLayout& l) {
+    if (!c || !(cell_min > 0.0) || !std::isfinite(cell_min) || c->N >= ((int64_t)1 << 32)) return false;
+    const double ncd = std::floor(c->L / cell_min);
+    if (ncd < (double)need) return false;
+    l.nc = ncd > 512.0 ? 512 : (int)ncd;               // larger cells are still correct (side >= cell_min)
     l.ncell = (int64_t)l.nc * l.nc * l.nc;
     const size_t N = (size_t)c->N, nce = (size_t)l.ncell;
     size_t off = 0;
@@ -748,7 +773,27 @@ bool sr_layout(const rbe_ctx* c, double rs, SrLayout& l) {
 
 size_t rbe_short_range_bytes(const rbe_ctx* c, double rs) {
     SrLayout l;
-    return sr_layout(c, rs, l) ? l.bytes : 0;
+    return sr_layout(c, rs, 3, l) ? l.bytes : 0;       // the 27-cell stencil needs 3 distinct cells per dimension
+}
+
+namespace {
+// Random batch list: cells of side >= r_c as Algorithm 2 says, but never so small that the stencil
+// exceeds 9^3 cells; R = cells the shell reaches beyond the atom's own; 2R + 1 distinct cells per dimension.
+bool rbl_layout(const rbe_ctx* c, double rc, double rs, SrLayout& l, int& R) {
+    if (!c || !(rc > 0.0) || !(rc < rs) || !std::isfinite(rs)) return false;
+    const double cell_min = rc > rs / 4.0 ? rc : rs / 4.0;
+    if (!sr_layout(c, cell_min, 3, l)) return false;
+    R = (int)std::ceil(rs / (c->L / l.nc) - 1e-12);
+    if (R < 1) R = 1;
+    if (R > 4 || 2 * R + 1 > l.nc) return false;
+    return true;
+}
+}  // namespace
+
+size_t rbe_rbl_bytes(const rbe_ctx* c, double rc, double rs) {
+    SrLayout l;
+    int R;
+    return rbl_layout(c, rc, rs, l, R) ? l.bytes : 0;
 }
 
 namespace {
@@ -760,10 +805,8 @@ struct SrBuffers {
     float* gbox;
 };
 // argument checks + the linked-cell list (bin, scan, scatter, sort) shared by rbe_short_range and rbe_rbl_forces
-rbe_status sr_build_cells(rbe_ctx* c, const char* who, const void* d_xyzq, double rs, void* d_force, void* d_ws,
-                          size_t ws_bytes, cudaStream_t st, SrLayout& l, SrBuffers& b) {
-    if (!sr_layout(c, rs, l))
-        return fail(c, RBE_ERR_INVALID_ARG, std::string(who) + ": need 0 < r_s <= L/3 (three cells of side >= r_s per dimension) and N < 2^32");
+rbe_status sr_build_cells(rbe_ctx* c, const char* who, const void* d_xyzq, void* d_force, void* d_ws,
+                          size_t ws_bytes, cudaStream_t st, const SrLayout& l, SrBuffers& b) {
     rbe_status s0 = init_device(c);
     if (s0 != RBE_OK) return s0;
     if (c->N == 0) return RBE_OK;
@@ -799,7 +842,9 @@ rbe_status rbe_short_range(rbe_ctx* c, const void* d_xyzq, double rs, void* d_fo
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     SrLayout l;
     SrBuffers b;
-    rbe_status s = sr_build_cells(c, "rbe_short_range", d_xyzq, rs, d_force, d_ws, ws_bytes, st, l, b);
+    if (!sr_layout(c, rs, 3, l))
+        return fail(c, RBE_ERR_INVALID_ARG, "rbe_short_range: need 0 < r_s <= L/3 (three cells of side >= r_s per dimension) and N < 2^32");
+    rbe_status s = sr_build_cells(c, "rbe_short_range", d_xyzq, d_force, d_ws, ws_bytes, st, l, b);
     if (s != RBE_OK || c->N == 0) return s;
     const unsigned nb = (unsigned)((c->N + 255) / 256);
     const float len_unit = (float)(c->L / rbe::TWO32);
@@ -827,19 +872,31 @@ rbe_status rbe_rbl_forces(rbe_ctx* c, const void* d_xyzq, double rc, double rs, 
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     SrLayout l;
     SrBuffers b;
-    rbe_status s = sr_build_cells(c, "rbe_rbl_forces", d_xyzq, rs, d_force, d_ws, ws_bytes, st, l, b);
+    int R = 0;
+    if (!rbl_layout(c, rc, rs, l, R))
+        return fail(c, RBE_ERR_INVALID_ARG, "rbe_rbl_forces: need r_s <= L/3 and a stencil of at most 9 cells of side max(r_c, r_s/4) per dimension that fits the box");
+    rbe_status s = sr_build_cells(c, "rbe_rbl_forces", d_xyzq, d_force, d_ws, ws_bytes, st, l, b);
     if (s != RBE_OK || c->N == 0) return s;
     RBE_CUDA(c, cudaMemsetAsync(b.acc, 0, 4 * sizeof(long long), st));
     rbe::RblParams rp;
     rp.sorted = b.sorted; rp.sidx = b.sidx; rp.start = b.start;
     rp.force = static_cast<float4*>(d_force);
     rp.fsum = b.acc;
-    rp.nc = l.nc; rp.p = p; rp.accumulate = accumulate;
+    rp.nc = l.nc; rp.R = R; rp.p = p; rp.accumulate = accumulate;
     rp.len_unit = (float)(c->L / rbe::TWO32);
     rp.rc2 = (float)(rc * rc); rp.rs2 = (float)(rs * rs);
     rp.sqrt_alpha = (float)std::sqrt(c->alpha);
-    rp.seed = seed; rp.step = step;
-    rbe::rbl_kernel<<<(unsigned)l.ncell, rbe::RBL_THREADS, 0, st>>>(rp);
+    // reading Q20: the per-step salt of the pair keys, one Philox4x32-10 call (counter (step, 0, 0), key seed)
+    uint32_t salt[4];
+    philox4x32_10_host((uint32_t)step, (uint32_t)(step >> 32), 0u, 0u, (uint32_t)seed, (uint32_t)(seed >> 32), salt);
+    rp.salt0 = salt[0]; rp.salt1 = salt[1];
+    // tile: 1.3 x the mean number of candidates of a cell, in steps of 256 (candidate indices are 15-bit: <= 8192)
+    const double mean_cand = (double)c->N / (double)l.ncell * (double)((2 * R + 1) * (2 * R + 1) * (2 * R + 1));
+    int tc = (int)std::ceil(1.3 * mean_cand / 256.0) * 256 + 256;
+    if (tc > rbe::RBL_TC_MAX) tc = rbe::RBL_TC_MAX;
+    rp.tc = tc;
+    RBE_CUDA(c, cudaFuncSetAttribute(rbe::rbl_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)rbe::rbl_smem_bytes(rbe::RBL_TC_MAX)));
+    rbe::rbl_kernel<<<(unsigned)l.ncell, rbe::RBL_THREADS, rbe::rbl_smem_bytes(tc), st>>>(rp);
     rbe::rbl_correct_kernel<<<(unsigned)((c->N + 255) / 256), 256, 0, st>>>(b.acc, c->N, static_cast<float4*>(d_force));
     RBE_CUDA(c, cudaGetLastError());
     return RBE_OK;
@@ -991,6 +1048,70 @@ rbe_status rbe_set_charges(rbe_ctx* c, const void* d_q) {
 rbe_status rbe_step_host_xyz(rbe_ctx* c, const float* h_xyz, const int32_t* h_m, const double* h_w, float* h_force3,
                              double* h_U, void* d_scratch, size_t scratch_bytes, void* stream) {
     return step_host_impl(c, h_xyz, h_m, h_w, h_force3, 0, h_U, d_scratch, scratch_bytes, stream, true);
+}
+
+rbe_status rbe_nve_kick(rbe_ctx* c, void* d_vel, const void* d_inv_mass, const void* d_force, double half_dt, void* d_pos,
+                        void* d_xyzq, double dt, void* stream) {
+    if (!c) return RBE_ERR_INVALID_ARG;
+    if (c->N == 0) return RBE_OK;
+    if (!d_vel || !d_inv_mass || !d_force || (d_pos && !d_xyzq) || (reinterpret_cast<uintptr_t>(d_force) & 15u) ||
+        (reinterpret_cast<uintptr_t>(d_xyzq) & 15u) || (reinterpret_cast<uintptr_t>(d_vel) & 7u) || (reinterpret_cast<uintptr_t>(d_pos) & 7u) ||
+        (reinterpret_cast<uintptr_t>(d_inv_mass) & 7u) || !std::isfinite(half_dt) || !std::isfinite(dt))
+        return fail(c, RBE_ERR_INVALID_ARG, "rbe_nve_kick: null or misaligned pointer, or a non-finite time step");
+    rbe::nve_kick_kernel<<<(unsigned)((c->N + 255) / 256), 256, 0, static_cast<cudaStream_t>(stream)>>>(
+        static_cast<double*>(d_vel), static_cast<const double*>(d_inv_mass), static_cast<const float4*>(d_force), half_dt,
+        static_cast<double*>(d_pos), static_cast<float4*>(d_xyzq), dt, c->N);
+    RBE_CUDA(c, cudaGetLastError());
+    return RBE_OK;
+}
+
+rbe_status rbe_nve_energies(rbe_ctx* c, const void* d_vel, const void* d_inv_mass, const void* d_force, double* h_out, void* stream) {
+    if (!c || !h_out) return fail(c, RBE_ERR_INVALID_ARG, "rbe_nve_energies: null argument");
+    if (!c->ws) return fail(c, RBE_ERR_NOT_READY, "rbe_nve_energies before rbe_set_workspace");
+    if ((d_vel && !d_inv_mass) || (reinterpret_cast<uintptr_t>(d_force) & 15u))
+        return fail(c, RBE_ERR_INVALID_ARG, "rbe_nve_energies: velocities without masses, or a misaligned pointer");
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    double2* part = ws_ptr<double2>(c, c->off_nve);
+    double* out = reinterpret_cast<double*>(part + rbe::NVE_RED_CTAS);
+    rbe::nve_energy_partial_kernel<<<rbe::NVE_RED_CTAS, 256, 0, st>>>(static_cast<const double*>(d_vel), static_cast<const double*>(d_inv_mass),
+                                                                      static_cast<const float4*>(d_force), c->N, part);
+    rbe::nve_energy_final_kernel<<<1, rbe::NVE_RED_CTAS, 0, st>>>(part, rbe::NVE_RED_CTAS, out);
+    RBE_CUDA(c, cudaGetLastError());
+    RBE_CUDA(c, cudaMemcpyAsync(h_out, out, 2 * sizeof(double), cudaMemcpyDeviceToHost, st));
+    RBE_CUDA(c, cudaStreamSynchronize(st));
+    return RBE_OK;
+}
+
+rbe_status rbe_md_capture(rbe_ctx* c, void* d_pos, void* d_vel, const void* d_inv_mass, void* d_xyzq, void* d_force, double rs, double dt,
+                          void* d_sr_ws, size_t sr_bytes, int32_t sampled, uint64_t seed, uint64_t first_step, int32_t with_energy) {
+    if (!c) return RBE_ERR_INVALID_ARG;
+    if (!c->ws) return fail(c, RBE_ERR_NOT_READY, "rbe_md_capture before rbe_set_workspace");
+    if (sampled && c->sampler_T.empty()) return fail(c, RBE_ERR_INVALID_ARG, "rbe_md_capture: the device sampler is unavailable for this L, alpha");
+    if (!sampled && !c->have_k) return fail(c, RBE_ERR_NOT_READY, "rbe_md_capture: no k-set (rbe_set_kvectors first, or sampled != 0)");
+    if (c->xch_world > 0) return fail(c, RBE_ERR_INVALID_ARG, "rbe_md_capture: not available with a fused exchange");
+    if (c->N < 1 || !d_pos || !d_vel || !d_inv_mass || !d_xyzq || !d_force || !(dt > 0.0) || !std::isfinite(dt))
+        return fail(c, RBE_ERR_INVALID_ARG, "rbe_md_capture: null pointer, empty system or bad time step");
+    if (c->graph_exec) { cudaGraphExecDestroy(c->graph_exec); c->graph_exec = nullptr; }
+    if (c->graph) { cudaGraphDestroy(c->graph); c->graph = nullptr; }
+    if (!c->s_cap) RBE_CUDA(c, cudaStreamCreateWithFlags(&c->s_cap, cudaStreamNonBlocking));
+    if (sampled) {
+        const unsigned long long st8[2] = {seed, first_step};
+        RBE_CUDA(c, cudaMemcpy(c->ws + c->off_state, st8, sizeof(st8), cudaMemcpyHostToDevice));
+    }
+    RBE_CUDA(c, cudaStreamBeginCapture(c->s_cap, cudaStreamCaptureModeThreadLocal));
+    // v(t+dt/2), x(t+dt)  ->  [a fresh batch]  ->  F_long  ->  + F_short  ->  v(t+dt)
+    rbe_status s = rbe_nve_kick(c, d_vel, d_inv_mass, d_force, 0.5 * dt, d_pos, d_xyzq, dt, c->s_cap);
+    if (s == RBE_OK && sampled) { s = launch_sampler(c, true, 0, 0, c->s_cap); c->have_w = false; }
+    if (s == RBE_OK) s = launch_kspace(c, d_xyzq, d_force, with_energy, c->s_cap);
+    if (s == RBE_OK) s = rbe_short_range(c, d_xyzq, rs, d_force, 1, with_energy, d_sr_ws, sr_bytes, c->s_cap);
+    if (s == RBE_OK) s = rbe_nve_kick(c, d_vel, d_inv_mass, d_force, 0.5 * dt, nullptr, nullptr, dt, c->s_cap);
+    cudaGraph_t g = nullptr;
+    const cudaError_t e = cudaStreamEndCapture(c->s_cap, &g);
+    if (s != RBE_OK) { if (g) cudaGraphDestroy(g); return s; }
+    if (e != cudaSuccess) return cuda_fail(c, "cudaStreamEndCapture", e);
+    c->graph = g;
+    RBE_CUDA(c, cudaGraphInstantiate(&c->graph_exec, c->graph, 0));
+    return RBE_OK;
 }
 
 rbe_status rbe_probe_pipe_rates(rbe_ctx* c, double* h_out, void* stream) {

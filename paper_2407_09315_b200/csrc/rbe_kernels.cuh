@@ -651,6 +651,8 @@ __device__ __forceinline__ float4 f_fetch(const FArgs& p, int64_t unit, int lane
 }
 
 // One pass: R units (R atoms per thread) against the nk wavevector records in shared memory.
+// (Tried: starting the record loop at a different k in every warp of a sub-partition, so that the warps do not
+// march in lock-step.  A stand-alone copy of this loop gained 6 % from it; inside the kernels it lost 1 %.)
 template <int R, bool ENERGY, bool ACCUM>
 __device__ __forceinline__ void f_pass(const FArgs& p, const int4* s_ka, const float4* s_kb, int nk, int64_t unit0, int lane) {
     uint32_t sx[R], sy[R], sz[R];

@@ -83,6 +83,8 @@ def lib():
         L.rbe_short_range_bytes.argtypes = [vp, dbl]
         L.rbe_short_range.restype = ctypes.c_int
         L.rbe_short_range.argtypes = [vp, vp, dbl, vp, i32, i32, vp, sz, vp]
+        L.rbe_rbl_bytes.restype = sz
+        L.rbe_rbl_bytes.argtypes = [vp, dbl, dbl]
         L.rbe_rbl_forces.restype = ctypes.c_int
         L.rbe_rbl_forces.argtypes = [vp, vp, dbl, dbl, i32, ctypes.c_uint64, ctypes.c_uint64, vp, i32, vp, sz, vp]
         L.rbe_structure_factor.restype = ctypes.c_int
@@ -97,6 +99,12 @@ def lib():
         L.rbe_step_host_bytes.argtypes = [vp, i32]
         L.rbe_probe_pipe_rates.restype = ctypes.c_int
         L.rbe_probe_pipe_rates.argtypes = [vp, vp, vp]
+        L.rbe_nve_kick.restype = ctypes.c_int
+        L.rbe_nve_kick.argtypes = [vp, vp, vp, vp, dbl, vp, vp, dbl, vp]
+        L.rbe_nve_energies.restype = ctypes.c_int
+        L.rbe_nve_energies.argtypes = [vp, vp, vp, vp, vp, vp]
+        L.rbe_md_capture.restype = ctypes.c_int
+        L.rbe_md_capture.argtypes = [vp, vp, vp, vp, vp, vp, dbl, dbl, vp, sz, i32, ctypes.c_uint64, ctypes.c_uint64, i32]
         L.rbe_kspace_energy.restype = ctypes.c_int
         L.rbe_kspace_energy.argtypes = [vp, ctypes.POINTER(dbl), vp]
         L.rbe_kspace_virial.restype = ctypes.c_int
@@ -305,6 +313,49 @@ class Rbe:
         return {"ffma": float(out[0]), "imad": float(out[1]), "i2fp": float(out[2]), "mufu": float(out[3]),
                 "sm_mhz": float(out[4])}
 
+    def rbe_nve_kick(self, vel, inv_mass, force, half_dt: float, pos=None, xyzq=None, dt: float = 0.0, stream=None):
+        """v += half_dt F / m; with pos (cuda float64 [N,3]) also x += dt v and xyzq[:, :3] = float32(x)."""
+        _check_tensor(vel, (self.N, 3), "float64")
+        _check_tensor(inv_mass, (self.N,), "float64")
+        _check_tensor(force, (self.N, 4), "float32")
+        if pos is not None:
+            _check_tensor(pos, (self.N, 3), "float64")
+            _check_tensor(xyzq, (self.N, 4), "float32")
+        self._check(lib().rbe_nve_kick(self._h, ctypes.c_void_p(vel.data_ptr()), ctypes.c_void_p(inv_mass.data_ptr()),
+                                       ctypes.c_void_p(force.data_ptr()), float(half_dt),
+                                       None if pos is None else ctypes.c_void_p(pos.data_ptr()),
+                                       None if pos is None else ctypes.c_void_p(xyzq.data_ptr()), float(dt), _stream_ptr(stream)))
+
+    def rbe_nve_energies(self, vel=None, inv_mass=None, force=None, stream=None):
+        """(kinetic energy, sum of force[:, 3]) in fp64, fixed order (synchronises)."""
+        import numpy as np
+        out = np.zeros(2, dtype=np.float64)
+        self._check(lib().rbe_nve_energies(self._h, None if vel is None else ctypes.c_void_p(vel.data_ptr()),
+                                           None if inv_mass is None else ctypes.c_void_p(inv_mass.data_ptr()),
+                                           None if force is None else ctypes.c_void_p(force.data_ptr()), _np_ptr(out),
+                                           _stream_ptr(stream)))
+        return float(out[0]), float(out[1])
+
+    def rbe_md_capture(self, pos, vel, inv_mass, xyzq, force, rs: float, dt: float, sampled: bool, seed: int = 0,
+                       first_step: int = 0, with_energy: bool = False):
+        import torch
+        _check_tensor(pos, (self.N, 3), "float64")
+        _check_tensor(vel, (self.N, 3), "float64")
+        _check_tensor(inv_mass, (self.N,), "float64")
+        _check_tensor(xyzq, (self.N, 4), "float32")
+        _check_tensor(force, (self.N, 4), "float32")
+        n = self.rbe_short_range_bytes(rs)
+        if n == 0:
+            raise RbeError(1, "rbe_md_capture: need 0 < r_s <= L/3")
+        if getattr(self, "_sr_ws", None) is None or self._sr_ws.numel() < n:
+            self._sr_ws = torch.empty(n, dtype=torch.uint8, device="cuda")
+        self._graph_buffers = (pos, vel, inv_mass, xyzq, force)
+        self._check(lib().rbe_md_capture(self._h, ctypes.c_void_p(pos.data_ptr()), ctypes.c_void_p(vel.data_ptr()),
+                                         ctypes.c_void_p(inv_mass.data_ptr()), ctypes.c_void_p(xyzq.data_ptr()),
+                                         ctypes.c_void_p(force.data_ptr()), float(rs), float(dt),
+                                         ctypes.c_void_p(self._sr_ws.data_ptr()), self._sr_ws.numel(), int(bool(sampled)),
+                                         int(seed), int(first_step), int(bool(with_energy))))
+
     def rbe_short_range_bytes(self, rs: float) -> int:
         return int(lib().rbe_short_range_bytes(self._h, float(rs)))
 
@@ -322,14 +373,17 @@ class Rbe:
                                           ctypes.c_void_p(force.data_ptr()), int(bool(accumulate)), int(bool(with_energy)),
                                           ctypes.c_void_p(self._sr_ws.data_ptr()), self._sr_ws.numel(), _stream_ptr(stream)))
 
+    def rbe_rbl_bytes(self, rc: float, rs: float) -> int:
+        return int(lib().rbe_rbl_bytes(self._h, float(rc), float(rs)))
+
     def rbe_rbl_forces(self, xyzq, rc: float, rs: float, p: int, seed: int, step: int, force, accumulate: bool = False, stream=None):
         """Random batch list estimate of the short-range force (Eqs. 2.13-2.16).  xyzq, force: cuda float32 [N,4]."""
         import torch
         _check_tensor(xyzq, (self.N, 4), "float32")
         _check_tensor(force, (self.N, 4), "float32")
-        n = self.rbe_short_range_bytes(rs)
+        n = self.rbe_rbl_bytes(rc, rs)
         if n == 0:
-            raise RbeError(1, "rbe_rbl_forces: need 0 < r_s <= L/3")
+            raise RbeError(1, "rbe_rbl_forces: need 0 < r_c < r_s <= L/3")
         if getattr(self, "_sr_ws", None) is None or self._sr_ws.numel() < n:
             self._sr_ws = torch.empty(n, dtype=torch.uint8, device="cuda")
         self._check(lib().rbe_rbl_forces(self._h, ctypes.c_void_p(xyzq.data_ptr()), float(rc), float(rs), int(p), int(seed),
