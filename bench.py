@@ -3,9 +3,11 @@
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--config NAME] [--impl reference]
 
-One *step* = one pass of the whole hot path over one batch of synthetic input:
-rbe_set_kvectors (a fresh, pre-generated k-set) + rbe_structure_factor (sf_kernel, which also
-runs the fixed-order second pass of the reduction) + rbe_forces (f_kernel): two launches.
+One *step* = one pass of the whole hot path over one batch of synthetic input: rbe_step with a
+fresh, pre-generated k-set = ONE cooperative launch (step_kernel: structure-factor phase, grid
+barrier, distributed fixed-order reduction, grid barrier, force phase; the k-set rides in the
+kernel parameters).  The two-launch form (rbe_set_kvectors + rbe_structure_factor + rbe_forces)
+is timed beside it, call by call.
 Workload at N = 1: BASELINE.json configs[2] (water + NaCl, N = 999 999, P = 200), the one the
 metric is quoted on.  With N > 1 GPUs (torchrun) the atoms are sharded, one rank per GPU, the
 k-set is replicated and the P complex structure factors are summed across ranks (weak
@@ -39,6 +41,36 @@ FP32_LANES_PER_SM = 128
 SFU_PER_PAIR_PER_KERNEL = 2
 FMA_PER_PAIR_STEP = 13
 BYTES_PER_ATOM_STEP = 48
+# what the kernels EXECUTE per (atom, k) pair: the SF phase pairs atoms of equal |q|
+# (3 MUFU per two pairs), the F phase uses the amplitude-phase form (1 MUFU per pair)
+MUFU_EXECUTED_PER_PAIR = {"sf": 1.5, "f": 1.0}
+
+
+def source_sha():
+    """Fingerprint of the kernel sources: ncu counters in profiles/kernel_counters.csv are tied to it."""
+    import hashlib
+    h = hashlib.sha256()
+    for f in ("rbe_kernels.cuh", "rbe_api.cu"):
+        h.update(open(os.path.join(ROOT, "paper_2407_09315_b200", "csrc", f), "rb").read())
+    return h.hexdigest()[:12]
+
+
+def read_counters(kernel, config):
+    """dram bytes / warp instructions per launch from ONE `ncu --set full` capture (profiles/kernel_counters.csv)."""
+    import csv
+    path = os.path.join(ROOT, "profiles", "kernel_counters.csv")
+    if not os.path.exists(path):
+        return None
+    for r in csv.DictReader(open(path)):
+        if r["kernel"] == kernel and r["config"] == config:
+            out = {"dram_bytes": float(r["dram_bytes"]), "inst_executed": float(r["inst_executed"]),
+                   "source_sha": r["source_sha"], "capture": r["capture"]}
+            out["stale"] = out["source_sha"] != source_sha()
+            if out["stale"]:
+                print(f"bench: profiles/kernel_counters.csv row {kernel}:{config} was captured at source {out['source_sha']}, "
+                      f"the kernels are now {source_sha()}: counters are stale", file=sys.stderr)
+            return out
+    return None
 
 
 def read_peaks():
@@ -106,13 +138,16 @@ class ClockSampler:
         return out
 
 
-def time_oracle(cfg_name, n_sample, steps, warmup):
+def time_oracle(cfg_name, n_sample, steps, warmup, threads=None):
     """The oracle as it stands, timed on the host cores, on the first n_sample atoms of the
     workload (cost is linear in atoms) with the workload's full batch of P wavevectors."""
     import oracle
     from paper_2407_09315_b200 import inputs
     cfg = workload_config(cfg_name, 1)
     atoms = inputs.make_atoms(cfg)[:n_sample].copy()
+    all_threads = oracle.max_threads()
+    if threads:
+        oracle.set_threads(threads)
     S = oracle.S(cfg.L, cfg.alpha)
     ts = []
     for it in range(warmup + steps):
@@ -124,7 +159,9 @@ def time_oracle(cfg_name, n_sample, steps, warmup):
         if it >= warmup:
             ts.append(dt)
     per_step = sum(ts) / len(ts)
-    return per_step, per_step / n_sample * 1e9, oracle.max_threads(), cfg
+    used = oracle.max_threads()
+    oracle.set_threads(all_threads)
+    return per_step, per_step / n_sample * 1e9, used, cfg
 
 
 def workload_config(name, world):
@@ -230,11 +267,13 @@ def main():
     xs = [torch.from_numpy(atoms).cuda() for _ in range(n_rot)]
     fs = [torch.empty((n_local, 4), dtype=torch.float32, device="cuda") for _ in range(n_rot)]
     n_k = args.warmup + args.steps
-    ksets = [inputs.sample_kset(L, alpha, P, base.seed, t) for t in range(n_k)]
+    ksets = [np.ascontiguousarray(inputs.sample_kset(L, alpha, P, base.seed, t), dtype=np.int32) for t in range(n_k)]
     rho_local = torch.empty((P, 2), dtype=torch.float64, device="cuda")
     gathered = torch.empty((world, P, 2), dtype=torch.float64, device="cuda") if world > 1 else None
 
-    def step(i, ev=None):
+    one_launch = world == 1 and bool(info["step_fused"])
+
+    def step_two(i, ev=None):
         x, f = xs[i % n_rot], fs[i % n_rot]
         ctx.rbe_set_kvectors(ksets[i % n_k])
         if ev: ev[0].record()
@@ -245,6 +284,37 @@ def main():
         if ev: ev[1].record()
         ctx.rbe_forces(x, f, args.with_energy)
         if ev: ev[2].record()
+
+    # rbe_step with the tensors marshalled once per buffer set (the per-step host cost matters for the small configs)
+    bound = [ctx.rbe_step_bound(xs[r], fs[r], with_energy=args.with_energy) for r in range(n_rot)] if world == 1 else None
+
+    def step(i, ev=None):
+        if world > 1:
+            return step_two(i, ev)
+        bound[i % n_rot](ksets[i % n_k])          # one launch (or two: large systems)
+
+    # N > 1: before anything is timed, one step through the fused exchange is checked against the NCCL sum
+    # (a mis-synchronised peer exchange that still arrives in time would otherwise give a timing line and no error)
+    exchange_used = "none" if world == 1 else ("fused" if fused else "nccl")
+    if fused:
+        ref = rbe.Rbe(n_local, L, alpha, P)
+        ref.rbe_set_kvectors(ksets[0])
+        ref.rbe_structure_factor(xs[0], rho_local)
+        dist.all_gather_into_tensor(gathered, rho_local)
+        ref.rbe_set_rho(gathered.sum(0))
+        u_ref = ref.rbe_kspace_energy()
+        step_two(0)
+        u_fused = ctx.rbe_kspace_energy()
+        ctx.rbe_exchange_check()
+        bad = torch.tensor([0.0 if u_fused == u_ref else 1.0], device="cuda")     # rank-ordered sums: bitwise equal
+        dist.all_reduce(bad, op=dist.ReduceOp.MAX)
+        if bad.item() > 0:
+            if rank == 0:
+                print(f"bench: fused exchange disagrees with the NCCL sum ({u_fused!r} vs {u_ref!r}); using NCCL", file=sys.stderr)
+            ctx.rbe_set_exchange(0, 0, None, 0)
+            fused = False
+            exchange_used = "nccl (fused exchange failed its cross-check)"
+        del ref
 
     def sync():
         if world > 1:
@@ -269,14 +339,22 @@ def main():
     sync()
     ms_total = e0.elapsed_time(e1)
 
-    # ---- timed region B: the same K steps with CUDA events around each call, for the
-    # per-kernel durations the roofline object needs
+    # ---- timed region B: the same K steps in the two-launch form with CUDA events around each call, for the
+    # per-kernel durations of sf_kernel and f_kernel
     evs = [[torch.cuda.Event(enable_timing=True) for _ in range(3)] for _ in range(args.steps)]
+    for i in range(3):
+        step_two(i)
     sync()
+    e2, e3 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e2.record()
     for i in range(args.steps):
-        step(args.warmup + i, evs[i])
+        step_two(args.warmup + i, evs[i])
+    e3.record()
     sync()
+    ms_two = e2.elapsed_time(e3) / args.steps
     clocks = sampler.stop() if rank == 0 else None
+    # issue rates of the pipes that bound the path, measured now on this device (rbe_probe_pipe_rates)
+    pipe = ctx.rbe_probe_pipe_rates() if rank == 0 else None
     if fused:
         ctx.rbe_exchange_check()   # raises if any kernel gave up waiting for a peer
     t_sf = [e[0].elapsed_time(e[1]) for e in evs]
@@ -331,15 +409,15 @@ def main():
               "r_s": args.rs, "neighbours_per_atom_expected": nbr, "calls": k_sr, "gpu_launches_per_call": 7,
               "pair_rate_G_per_s": nbr * n_local / (ms_sr * 1e-3) / 1e9,
               "rbl": {"ms_per_call": ms_rbl, "r_c": args.rs / 2, "p": 30,
-                      "note": "rbe_rbl_forces (Eqs. 2.13-2.16): first implementation, parity-exact batch; slower than "
-                              "the deterministic sum on B200 (DESIGN.md section 11)"},
+                      "note": "rbe_rbl_forces (Eqs. 2.13-2.16): cells of side r_c, warp per atom, parity-exact batch; still slower "
+                              "than the deterministic sum on B200 (instruction budget: profiles/r02_rbl_README.md)"},
               "note": "rbe_short_range: bin + scan + scatter + sort + group boxes + pair kernel (every unordered pair "
                       "once, fixed-point integer atomics across warps) + finalise; not part of `value`"}
 
     if world > 1:
-        t = torch.tensor([ms_total, ms_sf, ms_f], dtype=torch.float64, device="cuda")
+        t = torch.tensor([ms_total, ms_sf, ms_f, ms_two], dtype=torch.float64, device="cuda")
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms_total, ms_sf, ms_f = [float(v) for v in t.cpu()]
+        ms_total, ms_sf, ms_f, ms_two = [float(v) for v in t.cpu()]
     ms_step = ms_total / args.steps
     value = ms_step * 1e6 / n_total            # whole job: all atoms of all ranks per step time
 
@@ -413,14 +491,35 @@ def main():
         return
 
     peaks = read_peaks()
-    tr, sfu_rate = roofline_times(n_local, P, info["num_sms"], peaks)
+    tr, sfu_rate_nominal = roofline_times(n_local, P, info["num_sms"], peaks)
     t_roof = max(tr.values())
     pairs = n_local * P
-    sf_ops = SFU_PER_PAIR_PER_KERNEL * pairs
-    traffic = None
-    tpath = os.path.join(ROOT, "profiles", "traffic.json")
-    if os.path.exists(tpath):
-        traffic = json.load(open(tpath)).get(f"sf_kernel:{args.config}")
+    clk = peaks["sm_max_mhz"] * 1e6
+    sms = info["num_sms"]
+    # peaks: MEASURED lanes per SM per clock (this run) x SMs x the max SM clock
+    mufu_rate = pipe["mufu"] * sms * clk
+    issue_rate = 4 * sms * clk                     # warp instructions per second: 4 schedulers per SM, 1 per clock
+
+    def roof(kernel, ms, alg_per_pair, exe_per_pair):
+        """alu roofline of one kernel: algorithmic special-function evaluations (2 per pair per
+        phase) against the measured MUFU rate; beside it what the kernel executes, and its issue bound."""
+        cnt = read_counters(kernel, args.config)
+        t = ms * 1e-3
+        r = {"bound": "alu", "kernel": kernel, "achieved": alg_per_pair * pairs / t / 1e9, "peak": mufu_rate / 1e9,
+             "unit": "G sincos-evaluation/s, ALGORITHMIC count (2 per pair per phase) against the measured MUFU rate",
+             "frac": alg_per_pair * pairs / t / mufu_rate,
+             "executed": {"mufu_per_pair": exe_per_pair, "frac_of_mufu_peak": exe_per_pair * pairs / t / mufu_rate},
+             "traffic": None if cnt is None else cnt["dram_bytes"],
+             "peak_source": f"measured in this run: {pipe['mufu']:.2f} MUFU lanes/SM/clk (rbe_probe_pipe_rates) x {sms} SMs x "
+                            f"{peaks['sm_max_mhz']:.0f} MHz"}
+        if cnt is not None:
+            t_issue = cnt["inst_executed"] / issue_rate
+            r["executed"].update(warp_instructions=cnt["inst_executed"], issue_bound_us=t_issue * 1e6, frac_of_issue_bound=t_issue / t,
+                                 counters=cnt["capture"], counters_stale=cnt["stale"])
+        return r
+
+    main_kernel = "step_kernel" if one_launch else "sf_kernel"
+    main_ms = ms_step if one_launch else ms_sf
     out = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": False, "scaling": "weak",
@@ -430,29 +529,35 @@ def main():
                    "parallelism": f"atoms sharded over {world} GPU(s), k-set replicated" + (
                        "" if world == 1 else ", rho exchanged inside the kernels over NVLink peer memory (rbe_set_exchange)"
                        if fused else ", rho exchanged with NCCL all_gather + rank-ordered sum"),
+                   "exchange": exchange_used,
+                   "step": "rbe_step: one cooperative launch (step_kernel)" if one_launch else
+                           "rbe_set_kvectors + rbe_structure_factor + rbe_forces: two launches",
                    "launch": info, "with_energy": bool(args.with_energy)},
-        "kernels_ms": {"structure_factor_call": ms_sf, "forces_call": ms_f,
-                       "note": "region B (CUDA events around each C-ABI call); structure_factor_call = sf_kernel "
-                               "(incl. its in-kernel second pass), forces_call = f_kernel"},
-        "roofline": {
-            "bound": "alu", "kernel": "sf_kernel",
-            "achieved": sf_ops / (ms_sf * 1e-3) / 1e9, "peak": sfu_rate / 1e9, "unit": "G sincos-op/s (MUFU)",
-            "frac": (sf_ops / (ms_sf * 1e-3)) / sfu_rate, "traffic": traffic,
-            "peak_source": f"derived: {MUFU_LANES_PER_SM} MUFU lanes/SM/clk x {info['num_sms']} SMs x {peaks['sm_max_mhz']:.0f} MHz",
-        },
+        "kernels_ms": {"step_call": ms_step, "two_launch_step": ms_two, "structure_factor_call": ms_sf, "forces_call": ms_f,
+                       "note": "step_call = region A (rbe_step); the rest = region B, the two-launch form with CUDA events around "
+                               "each C-ABI call: structure_factor_call = sf_kernel (incl. its in-kernel second pass), forces_call = f_kernel"},
+        "peaks": {"lanes_per_sm_per_clk": {k: pipe[k] for k in ("ffma", "imad", "i2fp", "mufu")},
+                  "sm_mhz_during_probe": pipe["sm_mhz"], "sm_max_mhz": peaks["sm_max_mhz"], "hbm_gbs": peaks["hbm_gbs"],
+                  "hbm_source": peaks["src"] + " (MEASURED_PEAKS.json)" if peaks["src"] == "measured" else peaks["src"],
+                  "how": "rbe_probe_pipe_rates: dependent-free chains, 32 warps per SM, in-kernel clock64, in this run"},
+        "roofline": roof(main_kernel, main_ms, 2 * SFU_PER_PAIR_PER_KERNEL if one_launch else SFU_PER_PAIR_PER_KERNEL,
+                         MUFU_EXECUTED_PER_PAIR["sf"] + (MUFU_EXECUTED_PER_PAIR["f"] if one_launch else 0.0)),
+        "roofline_kernels": [roof("sf_kernel", ms_sf, SFU_PER_PAIR_PER_KERNEL, MUFU_EXECUTED_PER_PAIR["sf"]),
+                             roof("f_kernel", ms_f, SFU_PER_PAIR_PER_KERNEL, MUFU_EXECUTED_PER_PAIR["f"])],
         "roofline_step": {
             "t_roof_us": t_roof * 1e6, "t_hbm_us": tr["hbm"] * 1e6, "t_fma_us": tr["fma"] * 1e6, "t_sfu_us": tr["sfu"] * 1e6,
             "frac": t_roof / (ms_step * 1e-3), "ns_per_atom_at_roofline": t_roof * 1e9 / n_local,
             "hbm_peak_gbs": peaks["hbm_gbs"], "peaks": peaks["src"],
-            "note": "SURVEY.md s8(d): 4 sincos + 13 FMA per (atom,k) pair per step, 48 B per atom",
+            "note": "SURVEY.md s8(d): 4 sincos + 13 FMA per (atom,k) pair per step, 48 B per atom, at the NOMINAL 16 MUFU / 128 FP32 "
+                    "lanes per SM per clock (the survey's figures; `roofline` uses the rates measured in this run)",
         },
         "graph_step": None if ms_graph is None else {
-            "ms_per_step": ms_graph, "value": ms_graph * 1e6 / n_total, "unit": UNIT, "gpu_launches_per_step": 1,
-            "note": "rbe_graph_launch: device sampler (Philox) + sf_kernel + f_kernel replayed as one CUDA graph, "
+            "ms_per_step": ms_graph, "value": ms_graph * 1e6 / n_total, "unit": UNIT, "gpu_launches_per_step": 2 if one_launch else 3,
+            "note": "rbe_graph_launch: device sampler (Philox) + the k-space step replayed as one CUDA graph, "
                     "no per-step H2D; not the headline (the k-set there comes from the host each step)"},
         "short_range": sr,
         "clocks": clocks,
-        "gpu_launches": 2 * args.steps,
+        "gpu_launches": (1 if one_launch else 2) * args.steps,
         "paper_context": "8.20 ms/step, 1e6 atoms, A100, RBL+RBE nonbonded total, P=100 (PAPER.md P:284); 2.89 ms k-space at 1e5 atoms, P=200 (P:266)",
     }
     if e2e:
@@ -461,7 +566,12 @@ def main():
         n_s = min(args.cpu_baseline_atoms, base.N)
         k_cpu = max(1, args.cpu_baseline_steps)
         per_step, ns_cpu, cores, _ = time_oracle(args.config, n_s, k_cpu, 1)
+        # the same oracle on ONE thread, on a sample sized for ~5 s: a bare core count would mislead
+        n_1 = max(1000, min(n_s, 25_000))
+        per_step1, ns_cpu1, _, _ = time_oracle(args.config, n_1, 1, 1, threads=1)
         out["cpu_baseline"] = {"value": ns_cpu, "unit": UNIT, "cores": cores, "kind": "oracle",
+                               "one_thread": {"value": ns_cpu1, "unit": UNIT, "sample_atoms": n_1},
+                               "speedup_all_threads_vs_one": ns_cpu1 / ns_cpu,
                                "sample": f"first {n_s} atoms of {base.name} (N={base.N}), all P={P} wavevectors, oracle.rho + "
                                          f"oracle.force, {k_cpu} steps after 1 warm-up ({per_step * k_cpu:.1f} s of CPU work)"}
     print(json.dumps(out))

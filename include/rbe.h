@@ -258,7 +258,8 @@ rbe_status rbe_short_range(rbe_ctx* ctx, const void* d_xyzq, double rs, void* d_
  * -- a uniformly random p-subset, a pure function of (seed, step), distinct keys for distinct j.  N_s <= p:
  * the whole shell, scale 1.  Cell list with cells of side max(r_c, r_s / 4) (Algorithm 2: side r_c),
  * one CTA per cell, a warp per atom.  Forces only (d_force[i].w = 0, or unchanged with accumulate).
- * 1 <= p <= 32, 0 < rc < rs <= L/3.  d_ws: caller-owned scratch of rbe_rbl_bytes(ctx, rc, rs) bytes (~76 B per atom
+ * 1 <= p <= 32, 0 < rc < rs, and the 2R + 1 cells of side c = L / floor(L / max(r_c, r_s / 4)) that the shell spans
+ * (R = ceil(r_s / c) <= 4) must fit the box (r_s below about 0.44 L).  d_ws: caller-owned scratch of rbe_rbl_bytes(ctx, rc, rs) bytes (~76 B per atom
  * + 204 B per cell), 256-byte aligned; rbe_rbl_bytes returns 0 for invalid radii.  Bitwise reproducible.
  * Errors: RBE_ERR_INVALID_ARG, RBE_ERR_WORKSPACE, RBE_ERR_NO_DEVICE, RBE_ERR_CUDA. */
 size_t     rbe_rbl_bytes(const rbe_ctx* ctx, double rc, double rs);

@@ -874,7 +874,7 @@ rbe_status rbe_rbl_forces(rbe_ctx* c, const void* d_xyzq, double rc, double rs, 
     SrBuffers b;
     int R = 0;
     if (!rbl_layout(c, rc, rs, l, R))
-        return fail(c, RBE_ERR_INVALID_ARG, "rbe_rbl_forces: need r_s <= L/3 and a stencil of at most 9 cells of side max(r_c, r_s/4) per dimension that fits the box");
+        return fail(c, RBE_ERR_INVALID_ARG, "rbe_rbl_forces: the shell must span at most 9 cells of side max(r_c, r_s/4) per dimension, and they must fit the box");
     rbe_status s = sr_build_cells(c, "rbe_rbl_forces", d_xyzq, d_force, d_ws, ws_bytes, st, l, b);
     if (s != RBE_OK || c->N == 0) return s;
     RBE_CUDA(c, cudaMemsetAsync(b.acc, 0, 4 * sizeof(long long), st));

@@ -302,6 +302,28 @@ class Rbe:
                                    ctypes.c_void_p(force.data_ptr()), int(bool(with_energy)),
                                    None if rho is None else ctypes.c_void_p(rho.data_ptr()), _stream_ptr(stream)))
 
+    def rbe_step_bound(self, xyzq, force, with_energy: bool = False, rho=None, stream=None):
+        """rbe_step with everything but the k-set marshalled ONCE: returns call(m) for m a C-contiguous numpy int32
+        [P,3] array.  For loops whose per-step host cost matters (small systems are launch-bound): the call is one
+        ctypes transition, no tensor checks."""
+        import numpy as np
+        _check_tensor(xyzq, (self.N, 4), "float32")
+        _check_tensor(force, (self.N, 4), "float32")
+        if rho is not None:
+            _check_tensor(rho, (self.P, 2), "float64")
+        fn, h, st = lib().rbe_step, self._h, _stream_ptr(stream)
+        px, pf = ctypes.c_void_p(xyzq.data_ptr()), ctypes.c_void_p(force.data_ptr())
+        pr = None if rho is None else ctypes.c_void_p(rho.data_ptr())
+        we, shape = int(bool(with_energy)), (self.P, 3)
+        keep = (xyzq, force, rho)
+
+        def call(m):
+            assert m.dtype == np.int32 and m.shape == shape and m.flags["C_CONTIGUOUS"] and keep is not None
+            status = fn(h, m.ctypes.data, None, px, pf, we, pr, st)
+            if status != RBE_OK:
+                self._check(status)
+        return call
+
     def rbe_step_host_bytes(self, compact: bool) -> int:
         return int(lib().rbe_step_host_bytes(self._h, int(bool(compact))))
 

@@ -87,6 +87,32 @@ def test_kvector_validation_and_call_order(lib):
     assert lib.rbe_destroy(h) == 0
 
 
+def test_size_queries_need_no_device(lib):
+    """rbe_step_host_bytes / rbe_short_range_bytes / rbe_rbl_bytes are pure functions of the context (the binding
+    sizes its scratch buffers with them instead of repeating the layout)."""
+    lib.rbe_step_host_bytes.restype = ctypes.c_size_t
+    lib.rbe_rbl_bytes.restype = ctypes.c_size_t
+    lib.rbe_short_range_bytes.restype = ctypes.c_size_t
+    h = ctypes.c_void_p()
+    N = 100_003
+    assert lib.rbe_create(ctypes.byref(h), N, 60.0, 0.09, 8) == 0
+    b4, b3 = lib.rbe_step_host_bytes(h, 0), lib.rbe_step_host_bytes(h, 1)
+    assert 32 * N <= b4 <= 32 * N + 1024 and 56 * N <= b3 <= 56 * N + 2048 and b4 % 256 == 0 and b3 % 256 == 0
+    assert lib.rbe_step_host_bytes(None, 0) == 0
+    assert lib.rbe_short_range_bytes(h, ctypes.c_double(10.0)) > 76 * N
+    assert lib.rbe_short_range_bytes(h, ctypes.c_double(21.0)) == 0                 # r_s > L/3
+    assert lib.rbe_rbl_bytes(h, ctypes.c_double(5.0), ctypes.c_double(10.0)) > lib.rbe_short_range_bytes(h, ctypes.c_double(10.0))
+    assert lib.rbe_rbl_bytes(h, ctypes.c_double(10.0), ctypes.c_double(5.0)) == 0   # r_c >= r_s
+    assert lib.rbe_rbl_bytes(h, ctypes.c_double(5.0), ctypes.c_double(21.0)) > 0    # 9 cells of 5.45 A fit the 60 A box
+    assert lib.rbe_rbl_bytes(h, ctypes.c_double(5.0), ctypes.c_double(29.0)) == 0   # the stencil would meet itself
+    # the one-launch step and the NVE calls refuse to run without a workspace (no CUDA call is made)
+    m = np.array([[1, 0, 0]] * 8, dtype=np.int32)
+    assert lib.rbe_step(h, ctypes.c_void_p(m.ctypes.data), None, None, None, 0, None, None) == 3
+    out = (ctypes.c_double * 2)()
+    assert lib.rbe_nve_energies(h, None, None, None, out, None) == 3
+    assert lib.rbe_destroy(h) == 0
+
+
 def test_no_cpu_fallback_without_device(lib):
     """On a box without a GPU the product path must fail loudly, never compute on the CPU."""
     import torch

@@ -31,6 +31,13 @@ def test_bench_json_line_contract():
     e = d["e2e"]
     assert e["value"] > d["value"] and e["h2d_bytes_per_step"] >= 12 * 96000 and e["d2h_bytes_per_step"] == 12 * 96000
     assert e["float4_ms_per_step"] > 0
-    assert d["gpu_launches"] == 2 * 5
+    assert d["gpu_launches"] == 1 * 5 and d["config"]["launch"]["step_fused"] == 1      # one cooperative launch per step
     assert set(d["clocks"]) >= {"sm_mhz", "sm_max_mhz", "reasons"}
-    assert d["graph_step"]["gpu_launches_per_step"] == 1 and d["short_range"]["ms_per_call"] > 0
+    assert d["graph_step"]["gpu_launches_per_step"] == 2 and d["short_range"]["ms_per_call"] > 0
+    # hygiene keys of round 2: peaks measured in the same run, executed-work fractions, both kernels, one-thread oracle
+    lanes = d["peaks"]["lanes_per_sm_per_clk"]
+    assert 14.0 <= lanes["mufu"] <= 16.5 and 110.0 <= lanes["ffma"] <= 130.0 and 55.0 <= lanes["imad"] <= 66.0
+    assert r["kernel"] == "step_kernel" and r["executed"]["mufu_per_pair"] == 2.5 and "measured in this run" in r["peak_source"]
+    assert [k["kernel"] for k in d["roofline_kernels"]] == ["sf_kernel", "f_kernel"]
+    assert c["one_thread"]["value"] > 0 and c["speedup_all_threads_vs_one"] > 0
+    assert d["kernels_ms"]["two_launch_step"] > 0 and d["kernels_ms"]["step_call"] == d["ms_per_step"]
