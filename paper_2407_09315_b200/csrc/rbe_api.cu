@@ -73,6 +73,7 @@ struct rbe_ctx {
     cudaStream_t s_cap = nullptr;
     cudaGraph_t graph = nullptr;
     cudaGraphExec_t graph_exec = nullptr;
+    bool graph_have_w = false;   // whether the captured step reads the weight table (a replay leaves the context in that state)
 
     // fused multi-GPU exchange of rho (rbe_set_exchange): peers' buffers, this rank, step epoch
     int32_t xch_world = 0, xch_rank = 0;
@@ -692,6 +693,7 @@ rbe_status rbe_graph_capture(rbe_ctx* c, const void* d_xyzq, void* d_force, int3
     if (s != RBE_OK) { if (g) cudaGraphDestroy(g); return s; }
     if (e != cudaSuccess) return cuda_fail(c, "cudaStreamEndCapture", e);
     c->graph = g;
+    c->graph_have_w = false;
     RBE_CUDA(c, cudaGraphInstantiate(&c->graph_exec, c->graph, 0));
     return RBE_OK;
 }
@@ -700,7 +702,7 @@ rbe_status rbe_graph_launch(rbe_ctx* c, void* stream) {
     if (!c) return RBE_ERR_INVALID_ARG;
     if (!c->graph_exec) return fail(c, RBE_ERR_NOT_READY, "rbe_graph_launch before rbe_graph_capture");
     RBE_CUDA(c, cudaGraphLaunch(c->graph_exec, static_cast<cudaStream_t>(stream)));
-    c->have_k = true; c->have_w = false; c->have_rho = true;
+    c->have_k = true; c->have_w = c->graph_have_w; c->have_rho = true;
     return RBE_OK;
 }
 
@@ -1110,6 +1112,7 @@ rbe_status rbe_md_capture(rbe_ctx* c, void* d_pos, void* d_vel, const void* d_in
     if (s != RBE_OK) { if (g) cudaGraphDestroy(g); return s; }
     if (e != cudaSuccess) return cuda_fail(c, "cudaStreamEndCapture", e);
     c->graph = g;
+    c->graph_have_w = c->have_w;     // sampled: cleared above; else the weights of the k-set the caller uploaded
     RBE_CUDA(c, cudaGraphInstantiate(&c->graph_exec, c->graph, 0));
     return RBE_OK;
 }

@@ -141,6 +141,24 @@ def rocksalt(ncells: int, a: float = 5.64, seed: int = 7, jitter: float = 0.05, 
     return x, v, q, mass, float(ncells * a)
 
 
+def plasma(ncells: int, a: float = 4.0, seed: int = 7, jitter: float = 0.05, v_rms: float = 0.0):
+    """A one-component plasma for LONG NVE runs: ncells^3 body-centred cubic cells of side a [A]
+    (2 ions each), every ion with charge +1 e and the mass of Na; the k = 0 term is absent from Eq. (2.8), i.e. a
+    uniform neutralising background is implied (reading Q8), and it exerts no force.  Like charges repel, so -- unlike
+    the rock-salt crystal -- nothing collapses on a path without a repulsive core, and the energy error of a long run
+    measures the integrator and the random batch only.  Displacements, velocities and return values as rocksalt()."""
+    rng = np.random.default_rng(seed)
+    cells = np.stack(np.meshgrid(*[np.arange(ncells)] * 3, indexing="ij"), axis=-1).reshape(-1, 1, 3)
+    x = (cells + np.array([[0.0, 0.0, 0.0], [0.5, 0.5, 0.5]])[None]).reshape(-1, 3) * a
+    n = x.shape[0]
+    q = np.ones(n, dtype=np.float32)
+    mass = np.full(n, MASS_NA)
+    x = x + jitter * rng.standard_normal((n, 3))
+    v = v_rms * rng.standard_normal((n, 3)) / np.sqrt(mass)[:, None]
+    v -= (mass[:, None] * v).sum(0) / mass.sum()
+    return x, v, q, mass, float(ncells * a)
+
+
 def pmf_1d(L: float, alpha: float):
     """(support m = -M..M, probabilities) of the 1-D discrete Gaussian exp(-pi^2 m^2/(alpha L^2))."""
     c = np.pi ** 2 / (alpha * L * L)

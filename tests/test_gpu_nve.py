@@ -83,6 +83,15 @@ def test_deterministic_ewald_trajectory_matches_the_oracle():
     torch.cuda.synchronize()
     assert torch.equal(pos2, pos) and torch.equal(vel2, vel) and torch.equal(force2, force)
 
+    # a replay leaves the context on the WEIGHTED k-set it was captured with (regression: rbe_graph_launch used to
+    # switch the context back to the uniform weights S/P, so an energy evaluated between replays was wrong)
+    tmp = torch.empty_like(force2)
+    ctx.rbe_step(None, xyzq2, tmp)
+    ref = rbe.Rbe(x.shape[0], L, alpha, m.shape[0])
+    ref.rbe_set_kvectors(m, w)
+    ref.rbe_step(None, xyzq2, tmp)
+    assert ctx.rbe_kspace_energy() == ref.rbe_kspace_energy()
+
 
 def test_random_batch_trajectory_with_the_device_sampler_matches_the_oracle():
     """Eq. (2.12) forces from a fresh batch of P = 100 wavevectors per step, drawn on the device (bit-exact against
