@@ -394,6 +394,18 @@ def main():
         e1.record()
         sync()
         ms_sr = e0.elapsed_time(e1) / k_sr
+        # the same sum with the paper's tabulated pair term instead of the polynomial erfc (rbe_set_pair_table)
+        ctx.rbe_set_pair_table(True)
+        for i in range(2):
+            ctx.rbe_short_range(xs[i % n_rot], args.rs, fs[i % n_rot])
+        sync()
+        e0.record()
+        for i in range(k_sr):
+            ctx.rbe_short_range(xs[i % n_rot], args.rs, fs[i % n_rot])
+        e1.record()
+        sync()
+        ms_sr_tab = e0.elapsed_time(e1) / k_sr
+        ctx.rbe_set_pair_table(False)
         # the paper's own estimator of the same force: random batch list, r_c = r_s / 2, p = 30
         for i in range(2):
             ctx.rbe_rbl_forces(xs[i % n_rot], args.rs / 2, args.rs, 30, base.seed, i, fs[i % n_rot])
@@ -408,6 +420,8 @@ def main():
         sr = {"ms_per_call": ms_sr, "value": ms_sr * 1e6 / n_local, "unit": UNIT.replace("/step", "/call"),
               "r_s": args.rs, "neighbours_per_atom_expected": nbr, "calls": k_sr, "gpu_launches_per_call": 7,
               "pair_rate_G_per_s": nbr * n_local / (ms_sr * 1e-3) / 1e9,
+              "pair_table": {"ms_per_call": ms_sr_tab, "note": "rbe_set_pair_table(1): tabulated pair term with cubic interpolation "
+                             "(P:196) instead of the degree-8 polynomial erfc; one more launch (the table is rebuilt per call)"},
               "rbl": {"ms_per_call": ms_rbl, "r_c": args.rs / 2, "p": 30,
                       "note": "rbe_rbl_forces (Eqs. 2.13-2.16): cells of side r_c, warp per atom, parity-exact batch; still slower "
                               "than the deterministic sum on B200 (instruction budget: profiles/r02_rbl_README.md)"},

@@ -39,6 +39,7 @@ struct rbe_ctx {
     rbe_launch_info li{};
     int sf_gs = 0, sf_ng = 0;
     int sf_pairing = 3;
+    int sr_table = 0;          // rbe_set_pair_table
     int sf_ngroups = 1;
     size_t ws_bytes = 0;
     size_t off_kvec = 0, off_w = 0, off_part = 0, off_rho = 0, off_grow = 0, off_U = 0, off_ticket = 0;
@@ -529,6 +530,13 @@ rbe_status rbe_set_pairing(rbe_ctx* c, int32_t mode) {
     return RBE_OK;
 }
 
+rbe_status rbe_set_pair_table(rbe_ctx* c, int32_t on) {
+    if (!c) return RBE_ERR_INVALID_ARG;
+    if (on != 0 && on != 1) return fail(c, RBE_ERR_INVALID_ARG, "rbe_set_pair_table: on must be 0 or 1");
+    c->sr_table = on;
+    return RBE_OK;
+}
+
 rbe_status rbe_get_launch_info(const rbe_ctx* c, rbe_launch_info* out) {
     if (!c || !out) return RBE_ERR_INVALID_ARG;
     if (!c->dev_ready) return RBE_ERR_NOT_READY;
@@ -746,7 +754,7 @@ struct SrLayout {
     int nc = 0;
     int64_t ncell = 0;
     size_t off_turns = 0, off_sorted = 0, off_cell = 0, off_order = 0, off_sidx = 0, off_count = 0, off_cursor = 0, off_start = 0;
-    size_t off_acc = 0, off_gbox = 0;
+    size_t off_acc = 0, off_gbox = 0, off_tab = 0;
     size_t bytes = 0;
 };
 // cells of side >= cell_min; `need` distinct cells per dimension (the stencil must not meet itself around the box)
@@ -768,6 +776,7 @@ bool sr_layout(const rbe_ctx* c, double cell_min, int need, SrLayout& l) {
     l.off_start = off;  off = align_up(off + (nce + 1) * sizeof(uint32_t), 256);
     l.off_acc = off;    off = align_up(off + N * 4 * sizeof(long long), 256);
     l.off_gbox = off;   off = align_up(off + nce * rbe::SR_GMAX * 6 * sizeof(float), 256);
+    l.off_tab = off;    off = align_up(off + 2 * (size_t)rbe::SR_TAB_MAX * sizeof(float4), 256);   // pair-term tables (force, energy)
     l.bytes = off;
     return true;
 }
@@ -805,6 +814,7 @@ struct SrBuffers {
     uint32_t *order, *sidx, *count, *cursor, *start;
     long long* acc;
     float* gbox;
+    float4* tab;
 };
 // argument checks + the linked-cell list (bin, scan, scatter, sort) shared by rbe_short_range and rbe_rbl_forces
 rbe_status sr_build_cells(rbe_ctx* c, const char* who, const void* d_xyzq, void* d_force, void* d_ws,
@@ -827,6 +837,7 @@ rbe_status sr_build_cells(rbe_ctx* c, const char* who, const void* d_xyzq, void*
     b.start = reinterpret_cast<uint32_t*>(w + l.off_start);
     b.acc = reinterpret_cast<long long*>(w + l.off_acc);
     b.gbox = reinterpret_cast<float*>(w + l.off_gbox);
+    b.tab = reinterpret_cast<float4*>(w + l.off_tab);
     const unsigned nb = (unsigned)((c->N + 255) / 256);
     RBE_CUDA(c, cudaMemsetAsync(b.count, 0, (size_t)l.ncell * sizeof(uint32_t), st));
     rbe::sr_bin_kernel<<<nb, 256, 0, st>>>(static_cast<const float4*>(d_xyzq), c->N, rbe::TWO32 / c->L, l.nc, b.turns, b.cell_of, b.count);
@@ -859,8 +870,28 @@ rbe_status rbe_short_range(rbe_ctx* c, const void* d_xyzq, double rs, void* d_fo
     pp.cell_len = (float)(c->L / l.nc);
     pp.rs2 = (float)(rs * rs);
     pp.sqrt_alpha = (float)std::sqrt(c->alpha);
-    if (with_energy) rbe::sr_pair_kernel<true><<<(unsigned)l.ncell, 32 * rbe::SR_PAIR_WARPS, 0, st>>>(pp);
-    else rbe::sr_pair_kernel<false><<<(unsigned)l.ncell, 32 * rbe::SR_PAIR_WARPS, 0, st>>>(pp);
+    pp.nalpha_log2e = (float)(-c->alpha * 1.4426950408889634);
+    // the pair-term table: the octaves of u = r^2 from 2^EMIN up to r_s^2 (only pairs with r^2 < r_s^2 look it up)
+    const int emax = (int)std::floor(std::log2(rs * rs)) + 1;
+    int ntab = (emax - rbe::SR_TAB_EMIN) << rbe::SR_TAB_BITS;
+    if (ntab < (1 << rbe::SR_TAB_BITS)) ntab = 1 << rbe::SR_TAB_BITS;
+    if (ntab > rbe::SR_TAB_MAX) return fail(c, RBE_ERR_INVALID_ARG, "rbe_short_range: r_s too large for the pair-term table");
+    pp.ntab = ntab;
+    pp.tab_f = b.tab; pp.tab_e = b.tab + rbe::SR_TAB_MAX;
+    pp.tab_umin = (float)std::ldexp(1.0, rbe::SR_TAB_EMIN);
+    const bool table = c->sr_table != 0;
+    const size_t dyn = rbe::sr_pair_smem_bytes(ntab, table, with_energy != 0);
+    const unsigned grid = (unsigned)l.ncell, block = 32 * rbe::SR_PAIR_WARPS;
+    if (table) {
+        rbe::sr_table_kernel<<<(unsigned)((ntab + 127) / 128), 128, 0, st>>>(b.tab, b.tab + rbe::SR_TAB_MAX, ntab, c->alpha);
+        RBE_CUDA(c, cudaFuncSetAttribute(rbe::sr_pair_kernel<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 2 * rbe::SR_TAB_MAX * (int)sizeof(float4)));
+        RBE_CUDA(c, cudaFuncSetAttribute(rbe::sr_pair_kernel<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, rbe::SR_TAB_MAX * (int)sizeof(float4)));
+        if (with_energy) rbe::sr_pair_kernel<true, true><<<grid, block, dyn, st>>>(pp);
+        else rbe::sr_pair_kernel<false, true><<<grid, block, dyn, st>>>(pp);
+    } else {
+        if (with_energy) rbe::sr_pair_kernel<true, false><<<grid, block, 0, st>>>(pp);
+        else rbe::sr_pair_kernel<false, false><<<grid, block, 0, st>>>(pp);
+    }
     rbe::sr_finalize_kernel<<<nb, 256, 0, st>>>(b.acc, b.sorted, b.sidx, c->N, static_cast<float4*>(d_force), accumulate, with_energy);
     RBE_CUDA(c, cudaGetLastError());
     return RBE_OK;

@@ -39,6 +39,11 @@ struct SrPairParams {
     float cell_len;           // L / nc [A]
     float rs2;                // r_s^2 [A^2]
     float sqrt_alpha;
+    float nalpha_log2e;       // -alpha log2(e)
+    float tab_umin;           // below this r^2 the analytic branch is taken [A^2]
+    const float4* tab_f;      // [ntab] cubic coefficients of T_f per interval (sr_table_kernel)
+    const float4* tab_e;      // [ntab] ... of T_e
+    int32_t ntab;
 };
 
 __device__ __forceinline__ uint32_t sr_cell_centre(int cd, int nc) {
@@ -74,6 +79,57 @@ __device__ __forceinline__ void sr_atomic_add_fixed(long long* p, float v) {
     atomicAdd(reinterpret_cast<unsigned long long*>(p), (unsigned long long)__double2ll_rn((double)v * SR_FIXED_SCALE));
 }
 
+// ---------------------------------------------------------------------------------------
+// The pair-term table (PAPER.md: tabulated erfc / exp with interpolation above a small radius, the series
+// below it).  Tabulated over u = r^2, so no square root is needed:
+//   T_f(u) = e^{alpha u} g(r) / r = [erfcx(sqrt(alpha u)) / sqrt(u) + 2 sqrt(alpha / pi)] / u      (force, Eq. 2.10)
+//   T_e(u) = e^{alpha u} erfc(sqrt(alpha) r) / r = erfcx(sqrt(alpha u)) / sqrt(u)                  (energy, Eq. 2.8)
+// The Gaussian is factored out (one MUFU.EX2 per pair) so that what is tabulated behaves like a power of u at any
+// alpha r_s^2, and intervals of constant RELATIVE width keep a constant relative error: interval i covers
+// u in 2^e (1 + m / 32) + [0, 2^e / 32), e = SR_TAB_EMIN + i / 32, m = i % 32 -- the index is the top bits of the fp32
+// pattern of u, the interval origin is u with the low mantissa bits cleared.  Per interval a cubic in (u - origin)
+// through the four Chebyshev nodes (fp64, erfcx from the CUDA math library); its interpolation error is
+// <= 2e-7 relative.  Pairs closer than 2^(EMIN / 2) = 0.125 A take the analytic branch.
+// ---------------------------------------------------------------------------------------
+constexpr int SR_TAB_EMIN = -6;          // the table starts at u = 2^-6 A^2 (r = 0.125 A)
+constexpr int SR_TAB_BITS = 5;           // 32 intervals per octave of u
+constexpr int SR_TAB_MAX = 1024;         // entries per table the workspace holds (32 octaves)
+
+__global__ void __launch_bounds__(128) sr_table_kernel(float4* __restrict__ tf, float4* __restrict__ te, int n, double alpha) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const double base = ldexp(1.0, SR_TAB_EMIN + (i >> SR_TAB_BITS));
+    const double h = base / (1 << SR_TAB_BITS), u0 = base + h * (i & ((1 << SR_TAB_BITS) - 1));
+    const double sa = sqrt(alpha), c = 2.0 * sa / sqrt(PI_D);
+    double tau[4], ff[4], fe[4];
+    for (int k = 0; k < 4; ++k) {
+        tau[k] = 0.5 * (1.0 - cos((2 * k + 1) * PI_D / 8.0));      // Chebyshev nodes of [0, 1]
+        const double u = u0 + h * tau[k], r = sqrt(u), ex = erfcx(sa * r) / r;
+        fe[k] = ex;
+        ff[k] = (ex + c) / u;
+    }
+    for (int which = 0; which < 2; ++which) {
+        double* f = which ? fe : ff;
+        // Newton divided differences
+        double d[4] = {f[0], f[1], f[2], f[3]};
+        for (int lev = 1; lev < 4; ++lev)
+            for (int k = 3; k >= lev; --k) d[k] = (d[k] - d[k - 1]) / (tau[k] - tau[k - lev]);
+        // Newton form d0 + d1 (t - t0) + d2 (t - t0)(t - t1) + d3 (t - t0)(t - t1)(t - t2), expanded to monomials in tau
+        const double t0 = tau[0], t1 = tau[1], t2 = tau[2];
+        const double b0 = d[0] - d[1] * t0 + d[2] * t0 * t1 - d[3] * t0 * t1 * t2;
+        const double b1 = d[1] - d[2] * (t0 + t1) + d[3] * (t0 * t1 + t0 * t2 + t1 * t2);
+        const double b2 = d[2] - d[3] * (t0 + t1 + t2);
+        const double b3 = d[3];
+        const float4 o = make_float4((float)b0, (float)(b1 / h), (float)(b2 / (h * h)), (float)(b3 / (h * h * h)));
+        if (which) te[i] = o; else tf[i] = o;
+    }
+}
+
+// dynamic shared memory of the pair kernel: the table(s), when that variant runs (rbe_set_pair_table)
+__host__ __device__ constexpr size_t sr_pair_smem_bytes(int ntab, bool table, bool energy) {
+    return table ? (size_t)ntab * sizeof(float4) * (energy ? 2 : 1) : 0;
+}
+
 #ifndef RBE_SR_PAIR_WARPS
 #define RBE_SR_PAIR_WARPS 4
 #endif
@@ -87,7 +143,8 @@ __constant__ int8_t SR_HALF_STENCIL[14][3] = {
     {0, 0, 0},  {1, 0, 0},  {-1, 1, 0}, {0, 1, 0},  {1, 1, 0},  {-1, -1, 1}, {0, -1, 1},
     {1, -1, 1}, {-1, 0, 1}, {0, 0, 1},  {1, 0, 1},  {-1, 1, 1}, {0, 1, 1},   {1, 1, 1}};
 
-template <bool ENERGY>
+// TABLE: pair terms from the table (the paper's method); else erfc by the polynomial (sr_erfc_from_exp)
+template <bool ENERGY, bool TABLE>
 __global__ void __launch_bounds__(32 * SR_PAIR_WARPS, RBE_SR_PAIR_CTAS) sr_pair_kernel(const SrPairParams p) {
     __shared__ float4 vpos[SR_PAIR_WARPS][32];   // the visiting group: positions relative to THIS cell's centre, charge
     __shared__ float4 vacc[SR_PAIR_WARPS][32];   // ... and what this warp adds to its atoms
@@ -99,6 +156,15 @@ __global__ void __launch_bounds__(32 * SR_PAIR_WARPS, RBE_SR_PAIR_CTAS) sr_pair_
     const int ng_own = (int)((n_own + 31) >> 5);
     const float two_sa_over_sqrtpi = 1.1283791670955126f * p.sqrt_alpha;
     const float FAR = 1.0e18f;   // position of an empty lane: its pairs always fail the cutoff test (and FAR - FAR = 0 is skipped)
+    extern __shared__ __align__(16) unsigned char sr_dyn_smem[];          // the pair-term table(s), one copy per CTA
+    const float4* tab_f = reinterpret_cast<const float4*>(sr_dyn_smem);
+    const float4* tab_e = tab_f + p.ntab;
+    if (TABLE) {
+        float4* dst = reinterpret_cast<float4*>(sr_dyn_smem);
+        for (int i = threadIdx.x; i < p.ntab; i += 32 * SR_PAIR_WARPS) dst[i] = p.tab_f[i];
+        if (ENERGY) for (int i = threadIdx.x; i < p.ntab; i += 32 * SR_PAIR_WARPS) dst[p.ntab + i] = p.tab_e[i];
+        __syncthreads();
+    }
 
     for (int g = w; g < ng_own; g += SR_PAIR_WARPS) {
         const uint32_t ei = 32u * g + lane;
@@ -144,12 +210,26 @@ __global__ void __launch_bounds__(32 * SR_PAIR_WARPS, RBE_SR_PAIR_CTAS) sr_pair_
                     const float dx = o.x - me.x, dy = o.y - me.y, dz = o.z - me.z;
                     const float r2 = fmaf(dx, dx, fmaf(dy, dy, dz * dz));
                     if (r2 < p.rs2 && r2 > 0.f) {
-                        const float inv_r = sr_rsqrt(r2);
-                        const float x = p.sqrt_alpha * (r2 * inv_r);
-                        const float E = sr_ex2(-1.4426950408889634f * x * x);
-                        const float ec = sr_erfc_from_exp(x, E);
-                        const float s = fmaf(ec, inv_r, two_sa_over_sqrtpi * E) * inv_r * inv_r;   // g / r
-                        const float u = ec * inv_r;
+                        float s, u = 0.f;                            // g / r of Eq. (2.10), erfc / r of Eq. (2.8)
+                        if (TABLE && r2 >= p.tab_umin) {
+                            const uint32_t bits = __float_as_uint(r2);
+                            const int idx = (int)(bits >> (23 - SR_TAB_BITS)) - ((127 + SR_TAB_EMIN) << SR_TAB_BITS);
+                            const float dl = r2 - __uint_as_float(bits & ~((1u << (23 - SR_TAB_BITS)) - 1u));
+                            const float E = sr_ex2(p.nalpha_log2e * r2);
+                            const float4 cf = tab_f[idx];
+                            s = fmaf(fmaf(fmaf(cf.w, dl, cf.z), dl, cf.y), dl, cf.x) * E;
+                            if (ENERGY) {
+                                const float4 ce = tab_e[idx];
+                                u = fmaf(fmaf(fmaf(ce.w, dl, ce.z), dl, ce.y), dl, ce.x) * E;
+                            }
+                        } else {                                     // polynomial erfc; with TABLE: the closest pairs ("below r_0")
+                            const float inv_r = sr_rsqrt(r2);
+                            const float x = p.sqrt_alpha * (r2 * inv_r);
+                            const float E = sr_ex2(-1.4426950408889634f * x * x);
+                            const float ec = sr_erfc_from_exp(x, E);
+                            s = fmaf(ec, inv_r, two_sa_over_sqrtpi * E) * inv_r * inv_r;
+                            u = ec * inv_r;
+                        }
                         const float sj = o.w * s;
                         fx = fmaf(sj, dx, fx); fy = fmaf(sj, dy, fy); fz = fmaf(sj, dz, fz);
                         if (ENERGY) en = fmaf(o.w, u, en);

@@ -29,7 +29,7 @@ def _declared_symbols():
 def test_every_declared_symbol_is_exported(lib):
     names = _declared_symbols()
     assert {"rbe_create", "rbe_set_kvectors", "rbe_structure_factor", "rbe_forces",
-            "rbe_kspace_energy", "rbe_destroy", "rbe_step_host", "rbe_set_rho", "rbe_set_pairing",
+            "rbe_kspace_energy", "rbe_destroy", "rbe_step_host", "rbe_set_rho", "rbe_set_pairing", "rbe_set_pair_table",
             "rbe_host_alloc", "rbe_host_free"} <= set(names)
     for n in names:
         assert hasattr(lib, n), n

@@ -12,9 +12,10 @@ pytestmark = pytest.mark.gpu
 F_TOL = 2e-5
 
 
-def run(atoms, L, alpha, rs, accumulate=None, with_energy=True):
+def run(atoms, L, alpha, rs, accumulate=None, with_energy=True, table=False):
     N = atoms.shape[0]
     ctx = rbe.Rbe(N, L, alpha, 4, allocate=False)
+    ctx.rbe_set_pair_table(table)
     x = torch.from_numpy(atoms).cuda()
     F = torch.full((N, 4), float("nan"), dtype=torch.float32, device="cuda") if accumulate is None else accumulate.clone()
     ctx.rbe_short_range(x, rs, F, accumulate=accumulate is not None, with_energy=with_energy)
@@ -22,8 +23,8 @@ def run(atoms, L, alpha, rs, accumulate=None, with_energy=True):
     return ctx, x, F
 
 
-def check(atoms, L, alpha, rs, sel=None):
-    ctx, x, F = run(atoms, L, alpha, rs)
+def check(atoms, L, alpha, rs, sel=None, table=False):
+    ctx, x, F = run(atoms, L, alpha, rs, table=table)
     Fg = F.cpu().numpy().astype(np.float64)
     assert np.isfinite(Fg).all()
     F_o, e_o = oracle.short_range(atoms, L, alpha, rs, sel=sel)
@@ -139,3 +140,20 @@ def test_total_coulomb_force_is_kspace_plus_real_space():
     _, Fs, Fl = oracle.ewald_full(atoms[:, :3].astype(np.float64), atoms[:, 3].astype(np.float64), L, alpha, nreal=1, mmax=mmax)
     tot = Fs + Fl
     assert np.linalg.norm(F.cpu().numpy()[:, :3] - tot) / np.linalg.norm(tot) <= 5e-5
+
+
+@pytest.mark.parametrize("name,rs,alpha", [("water_3k", 10.0, None), ("ions_20000", 12.5, None), ("ions_20000", 6.0, 0.35),
+                                           ("ions_20000", 11.3, 0.02)])
+def test_pair_table_variant(name, rs, alpha):
+    """rbe_set_pair_table(1), the paper's tabulated pair term: same tolerance as the polynomial, for several
+    alpha r_s^2 (0.7 ... 12.6) and an r_s^2 just below a power of two (11.3^2 = 127.7: the last interval of the table);
+    the random ions include pairs closer than the table's first interval (the analytic branch)."""
+    cfg = inputs.CONFIGS[name] if name in inputs.CONFIGS else inputs.ions_config(20_000)
+    atoms = inputs.make_atoms(cfg)
+    a = cfg.alpha if alpha is None else alpha
+    F_t, _ = check(atoms, cfg.L, a, rs, table=True)
+    _, _, F_p = run(atoms, cfg.L, a, rs)
+    d = (F_t[:, :3] - F_p[:, :3]).double().norm() / F_p[:, :3].double().norm()
+    assert d.item() <= 1e-5                                               # the two variants against each other
+    _, _, F_t2 = run(atoms, cfg.L, a, rs, table=True)
+    assert torch.equal(F_t, F_t2)                                         # bitwise reproducible as well
