@@ -1035,30 +1035,39 @@ rbe_status step_host_impl(rbe_ctx* c, const float* h_in, const int32_t* h_m, con
         unpack(0, c->N);
         if (c->N > 0) RBE_CUDA(c, copy_out(0, c->N, st));
     } else {
-        RBE_CUDA(c, cudaEventRecord(c->ev_start, st));          // the copies start after the caller's earlier work
-        RBE_CUDA(c, cudaStreamWaitEvent(c->s_h2d, c->ev_start, 0));
-        RBE_CUDA(c, cudaStreamWaitEvent(c->s_d2h, c->ev_start, 0));
-        for (int64_t i = 0; i < nchunk; ++i) {
-            const int64_t lo = in_lo[i], n = in_lo[i + 1] - lo;
-            RBE_CUDA(c, copy_in(lo, n, c->s_h2d));
-            RBE_CUDA(c, cudaEventRecord(c->ev_in[i], c->s_h2d));
-            RBE_CUDA(c, cudaStreamWaitEvent(st, c->ev_in[i], 0));
-            pack(lo, n);
-            s = launch_sf(c, d_x + lo, n, i > 0, i == nchunk - 1, nullptr, st);
-            if (s != RBE_OK) return s;
+        auto pipeline = [&]() -> rbe_status {
+            RBE_CUDA(c, cudaEventRecord(c->ev_start, st));          // the copies start after the caller's earlier work
+            RBE_CUDA(c, cudaStreamWaitEvent(c->s_h2d, c->ev_start, 0));
+            RBE_CUDA(c, cudaStreamWaitEvent(c->s_d2h, c->ev_start, 0));
+            for (int64_t i = 0; i < nchunk; ++i) {
+                const int64_t lo = in_lo[i], n = in_lo[i + 1] - lo;
+                RBE_CUDA(c, copy_in(lo, n, c->s_h2d));
+                RBE_CUDA(c, cudaEventRecord(c->ev_in[i], c->s_h2d));
+                RBE_CUDA(c, cudaStreamWaitEvent(st, c->ev_in[i], 0));
+                pack(lo, n);
+                s = launch_sf(c, d_x + lo, n, i > 0, i == nchunk - 1, nullptr, st);
+                if (s != RBE_OK) return s;
+            }
+            c->have_rho = true;
+            for (int64_t i = 0; i < nchunk; ++i) {
+                const int64_t lo = out_lo[i], n = out_lo[i + 1] - lo;
+                s = launch_f(c, d_x + lo, d_f + lo, n, with_energy, st);
+                if (s != RBE_OK) return s;
+                unpack(lo, n);
+                RBE_CUDA(c, cudaEventRecord(c->ev_f[i], st));
+                RBE_CUDA(c, cudaStreamWaitEvent(c->s_d2h, c->ev_f[i], 0));
+                RBE_CUDA(c, copy_out(lo, n, c->s_d2h));
+            }
+            RBE_CUDA(c, cudaEventRecord(c->ev_done, c->s_d2h));
+            RBE_CUDA(c, cudaStreamWaitEvent(st, c->ev_done, 0));
+            return RBE_OK;
+        };
+        s = pipeline();
+        if (s != RBE_OK) {      // never return with the library's copy streams still running into the caller's buffers
+            cudaStreamSynchronize(c->s_h2d);
+            cudaStreamSynchronize(c->s_d2h);
+            return s;
         }
-        c->have_rho = true;
-        for (int64_t i = 0; i < nchunk; ++i) {
-            const int64_t lo = out_lo[i], n = out_lo[i + 1] - lo;
-            s = launch_f(c, d_x + lo, d_f + lo, n, with_energy, st);
-            if (s != RBE_OK) return s;
-            unpack(lo, n);
-            RBE_CUDA(c, cudaEventRecord(c->ev_f[i], st));
-            RBE_CUDA(c, cudaStreamWaitEvent(c->s_d2h, c->ev_f[i], 0));
-            RBE_CUDA(c, copy_out(lo, n, c->s_d2h));
-        }
-        RBE_CUDA(c, cudaEventRecord(c->ev_done, c->s_d2h));
-        RBE_CUDA(c, cudaStreamWaitEvent(st, c->ev_done, 0));
     }
     if (h_U) return rbe_kspace_energy(c, h_U, stream);
     RBE_CUDA(c, cudaStreamSynchronize(st));

@@ -374,18 +374,34 @@ struct SfCtl {
 // FIRST: the tile every warp stages at once when the kernel starts -- the counts meet at a __syncthreads
 // (called by ALL threads of the CTA); otherwise through the per-warp flags (a warp stages tile t + 1 in the
 // middle of its loop over tile t and waits only for warps whose turn came earlier).
-template <bool FIRST>
-__device__ __forceinline__ void sf_stage(const SfArgs& p, int64_t a0, int64_t hi, int warp, int lane, int nwarps, uint4* A,
-                                         SfCtl& ctl, uint32_t* tot, uint32_t seq) {
-    const uint32_t lt_mask = (1u << lane) - 1u;
-    float4 a[SF_WPT];
-    SfWindow cw[SF_WPT];
-    uint32_t mine = 0;    // this warp's pair | single << 16 counts
+// This warp's SF_WPT windows of one tile, lane = atom: atoms [a0, a0 + 32 * SF_WPT) clipped to `hi`.
+__device__ __forceinline__ void sf_load(const SfArgs& p, int64_t a0, int64_t hi, int lane, float4 (&a)[SF_WPT]) {
 #pragma unroll
     for (int j = 0; j < SF_WPT; ++j) {
         const int64_t i = a0 + j * 32 + lane;
         a[j] = i < hi ? __ldg(&p.xyzq[i]) : make_float4(0.f, 0.f, 0.f, 0.f);
     }
+}
+// The atom range [lo, hi) of CTA bx of gx, aligned to 32-atom windows.
+__device__ __forceinline__ void sf_range(const SfArgs& p, int bx, int gx, int64_t& lo, int64_t& hi) {
+    const int64_t units = (p.N + 31) >> 5;
+    lo = (units * bx / gx) << 5;
+    hi = (units * (bx + 1) / gx) << 5;
+    if (hi > p.N) hi = p.N;
+}
+// The loads of tile 0, for a kernel to issue as its very first instructions (their latency then hides behind its prologue).
+__device__ __forceinline__ void sf_load_first(const SfArgs& p, int bx, int gx, float4 (&a)[SF_WPT]) {
+    int64_t lo, hi;
+    sf_range(p, bx, gx, lo, hi);
+    sf_load(p, lo + (int64_t)(threadIdx.x >> 5) * (SF_WPT * 32), hi, threadIdx.x & 31, a);
+}
+
+template <bool FIRST>
+__device__ __forceinline__ void sf_stage(const SfArgs& p, const float4 (&a)[SF_WPT], int64_t a0, int64_t hi, int warp, int lane, int nwarps,
+                                         uint4* A, SfCtl& ctl, uint32_t* tot, uint32_t seq) {
+    const uint32_t lt_mask = (1u << lane) - 1u;
+    SfWindow cw[SF_WPT];
+    uint32_t mine = 0;    // this warp's pair | single << 16 counts
 #pragma unroll
     for (int j = 0; j < SF_WPT; ++j) {
         cw[j] = sf_classify(__float_as_uint(a[j].w), a0 + j * 32 + lane < hi, p.pairing, lane);
@@ -452,20 +468,18 @@ __host__ __device__ constexpr size_t sf_smem_bytes(int threads) {
 // The accumulation over this CTA's atoms.  On return the fp64 accumulators in shared memory hold every
 // thread's sums (call sf_write_row next).  bx / gx: this CTA's index among the CTAs that share the atoms.
 template <bool DEEP>
-__device__ __forceinline__ void sf_accumulate(const SfArgs& p, const int (&mx)[SF_KPT], const int (&my)[SF_KPT],
+__device__ __forceinline__ void sf_accumulate(const SfArgs& p, const float4 (&first)[SF_WPT], const int (&mx)[SF_KPT], const int (&my)[SF_KPT],
                                               const int (&mz)[SF_KPT], unsigned char* smem_raw, SfCtl& ctl, int bx, int gx) {
     const int tid = threadIdx.x, T = blockDim.x, lane = tid & 31, warp = tid >> 5, nwarps = T >> 5;
     uint4* arena = reinterpret_cast<uint4*>(smem_raw);                           // [2][SF_TILE_MAX] records
     double2* acc_all = reinterpret_cast<double2*>(arena + 2 * SF_TILE_MAX);      // [SF_KPT][T] fp64 accumulators
     // this CTA's atom range, aligned to 32-atom windows, in tiles of nwarps * SF_WPT windows
-    const int64_t units = (p.N + 31) >> 5;
-    const int64_t lo = (units * bx / gx) << 5;
-    int64_t hi = (units * (bx + 1) / gx) << 5;
-    if (hi > p.N) hi = p.N;
+    int64_t lo, hi;
+    sf_range(p, bx, gx, lo, hi);
     const int tile_atoms = nwarps * SF_WPT * 32;
     const int ntiles = hi > lo ? (int)((hi - lo + tile_atoms - 1) / tile_atoms) : 0;
-    // tile 0 first: its loads are the longest latency of the prologue (every thread calls: it has a barrier inside)
-    sf_stage<true>(p, lo + (int64_t)warp * (SF_WPT * 32), hi, warp, lane, nwarps, arena, ctl, &ctl.tot[0], 1u);
+    // tile 0 first, from the atoms the caller loaded when the kernel started (every thread calls: it has a barrier inside)
+    sf_stage<true>(p, first, lo + (int64_t)warp * (SF_WPT * 32), hi, warp, lane, nwarps, arena, ctl, &ctl.tot[0], 1u);
 
     const bool active = tid < p.gs * p.ng;
     const int g = active ? tid / p.gs : (1 << 28);  // inactive threads: cursor past every list -> empty loops
@@ -511,9 +525,12 @@ __device__ __forceinline__ void sf_accumulate(const SfArgs& p, const int (&mx)[S
                 }
                 if (DEEP) { depth += 2; if (depth >= SF_DEPTH) { sf_flush(acc, T, c, s); depth = 0; } }
             }
-            if (part == 0 && more)
-                sf_stage<false>(p, lo + (int64_t)(t + 1) * tile_atoms + (int64_t)warp * (SF_WPT * 32), hi, warp, lane, nwarps,
-                                arena + (buf ^ 1) * SF_TILE_MAX, ctl, &ctl.tot[buf ^ 1], (uint32_t)t + 2u);
+            if (part == 0 && more) {
+                float4 nxt[SF_WPT];
+                const int64_t a0 = lo + (int64_t)(t + 1) * tile_atoms + (int64_t)warp * (SF_WPT * 32);
+                sf_load(p, a0, hi, lane, nxt);
+                sf_stage<false>(p, nxt, a0, hi, warp, lane, nwarps, arena + (buf ^ 1) * SF_TILE_MAX, ctl, &ctl.tot[buf ^ 1], (uint32_t)t + 2u);
+            }
         }
         ep -= np;
 #pragma unroll 1
@@ -576,6 +593,8 @@ __global__ void __launch_bounds__(SF_TMAX, 1) sf_kernel(const SfParams p) {
     __shared__ SfCtl ctl;
     __shared__ uint32_t s_last;
     const int tid = threadIdx.x, T = blockDim.x;
+    float4 tile0[SF_WPT];
+    sf_load_first(p.a, blockIdx.x, gridDim.x, tile0);
     const bool active = tid < p.a.gs * p.a.ng;
     const int kbase = (blockIdx.y * p.a.gs + (active ? tid % p.a.gs : 0)) * SF_KPT;
     int mx[SF_KPT], my[SF_KPT], mz[SF_KPT];
@@ -585,7 +604,7 @@ __global__ void __launch_bounds__(SF_TMAX, 1) sf_kernel(const SfParams p) {
         if (active && kbase + r < p.a.P) m = __ldg(&p.kvec[kbase + r]);
         mx[r] = m.x; my[r] = m.y; mz[r] = m.z;
     }
-    sf_accumulate<DEEP>(p.a, mx, my, mz, smem_raw, ctl, blockIdx.x, gridDim.x);
+    sf_accumulate<DEEP>(p.a, tile0, mx, my, mz, smem_raw, ctl, blockIdx.x, gridDim.x);
 
     // let the dependent (force) kernel start launching; it waits for this grid's completion
     grid_launch_dependents();
@@ -802,17 +821,24 @@ __device__ __forceinline__ unsigned long long ld_acquire_gpu_u64(const unsigned 
     return v;
 }
 
-// All threads of all CTAs of a cooperative launch.  Release: barrier + fence by thread 0 before its
-// arrival; acquire: its polling load + fence before the barrier that lets the CTA continue.
-__device__ __forceinline__ void grid_barrier(unsigned long long* ctr) {
+// Grid barrier of a cooperative launch: a 64-bit arrival counter in the workspace that only ever grows (a launch
+// adds 2 * gridDim.x; zeroed by rbe_set_workspace, one grid size per context).  Thread 0 of every CTA reads it when
+// the kernel starts -- long before anybody can arrive at the first barrier, so off the critical path -- and rounds
+// down to a multiple of gridDim.x: the count before this launch, whatever early arrivals it saw.  The barriers then
+// wait for base + gridDim.x and base + 2 gridDim.x.  Arriving is a one-way red.release (no value comes back), so a
+// barrier costs one fence, one reduction on its way and the polling load -- not an atomic round trip plus the poll.
+__device__ __forceinline__ unsigned long long grid_barrier_base(const unsigned long long* ctr) {
+    unsigned long long v;
+    asm volatile("ld.relaxed.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(ctr) : "memory");
+    return v - v % gridDim.x;
+}
+// All threads of all CTAs.  Release: barrier + red.release by thread 0; acquire: its polling load before the barrier
+// that lets the CTA continue.
+__device__ __forceinline__ void grid_barrier(unsigned long long* ctr, unsigned long long target) {
     __syncthreads();
     if (threadIdx.x == 0) {
-        __threadfence();
-        const unsigned long long n = gridDim.x;
-        const unsigned long long old = atomicAdd(ctr, 1ull);
-        const unsigned long long target = (old / n + 1ull) * n;
+        asm volatile("red.release.gpu.global.add.u64 [%0], %1;" ::"l"(ctr), "l"(1ull) : "memory");
         while (ld_acquire_gpu_u64(ctr) < target) { }
-        __threadfence();
     }
     __syncthreads();
 }
@@ -828,6 +854,10 @@ __global__ void __launch_bounds__(SF_TMAX, 1) step_kernel(const __grid_constant_
     __shared__ SfCtl ctl;
     const int tid = threadIdx.x, T = blockDim.x, lane = tid & 31, warp = tid >> 5, nwarps = T >> 5;
     const int bx = blockIdx.x, G = gridDim.x, P = p.sf.P;
+    float4 first[SF_WPT];
+    sf_load_first(p.sf, bx, G, first);                  // the longest latency of the prologue: issued before anything else
+    unsigned long long bar_base = 0ull;
+    if (tid == 0) bar_base = grid_barrier_base(p.bar);
 
     // ---- 1. SF phase                                                                   // @stamp
     // wavevectors from the kernel parameters: the constant bank serves one address per request, so every warp
@@ -855,10 +885,10 @@ __global__ void __launch_bounds__(SF_TMAX, 1) step_kernel(const __grid_constant_
         }
         if (p.kparam && bx == 0)   // keep the workspace copy current for the energy / virial / read-back calls
             for (int k = tid; k < P; k += T) const_cast<int4*>(p.kvec)[k] = step_kvec(p, s_km, k);
-        sf_accumulate<DEEP>(p.sf, mx, my, mz, smem_raw, ctl, bx, G);                    // @stamp
+        sf_accumulate<DEEP>(p.sf, first, mx, my, mz, smem_raw, ctl, bx, G);                    // @stamp
         sf_write_row(p.sf, smem_raw, bx, 0);                                              // @stamp
     }
-    grid_barrier(p.bar);                                                                  // @stamp
+    grid_barrier(p.bar, bar_base + (unsigned long long)G);                                // @stamp
 
     // ---- 3. distributed fixed-order reduction + the per-k force records
     {
@@ -886,7 +916,7 @@ __global__ void __launch_bounds__(SF_TMAX, 1) step_kernel(const __grid_constant_
         }
     }
                                                                                           // @stamp
-    grid_barrier(p.bar);                                                                  // @stamp
+    grid_barrier(p.bar, bar_base + 2ull * (unsigned long long)G);                         // @stamp
 
     // ---- 5. F phase: this CTA's warps take the same atom range the CTA had in the SF phase
     if (p.f.force == nullptr) return;
