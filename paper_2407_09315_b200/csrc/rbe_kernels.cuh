@@ -33,6 +33,7 @@ constexpr int F_THREADS = 512;   // threads per CTA (force kernel)
 constexpr int F_CTAS_PER_SM = 2;
 constexpr int F_RMAX = 4;        // max atoms per thread per pass (force kernel)
 constexpr int F_KCHUNK = 2048;   // wavevectors staged in shared memory at a time (force kernel)
+constexpr int F_KSPLIT = 8;      // step kernel, small systems: most slices a unit's wavevectors are cut into (one slice per warp)
 constexpr int SF_RED_GROUP = 16; // CTAs per group in the two-level reduction of the per-CTA rows (two-launch path)
 
 constexpr double TWO32 = 4294967296.0;
@@ -672,8 +673,11 @@ __device__ __forceinline__ float4 f_fetch(const FArgs& p, int64_t unit, int lane
 // One pass: R units (R atoms per thread) against the nk wavevector records in shared memory.
 // (Tried: starting the record loop at a different k in every warp of a sub-partition, so that the warps do not
 // march in lock-step.  A stand-alone copy of this loop gained 6 % from it; inside the kernels it lost 1 %.)
+// s_out != nullptr (R = 1 only): the q-scaled sums go to s_out[lane] in shared memory instead of the force array
+// (the k-split force phase of small systems adds such partial sums in a fixed order).
 template <int R, bool ENERGY, bool ACCUM>
-__device__ __forceinline__ void f_pass(const FArgs& p, const int4* s_ka, const float4* s_kb, int nk, int64_t unit0, int lane) {
+__device__ __forceinline__ void f_pass(const FArgs& p, const int4* s_ka, const float4* s_kb, int nk, int64_t unit0, int lane,
+                                       float4* s_out = nullptr) {
     uint32_t sx[R], sy[R], sz[R];
     float q[R], fx[R], fy[R], fz[R], en[R];
     const float K = phase_scale();
@@ -686,7 +690,9 @@ __device__ __forceinline__ void f_pass(const FArgs& p, const int4* s_ka, const f
         q[r] = a.w;
         fx[r] = fy[r] = fz[r] = en[r] = 0.f;
     }
-#pragma unroll 2
+    // 8 (atom, k) pairs in flight whatever R is: a thread with one atom is otherwise bound by the latency of its
+    // IMAD -> I2FP -> FMUL -> MUFU -> FFMA chain (small systems: 45 cycles per wavevector instead of ~10)
+#pragma unroll(R >= 3 ? 2 : R == 2 ? 4 : 8)
     for (int k = 0; k < nk; ++k) {
         const int4 a = s_ka[k];
         const float4 b = s_kb[k];
@@ -704,7 +710,9 @@ __device__ __forceinline__ void f_pass(const FArgs& p, const int4* s_ka, const f
 #pragma unroll
     for (int r = 0; r < R; ++r) {
         const int64_t i = (unit0 + r) * 32 + lane;
-        if (i < p.N) {
+        if (R == 1 && s_out != nullptr) {
+            s_out[lane] = make_float4(q[r] * fx[r], q[r] * fy[r], q[r] * fz[r], ENERGY ? q[r] * en[r] : 0.f);
+        } else if (i < p.N) {
             float4 o = make_float4(q[r] * fx[r], q[r] * fy[r], q[r] * fz[r], ENERGY ? q[r] * en[r] : 0.f);
             if (ACCUM) {
                 const float4 prev = p.force[i];
@@ -925,9 +933,39 @@ __global__ void __launch_bounds__(SF_TMAX, 1) step_kernel(const __grid_constant_
     for (int t = tid; t < P; t += T) { s_ka[t] = __ldcg(&p.ka[t]); s_kb[t] = __ldcg(&p.kb[t]); }
     __syncthreads();
     const int64_t units = (p.f.N + 31) / 32;
+    const int64_t c0 = units * bx / G, c1 = units * (bx + 1) / G;              // the CTA's units (as in the SF phase)
+    const int nu = (int)(c1 - c0);
+    uint32_t dyn_smem;
+    asm("mov.u32 %0, %%dynamic_smem_size;" : "=r"(dyn_smem));
+    int ksplit = nu > 0 ? nwarps / nu : 0;                 // slices per unit: as many (unit, slice) items as warps, at most F_KSPLIT
+    if (ksplit > F_KSPLIT) ksplit = F_KSPLIT;
+    if (ksplit >= 2 && P >= 8 * ksplit &&
+        (size_t)P * (sizeof(int4) + sizeof(float4)) + (size_t)nu * ksplit * 32 * sizeof(float4) <= (size_t)dyn_smem) {
+        // Small system: at most half as many units as warps.  Every unit's wavevectors are cut into ksplit slices, the
+        // (unit, slice) items go one to a warp (one atom per thread, 8 wavevectors in flight), and the slices of a unit are
+        // added in order.
+        float4* parts = reinterpret_cast<float4*>(smem_raw + (size_t)P * (sizeof(int4) + sizeof(float4)));   // [nu * ksplit][32]
+        if (warp < nu * ksplit) {
+            const int unit = warp / ksplit, part = warp % ksplit;
+            const int k0 = P * part / ksplit, k1 = P * (part + 1) / ksplit;
+            f_pass<1, ENERGY, false>(p.f, s_ka + k0, s_kb + k0, k1 - k0, c0 + unit, lane, parts + (size_t)warp * 32);
+        }
+        __syncthreads();
+        for (int idx = tid; idx < nu * 32; idx += T) {
+            const int unit = idx >> 5, l = idx & 31;
+            float4 a = parts[(size_t)(unit * ksplit) * 32 + l];
+            for (int q = 1; q < ksplit; ++q) {
+                const float4 v = parts[(size_t)(unit * ksplit + q) * 32 + l];
+                a.x += v.x; a.y += v.y; a.z += v.z; a.w += v.w;
+            }
+            const int64_t i = (c0 + unit) * 32 + l;
+            if (i < p.f.N) p.f.force[i] = a;
+        }
+        return;                                                                       // @stamp @stamp_sync
+    }
     int64_t u0;
     int n;
-    f_warp_share(units * bx / G, units * (bx + 1) / G, warp, nwarps, u0, n);   // the CTA's units (as in the SF phase)
+    f_warp_share(c0, c1, warp, nwarps, u0, n);
     f_run<ENERGY, false>(p.f, s_ka, s_kb, P, u0, n, lane);                            // @stamp @stamp_sync
 }
 
