@@ -252,7 +252,7 @@ rbe_status rbe_step(rbe_ctx* ctx, const int32_t* h_m, const double* h_w, const v
  *   accumulate  != 0: add to what d_force holds (e.g. the k-space force of rbe_forces)
  *   d_ws        caller-owned device scratch of rbe_short_range_bytes(ctx, rs) bytes (~76 B per atom
  *               + 204 B per cell), 256-byte aligned; its contents are rebuilt by every call
- * rbe_short_range_bytes returns 0 for an invalid rs.  Enqueues seven kernels and one memset on `stream`.
+ * rbe_short_range_bytes returns 0 for an invalid rs.  Enqueues seven kernels (eight with rbe_set_pair_table) and two memsets on `stream`.
  * Errors: RBE_ERR_INVALID_ARG, RBE_ERR_WORKSPACE, RBE_ERR_NO_DEVICE, RBE_ERR_CUDA. */
 size_t     rbe_short_range_bytes(const rbe_ctx* ctx, double rs);
 rbe_status rbe_short_range(rbe_ctx* ctx, const void* d_xyzq, double rs, void* d_force, int32_t accumulate,
