@@ -89,7 +89,10 @@ double rbe_normaliser_S(const rbe_ctx* ctx);
 size_t rbe_workspace_bytes(const rbe_ctx* ctx);
 
 /* Hand the context a device buffer of at least rbe_workspace_bytes bytes, 256-byte aligned,
- * allocated on the current CUDA device.  Caller keeps ownership and must keep it alive.
+ * allocated on the current CUDA device.  Caller keeps ownership and must keep it alive.  The buffer belongs to
+ * THIS context alone for as long as it is set (it holds state that survives from launch to launch: the k-set,
+ * rho, the step counter of the device sampler, the arrival counter of rbe_step's grid barrier, which the call
+ * zeroes and which must stay a multiple of the context's grid size): never share it between contexts.
  * Errors: RBE_ERR_WORKSPACE, RBE_ERR_NO_DEVICE, RBE_ERR_CUDA. */
 rbe_status rbe_set_workspace(rbe_ctx* ctx, void* d_ws, size_t bytes);
 
