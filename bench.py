@@ -339,6 +339,16 @@ def main():
     sync()
     ms_total = e0.elapsed_time(e1)
 
+    # ---- region A2: the same K steps with CUDA events around every step, for the median and the minimum;
+    # the headline stays region A's mean, which carries no per-step event
+    evs_a = [[torch.cuda.Event(enable_timing=True) for _ in range(2)] for _ in range(args.steps)]
+    for i in range(args.steps):
+        evs_a[i][0].record()
+        step(args.warmup + i)
+        evs_a[i][1].record()
+    sync()
+    t_step = sorted(e[0].elapsed_time(e[1]) for e in evs_a)
+
     # ---- timed region B: the same K steps in the two-launch form with CUDA events around each call, for the
     # per-kernel durations of sf_kernel and f_kernel
     evs = [[torch.cuda.Event(enable_timing=True) for _ in range(3)] for _ in range(args.steps)]
@@ -547,8 +557,11 @@ def main():
                    "step": "rbe_step: one cooperative launch (step_kernel)" if one_launch else
                            "rbe_set_kvectors + rbe_structure_factor + rbe_forces: two launches",
                    "launch": info, "with_energy": bool(args.with_energy)},
-        "kernels_ms": {"step_call": ms_step, "two_launch_step": ms_two, "structure_factor_call": ms_sf, "forces_call": ms_f,
-                       "note": "step_call = region A (rbe_step); the rest = region B, the two-launch form with CUDA events around "
+        "kernels_ms": {"step_call": ms_step, "step_call_median": t_step[len(t_step) // 2], "step_call_min": t_step[0],
+                       "two_launch_step": ms_two, "structure_factor_call": ms_sf, "forces_call": ms_f,
+                       "structure_factor_call_median": statistics.median(t_sf), "structure_factor_call_min": min(t_sf),
+                       "forces_call_median": statistics.median(t_f), "forces_call_min": min(t_f),
+                       "note": "step_call = region A (rbe_step; _median / _min: region A2, per-step events); the rest = region B, the two-launch form with CUDA events around "
                                "each C-ABI call: structure_factor_call = sf_kernel (incl. its in-kernel second pass), forces_call = f_kernel"},
         "peaks": {"lanes_per_sm_per_clk": {k: pipe[k] for k in ("ffma", "imad", "i2fp", "mufu")},
                   "sm_mhz_during_probe": pipe["sm_mhz"], "sm_max_mhz": peaks["sm_max_mhz"], "hbm_gbs": peaks["hbm_gbs"],
