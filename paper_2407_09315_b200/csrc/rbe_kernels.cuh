@@ -640,8 +640,10 @@ __global__ void __launch_bounds__(SF_TMAX, 1) sf_kernel(const SfParams p) {
         // fused exchange: this CTA (the last one of the grid) writes the partial rho into its slot on
         // every rank over NVLink, then releases the per-rank flags (stores, fence, flag)
         __syncthreads();
-        for (int r = 0; r < rp.xch.world; ++r)
-            for (int k = tid; k < p.a.P; k += T) rp.xch.slot[r][k] = __ldcg(&rp.rho[k]);
+        for (int idx = tid; idx < rp.xch.world * p.a.P; idx += T) {       // all (rank, k) stores in flight together
+            const int r = idx / p.a.P, k = idx - r * p.a.P;
+            rp.xch.slot[r][k] = __ldcg(&rp.rho[k]);
+        }
         __threadfence_system();
         __syncthreads();
         if (tid < rp.xch.world) st_release_sys(rp.xch.flag[tid], rp.xch.epoch);
