@@ -416,6 +416,18 @@ def main():
         sync()
         ms_sr_tab = e0.elapsed_time(e1) / k_sr
         ctx.rbe_set_pair_table(False)
+        # ... and with the second force kernel (rbe_set_pair_kernel(1): fine cells, tensor-core cutoff test, ordered pairs)
+        ctx.rbe_set_pair_kernel(1)
+        for i in range(2):
+            ctx.rbe_short_range(xs[i % n_rot], args.rs, fs[i % n_rot])
+        sync()
+        e0.record()
+        for i in range(k_sr):
+            ctx.rbe_short_range(xs[i % n_rot], args.rs, fs[i % n_rot])
+        e1.record()
+        sync()
+        ms_sr_cells = e0.elapsed_time(e1) / k_sr
+        ctx.rbe_set_pair_kernel(0)
         # the paper's own estimator of the same force: random batch list, r_c = r_s / 2, p = 30
         for i in range(2):
             ctx.rbe_rbl_forces(xs[i % n_rot], args.rs / 2, args.rs, 30, base.seed, i, fs[i % n_rot])
@@ -432,6 +444,8 @@ def main():
               "pair_rate_G_per_s": nbr * n_local / (ms_sr * 1e-3) / 1e9,
               "pair_table": {"ms_per_call": ms_sr_tab, "note": "rbe_set_pair_table(1): tabulated pair term with cubic interpolation "
                              "(P:196) instead of the degree-8 polynomial erfc; one more launch (the table is rebuilt per call)"},
+              "pair_kernel_cells": {"ms_per_call": ms_sr_cells, "note": "rbe_set_pair_kernel(1): one CTA per cell of side r_s / 2, cutoff test as a TF32 "
+                                    "mma on the tensor cores, every ordered pair evaluated by one lane, no atomics"},
               "rbl": {"ms_per_call": ms_rbl, "r_c": args.rs / 2, "p": 30,
                       "note": "rbe_rbl_forces (Eqs. 2.13-2.16): cells of side r_c, warp per atom, parity-exact batch; still slower "
                               "than the deterministic sum on B200 (instruction budget: profiles/r02_rbl_README.md)"},

@@ -106,6 +106,15 @@ rbe_status rbe_set_workspace(rbe_ctx* ctx, void* d_ws, size_t bytes);
  * Errors: RBE_ERR_INVALID_ARG. */
 rbe_status rbe_set_pairing(rbe_ctx* ctx, int32_t mode);
 
+/* Which force kernel rbe_short_range runs (default 0).  Same definition, same tolerances, both bitwise reproducible.
+ *   kind 0: cells of side >= r_s; a warp ring over 32 x 32 blocks of atoms, every unordered pair once (Newton's third
+ *           law), partial sums of different warps combined in 64-bit fixed point with integer atomics;
+ *   kind 1: cells of side >= r_s / 2 (125-cell stencil), one CTA per cell; the cutoff test runs on the tensor cores
+ *           (r^2 as a K = 8 TF32 product with a margin, the exact fp32 test repeated at evaluation), every ordered pair
+ *           is evaluated by one lane and F_i is written directly: no atomics, no fixed point, no finalise pass.
+ * rbe_short_range_bytes covers either.  Errors: RBE_ERR_INVALID_ARG. */
+rbe_status rbe_set_pair_kernel(rbe_ctx* ctx, int32_t kind);
+
 /* How rbe_short_range evaluates the pair term of Eq. (2.10) (default 0).
  *   on 0: erfc by a degree-8 polynomial fit (3.4e-7 relative error), exp and 1/r by the special-function unit;
  *   on 1: the paper's method: a table over u = r^2 with interpolation above a small radius, the

@@ -13,6 +13,7 @@
 #include "rbe_kernels.cuh"
 #include "sr_kernels.cuh"
 #include "sr_pair_kernels.cuh"
+#include "sr_cell_kernels.cuh"
 #include "rbl_kernels.cuh"
 #include "nve_kernels.cuh"
 
@@ -40,6 +41,7 @@ struct rbe_ctx {
     int sf_gs = 0, sf_ng = 0;
     int sf_pairing = 3;
     int sr_table = 0;          // rbe_set_pair_table
+    int sr_kernel = 0;         // rbe_set_pair_kernel: 0 ring kernel (cells of side r_s), 1 cell kernel (cells of side r_s / 2, tensor-core test)
     int sf_ngroups = 1;
     size_t ws_bytes = 0;
     size_t off_kvec = 0, off_w = 0, off_part = 0, off_rho = 0, off_grow = 0, off_U = 0, off_ticket = 0;
@@ -530,6 +532,13 @@ rbe_status rbe_set_pairing(rbe_ctx* c, int32_t mode) {
     return RBE_OK;
 }
 
+rbe_status rbe_set_pair_kernel(rbe_ctx* c, int32_t kind) {
+    if (!c) return RBE_ERR_INVALID_ARG;
+    if (kind != 0 && kind != 1) return fail(c, RBE_ERR_INVALID_ARG, "rbe_set_pair_kernel: kind must be 0 or 1");
+    c->sr_kernel = kind;
+    return RBE_OK;
+}
+
 rbe_status rbe_set_pair_table(rbe_ctx* c, int32_t on) {
     if (!c) return RBE_ERR_INVALID_ARG;
     if (on != 0 && on != 1) return fail(c, RBE_ERR_INVALID_ARG, "rbe_set_pair_table: on must be 0 or 1");
@@ -782,9 +791,24 @@ bool sr_layout(const rbe_ctx* c, double cell_min, int need, SrLayout& l) {
 }
 }  // namespace
 
+namespace {
+// The cell kernel's list: cells of side >= r_s / 2 (125-cell stencil, R = 2) where the box holds five of them per dimension,
+// else cells of side >= r_s (27-cell stencil, R = 1): the stencil must not meet itself around the box.
+bool sr_cell_layout(const rbe_ctx* c, double rs, SrLayout& l, int& R) {
+    if (!c || !(rs > 0.0) || !std::isfinite(rs)) return false;
+    if (sr_layout(c, 0.5 * rs, 5, l)) R = 2;
+    else if (sr_layout(c, rs, 3, l)) R = 1;
+    else return false;
+    return true;
+}
+}  // namespace
+
 size_t rbe_short_range_bytes(const rbe_ctx* c, double rs) {
-    SrLayout l;
-    return sr_layout(c, rs, 3, l) ? l.bytes : 0;       // the 27-cell stencil needs 3 distinct cells per dimension
+    SrLayout l, l2;
+    int R;
+    if (!sr_layout(c, rs, 3, l)) return 0;             // the 27-cell stencil needs 3 distinct cells per dimension
+    if (sr_cell_layout(c, rs, l2, R) && l2.bytes > l.bytes) return l2.bytes;   // enough for either kernel (rbe_set_pair_kernel)
+    return l.bytes;
 }
 
 namespace {
@@ -849,6 +873,64 @@ rbe_status sr_build_cells(rbe_ctx* c, const char* who, const void* d_xyzq, void*
 }
 }  // namespace
 
+namespace {
+// rbe_short_range with the cell kernel (rbe_set_pair_kernel(ctx, 1)): the same linked-cell build on finer cells, then ONE
+// force kernel that writes the caller's array directly.
+rbe_status short_range_cells(rbe_ctx* c, const void* d_xyzq, double rs, void* d_force, int32_t accumulate, int32_t with_energy,
+                             void* d_ws, size_t ws_bytes, cudaStream_t st) {
+    SrLayout l;
+    SrBuffers b;
+    int R = 0;
+    if (!sr_cell_layout(c, rs, l, R)) return fail(c, RBE_ERR_INVALID_ARG, "rbe_short_range: invalid r_s");
+    rbe_status s = sr_build_cells(c, "rbe_short_range", d_xyzq, d_force, d_ws, ws_bytes, st, l, b);
+    if (s != RBE_OK || c->N == 0) return s;
+    rbe::SrCellParams pp;
+    pp.sorted = b.sorted; pp.sidx = b.sidx; pp.start = b.start;
+    pp.force = static_cast<float4*>(d_force);
+    pp.nc = l.nc; pp.R = R; pp.accumulate = accumulate;
+    pp.len_unit = (float)(c->L / rbe::TWO32);
+    const double cell_len = c->L / l.nc;
+    pp.rs2 = (float)(rs * rs);
+    // margin of the tensor-core cutoff test: the own atom is rounded to TF32 (<= 2^-12 cell sides per component, i.e.
+    // |dr| <= sqrt(3) 2^-12 cell sides), plus 2e-5 |x|^2_max for the fp32 / TF32 rounding of the sums (candidates lie within
+    // R + 1/2 cell sides of the cell centre per component)
+    const double dr = std::sqrt(3.0) * cell_len / 4096.0, xmax = (R + 0.5) * cell_len;
+    const double margin = 1.5 * (2.0 * rs * dr + dr * dr) + 2e-5 * 3.0 * xmax * xmax;
+    pp.thr = (float)(rs * rs + margin);
+    pp.sqrt_alpha = (float)std::sqrt(c->alpha);
+    pp.nalpha_log2e = (float)(-c->alpha * 1.4426950408889634);
+    // the pair-term table: up to past r_s^2 + 2 margins (what can pass the test; the exact test then zeroes it)
+    const int emax = (int)std::floor(std::log2(rs * rs + 2.0 * margin)) + 1;
+    int ntab = (emax - rbe::SR_TAB_EMIN) << rbe::SR_TAB_BITS;
+    if (ntab < (1 << rbe::SR_TAB_BITS)) ntab = 1 << rbe::SR_TAB_BITS;
+    if (ntab > rbe::SR_TAB_MAX) return fail(c, RBE_ERR_INVALID_ARG, "rbe_short_range: r_s too large for the pair-term table");
+    pp.ntab = ntab;
+    pp.tab_f = b.tab; pp.tab_e = b.tab + rbe::SR_TAB_MAX;
+    pp.tab_umin = (float)std::ldexp(1.0, rbe::SR_TAB_EMIN);
+    // candidate list in shared memory: 1.5 x the mean number of candidates of a cell, in steps of 256
+    const int side = 2 * R + 1;
+    const double mean_cand = (double)c->N / (double)l.ncell * (double)(side * side * side);
+    int cap = (int)std::ceil(1.5 * mean_cand / 256.0) * 256 + 256;
+    if (cap > rbe::SR_CAP_MAX) cap = rbe::SR_CAP_MAX;
+    pp.cap = cap;
+    const bool table = c->sr_table != 0;
+    const size_t dyn = rbe::sr_cell_smem_bytes(ntab, table, with_energy != 0, cap);
+    const int dyn_max = (int)rbe::sr_cell_smem_bytes(rbe::SR_TAB_MAX, true, true, rbe::SR_CAP_MAX);
+    const unsigned grid = (unsigned)l.ncell, block = 32 * rbe::SR_W;
+    if (table) rbe::sr_table_kernel<<<(unsigned)((ntab + 127) / 128), 128, 0, st>>>(b.tab, b.tab + rbe::SR_TAB_MAX, ntab, c->alpha);
+#define RBE_SR_CELL_LAUNCH(E, T)                                                                                              \
+    do {                                                                                                                      \
+        RBE_CUDA(c, cudaFuncSetAttribute(rbe::sr_cell_kernel<E, T>, cudaFuncAttributeMaxDynamicSharedMemorySize, dyn_max));   \
+        rbe::sr_cell_kernel<E, T><<<grid, block, dyn, st>>>(pp);                                                              \
+    } while (0)
+    if (with_energy) { if (table) RBE_SR_CELL_LAUNCH(true, true); else RBE_SR_CELL_LAUNCH(true, false); }
+    else { if (table) RBE_SR_CELL_LAUNCH(false, true); else RBE_SR_CELL_LAUNCH(false, false); }
+#undef RBE_SR_CELL_LAUNCH
+    RBE_CUDA(c, cudaGetLastError());
+    return RBE_OK;
+}
+}  // namespace
+
 rbe_status rbe_short_range(rbe_ctx* c, const void* d_xyzq, double rs, void* d_force, int32_t accumulate,
                            int32_t with_energy, void* d_ws, size_t ws_bytes, void* stream) {
     if (!c) return RBE_ERR_INVALID_ARG;
@@ -857,6 +939,7 @@ rbe_status rbe_short_range(rbe_ctx* c, const void* d_xyzq, double rs, void* d_fo
     SrBuffers b;
     if (!sr_layout(c, rs, 3, l))
         return fail(c, RBE_ERR_INVALID_ARG, "rbe_short_range: need 0 < r_s <= L/3 (three cells of side >= r_s per dimension) and N < 2^32");
+    if (c->sr_kernel == 1) return short_range_cells(c, d_xyzq, rs, d_force, accumulate, with_energy, d_ws, ws_bytes, st);
     rbe_status s = sr_build_cells(c, "rbe_short_range", d_xyzq, d_force, d_ws, ws_bytes, st, l, b);
     if (s != RBE_OK || c->N == 0) return s;
     const unsigned nb = (unsigned)((c->N + 255) / 256);

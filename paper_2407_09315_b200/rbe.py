@@ -62,6 +62,8 @@ def lib():
         L.rbe_set_pairing.argtypes = [vp, i32]
         L.rbe_set_pair_table.restype = ctypes.c_int
         L.rbe_set_pair_table.argtypes = [vp, i32]
+        L.rbe_set_pair_kernel.restype = ctypes.c_int
+        L.rbe_set_pair_kernel.argtypes = [vp, i32]
         L.rbe_get_launch_info.restype = ctypes.c_int
         L.rbe_get_launch_info.argtypes = [vp, ctypes.POINTER(LaunchInfo)]
         L.rbe_set_kvectors.restype = ctypes.c_int
@@ -215,6 +217,9 @@ class Rbe:
 
     def rbe_set_pairing(self, mode: int):
         self._check(lib().rbe_set_pairing(self._h, int(mode)))
+
+    def rbe_set_pair_kernel(self, kind: int):
+        self._check(lib().rbe_set_pair_kernel(self._h, int(kind)))
 
     def rbe_set_pair_table(self, on: bool):
         self._check(lib().rbe_set_pair_table(self._h, int(bool(on))))

@@ -1,4 +1,5 @@
-"""Time the real-space partner on one GPU: rbe_short_range (polynomial and tabulated pair term) and rbe_rbl_forces.
+"""Time the real-space partner on one GPU: rbe_short_range (both force kernels, polynomial and tabulated pair term) and
+rbe_rbl_forces.
 
     python -m paper_2407_09315_b200.time_short_range [--config water_nacl_1m] [--rs 10] [--rc 5] [--p 30] [--calls 10]
 
@@ -47,6 +48,12 @@ def main():
     ctx.rbe_set_pair_table(True)
     out["short_range_table_ms"] = timed(lambda i: ctx.rbe_short_range(x, args.rs, f, with_energy=args.with_energy))
     ctx.rbe_set_pair_table(False)
+    ctx.rbe_set_pair_kernel(1)            # fine cells, tensor-core cutoff test, ordered pairs
+    out["short_range_cells_ms"] = timed(lambda i: ctx.rbe_short_range(x, args.rs, f, with_energy=args.with_energy))
+    ctx.rbe_set_pair_table(True)
+    out["short_range_cells_table_ms"] = timed(lambda i: ctx.rbe_short_range(x, args.rs, f, with_energy=args.with_energy))
+    ctx.rbe_set_pair_table(False)
+    ctx.rbe_set_pair_kernel(0)
     out["rbl_ms"] = timed(lambda i: ctx.rbe_rbl_forces(x, args.rc, args.rs, args.p, cfg.seed, i, f))
     print(json.dumps(out))
 

@@ -29,7 +29,7 @@ def _declared_symbols():
 def test_every_declared_symbol_is_exported(lib):
     names = _declared_symbols()
     assert {"rbe_create", "rbe_set_kvectors", "rbe_structure_factor", "rbe_forces",
-            "rbe_kspace_energy", "rbe_destroy", "rbe_step_host", "rbe_set_rho", "rbe_set_pairing", "rbe_set_pair_table",
+            "rbe_kspace_energy", "rbe_destroy", "rbe_step_host", "rbe_set_rho", "rbe_set_pairing", "rbe_set_pair_table", "rbe_set_pair_kernel",
             "rbe_host_alloc", "rbe_host_free"} <= set(names)
     for n in names:
         assert hasattr(lib, n), n
@@ -101,7 +101,9 @@ def test_size_queries_need_no_device(lib):
     assert lib.rbe_step_host_bytes(None, 0) == 0
     assert lib.rbe_short_range_bytes(h, ctypes.c_double(10.0)) > 76 * N
     assert lib.rbe_short_range_bytes(h, ctypes.c_double(21.0)) == 0                 # r_s > L/3
-    assert lib.rbe_rbl_bytes(h, ctypes.c_double(5.0), ctypes.c_double(10.0)) > lib.rbe_short_range_bytes(h, ctypes.c_double(10.0))
+    # rbe_short_range_bytes covers both of its force kernels: the finer list of rbe_set_pair_kernel(1) is the RBL's at r_c = r_s / 2
+    assert lib.rbe_rbl_bytes(h, ctypes.c_double(5.0), ctypes.c_double(10.0)) == lib.rbe_short_range_bytes(h, ctypes.c_double(10.0))
+    assert lib.rbe_rbl_bytes(h, ctypes.c_double(4.0), ctypes.c_double(10.0)) > lib.rbe_short_range_bytes(h, ctypes.c_double(10.0))
     assert lib.rbe_rbl_bytes(h, ctypes.c_double(10.0), ctypes.c_double(5.0)) == 0   # r_c >= r_s
     assert lib.rbe_rbl_bytes(h, ctypes.c_double(5.0), ctypes.c_double(21.0)) > 0    # 9 cells of 5.45 A fit the 60 A box
     assert lib.rbe_rbl_bytes(h, ctypes.c_double(5.0), ctypes.c_double(29.0)) == 0   # the stencil would meet itself

@@ -10,12 +10,23 @@ from paper_2407_09315_b200 import inputs, rbe
 
 pytestmark = pytest.mark.gpu
 F_TOL = 2e-5
+KIND = 0
+
+
+@pytest.fixture(autouse=True, params=[0, 1], ids=["ring", "cells"])
+def pair_kernel(request):
+    """Every test of this module runs with both force kernels (rbe_set_pair_kernel): 0 = warp ring over cells of side r_s,
+    1 = one CTA per cell of side r_s / 2 with the cutoff test on the tensor cores."""
+    global KIND
+    KIND = request.param
+    yield
 
 
 def run(atoms, L, alpha, rs, accumulate=None, with_energy=True, table=False):
     N = atoms.shape[0]
     ctx = rbe.Rbe(N, L, alpha, 4, allocate=False)
     ctx.rbe_set_pair_table(table)
+    ctx.rbe_set_pair_kernel(KIND)
     x = torch.from_numpy(atoms).cuda()
     F = torch.full((N, 4), float("nan"), dtype=torch.float32, device="cuda") if accumulate is None else accumulate.clone()
     ctx.rbe_short_range(x, rs, F, accumulate=accumulate is not None, with_energy=with_energy)
