@@ -332,6 +332,10 @@ def main():
         time.sleep(0.15)
     sync()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    # one more UNTIMED step goes out right before the first event: the GPU has been idle since the synchronise (and the
+    # sampler's start-up sleep), and without it the host-side latency of issuing the first timed step lands inside the
+    # region (~100 us: 5 us per step of a 20-step run, 0.5 us of a 200-step run); with it the K timed steps run back to back
+    step(args.warmup - 1)
     e0.record()
     for i in range(args.steps):
         step(args.warmup + i)
