@@ -168,3 +168,17 @@ def test_pair_table_variant(name, rs, alpha):
     assert d.item() <= 1e-5                                               # the two variants against each other
     _, _, F_t2 = run(atoms, cfg.L, a, rs, table=True)
     assert torch.equal(F_t, F_t2)                                         # bitwise reproducible as well
+
+
+def test_very_crowded_cell_beyond_the_candidate_list():
+    """9 000 of 10 000 atoms sit in one cell of the fine list: its candidates exceed what the cell kernel lists in shared
+    memory (8 192 positions; the rest are found by search over the runs) and its own atoms fill 560 M-tiles; the ring kernel
+    walks 280 groups of that cell.  Both against the oracle."""
+    L, alpha, rs = 40.0, 0.09, 10.0
+    rng = np.random.default_rng(16)
+    n = 10_000
+    atoms = np.empty((n, 4), dtype=np.float32)
+    atoms[:, :3] = rng.random((n, 3)) * L
+    atoms[:9000, :3] = 20.1 + rng.random((9000, 3)) * 4.8                   # inside the fine cell [20, 25)^3
+    atoms[:, 3] = np.where(np.arange(n) % 2 == 0, 1.0, -1.0)
+    check(atoms, L, alpha, rs)
