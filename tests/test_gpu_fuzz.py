@@ -74,6 +74,16 @@ def test_randomised_parity_sweep():
             floor = 1e-11 * np.sqrt(N) * max(np.abs(q).max(), 1e-300)       # fixed-point resolution of the accumulators
             assert np.isfinite(Fsg).all(), tag
             assert np.linalg.norm(Fsg[:, :3] - Fs_o) <= 2e-5 * np.linalg.norm(Fs_o) + floor, (tag, rs)
+            for kind, table in ((0, True), (1, False), (1, True)):          # the other force kernel / the tabulated pair term
+                ctx.rbe_set_pair_kernel(kind)
+                ctx.rbe_set_pair_table(table)
+                Fv = torch.full((N, 4), float("nan"), dtype=torch.float32, device="cuda")
+                ctx.rbe_short_range(x, rs, Fv, with_energy=True)
+                Fvg = Fv.cpu().numpy().astype(np.float64)
+                assert np.isfinite(Fvg).all(), (tag, kind, table)
+                assert np.linalg.norm(Fvg[:, :3] - Fs_o) <= 2e-5 * np.linalg.norm(Fs_o) + floor, (tag, rs, kind, table)
+            ctx.rbe_set_pair_kernel(0)
+            ctx.rbe_set_pair_table(False)
             if 2 <= N <= 1200:
                 p, rc = int(rng.integers(1, 33)), float(rng.uniform(0.3, 0.8) * rs)
                 Fr = torch.full((N, 4), float("nan"), dtype=torch.float32, device="cuda")
