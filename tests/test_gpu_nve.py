@@ -93,14 +93,18 @@ def test_deterministic_ewald_trajectory_matches_the_oracle():
     assert ctx.rbe_kspace_energy() == ref.rbe_kspace_energy()
 
 
-def test_random_batch_trajectory_with_the_device_sampler_matches_the_oracle():
+@pytest.mark.parametrize("kind,table", [(0, False), (1, True)], ids=["ring-polynomial", "cells-table"])
+def test_random_batch_trajectory_with_the_device_sampler_matches_the_oracle(kind, table):
     """Eq. (2.12) forces from a fresh batch of P = 100 wavevectors per step, drawn on the device (bit-exact against
-    oracle/sampler.py), inside the captured graph; the oracle loop uses the same batches."""
+    oracle/sampler.py), inside the captured graph; the oracle loop uses the same batches.  Once with the default
+    real-space kernel, once with the tensor-core cell kernel and the tabulated pair term inside the graph."""
     x, v, q, mass, L, alpha, rs = _system()
     P, seed, step0 = 100, 21, 5
     xs, vs, Es = onve.run(x, v, q, mass, L, alpha, rs, DT, NSTEPS,
                           lambda n: osampler.sample_kset(L, alpha, P, seed, step0 + n))
     ctx = rbe.Rbe(x.shape[0], L, alpha, P)
+    ctx.rbe_set_pair_kernel(kind)
+    ctx.rbe_set_pair_table(table)
     pos, vel, inv_m, xyzq, force = _gpu_state(x, v, q, mass)
     ctx.rbe_sample_kvectors(seed, step0)
     ctx.rbe_step(None, xyzq, force)
