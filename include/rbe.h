@@ -126,6 +126,14 @@ rbe_status rbe_set_pair_kernel(rbe_ctx* ctx, int32_t kind);
  * Errors: RBE_ERR_INVALID_ARG. */
 rbe_status rbe_set_pair_table(rbe_ctx* ctx, int32_t on);
 
+/* The same table computed on the HOST (the device kernel and this call run one function), for inspection and for tests
+ * that need no GPU.  *n_out = number of intervals for this r_s: (floor(log2 r_s^2) + 1 + 6) * 32; interval i covers
+ * u = r^2 in u0 + [0, h), u0 = 2^e (1 + m/32), h = 2^e / 32, e = -6 + i / 32, m = i % 32.  h_tf / h_te: float [capacity][4]
+ * (host) or NULL, entry i = {c0, c1, c2, c3} with T(u) ~ c0 + c1 d + c2 d^2 + c3 d^3, d = u - u0, where
+ * T_f(u) = e^{alpha u} g(r)/r (g of Eq. 2.10) and T_e(u) = e^{alpha u} erfc(sqrt(alpha) r)/r.  Both NULL: size query.
+ * Errors: RBE_ERR_INVALID_ARG (also when capacity < *n_out or the table would exceed 1024 intervals). */
+rbe_status rbe_pair_table_host(const rbe_ctx* ctx, double rs, float* h_tf, float* h_te, int32_t capacity, int32_t* n_out);
+
 /* Fill *out with the launch geometry chosen for this context (valid after rbe_set_workspace). */
 rbe_status rbe_get_launch_info(const rbe_ctx* ctx, rbe_launch_info* out);
 

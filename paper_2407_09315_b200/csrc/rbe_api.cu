@@ -539,6 +539,24 @@ rbe_status rbe_set_pair_kernel(rbe_ctx* c, int32_t kind) {
     return RBE_OK;
 }
 
+rbe_status rbe_pair_table_host(const rbe_ctx* c, double rs, float* h_tf, float* h_te, int32_t capacity, int32_t* n_out) {
+    if (!c || !(rs > 0.0) || !std::isfinite(rs) || !n_out) return RBE_ERR_INVALID_ARG;
+    const int emax = (int)std::floor(std::log2(rs * rs)) + 1;
+    int ntab = (emax - rbe::SR_TAB_EMIN) << rbe::SR_TAB_BITS;
+    if (ntab < (1 << rbe::SR_TAB_BITS)) ntab = 1 << rbe::SR_TAB_BITS;
+    if (ntab > rbe::SR_TAB_MAX) return RBE_ERR_INVALID_ARG;
+    *n_out = ntab;
+    if (!h_tf && !h_te) return RBE_OK;                       // size query
+    if (capacity < ntab) return RBE_ERR_INVALID_ARG;
+    for (int i = 0; i < ntab; ++i) {
+        float4 f, e;
+        rbe::sr_table_entry(i, c->alpha, f, e);
+        if (h_tf) { h_tf[4 * i] = f.x; h_tf[4 * i + 1] = f.y; h_tf[4 * i + 2] = f.z; h_tf[4 * i + 3] = f.w; }
+        if (h_te) { h_te[4 * i] = e.x; h_te[4 * i + 1] = e.y; h_te[4 * i + 2] = e.z; h_te[4 * i + 3] = e.w; }
+    }
+    return RBE_OK;
+}
+
 rbe_status rbe_set_pair_table(rbe_ctx* c, int32_t on) {
     if (!c) return RBE_ERR_INVALID_ARG;
     if (on != 0 && on != 1) return fail(c, RBE_ERR_INVALID_ARG, "rbe_set_pair_table: on must be 0 or 1");

@@ -88,28 +88,31 @@ __device__ __forceinline__ void sr_atomic_add_fixed(long long* p, float v) {
 // alpha r_s^2, and intervals of constant RELATIVE width keep a constant relative error: interval i covers
 // u in 2^e (1 + m / 32) + [0, 2^e / 32), e = SR_TAB_EMIN + i / 32, m = i % 32 -- the index is the top bits of the fp32
 // pattern of u, the interval origin is u with the low mantissa bits cleared.  Per interval a cubic in (u - origin)
-// through the four Chebyshev nodes (fp64, erfcx from the CUDA math library); its interpolation error is
+// through the four Chebyshev nodes (fp64, erfcx(x) = e^{x^2} erfc(x)); its interpolation error is
 // <= 2e-7 relative.  Pairs closer than 2^(EMIN / 2) = 0.125 A take the analytic branch.
 // ---------------------------------------------------------------------------------------
 constexpr int SR_TAB_EMIN = -6;          // the table starts at u = 2^-6 A^2 (r = 0.125 A)
 constexpr int SR_TAB_BITS = 5;           // 32 intervals per octave of u
 constexpr int SR_TAB_MAX = 1024;         // entries per table the workspace holds (32 octaves)
 
-__global__ void __launch_bounds__(128) sr_table_kernel(float4* __restrict__ tf, float4* __restrict__ te, int n, double alpha) {
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= n) return;
+// Interval i of the table: its cubic coefficients for T_f (tf) and T_e (te).  Host and device run the same code
+// (rbe_pair_table_host returns the host's copy, which the CPU tests check against the closed forms).
+__host__ __device__ inline void sr_table_entry(int i, double alpha, float4& tf, float4& te) {
     const double base = ldexp(1.0, SR_TAB_EMIN + (i >> SR_TAB_BITS));
     const double h = base / (1 << SR_TAB_BITS), u0 = base + h * (i & ((1 << SR_TAB_BITS) - 1));
     const double sa = sqrt(alpha), c = 2.0 * sa / sqrt(PI_D);
     double tau[4], ff[4], fe[4];
     for (int k = 0; k < 4; ++k) {
         tau[k] = 0.5 * (1.0 - cos((2 * k + 1) * PI_D / 8.0));      // Chebyshev nodes of [0, 1]
-        const double u = u0 + h * tau[k], r = sqrt(u), ex = erfcx(sa * r) / r;
+        const double u = u0 + h * tau[k], r = sqrt(u), x = sa * r;
+        const double x2 = x * x;                                    // erfcx(x) = e^{x^2} erfc(x); its asymptotic series where e^{x^2} would overflow
+        const double ecx = x2 < 600.0 ? exp(x2) * erfc(x) : (1.0 - 0.5 / x2 + 0.75 / (x2 * x2)) / (x * sqrt(PI_D));
+        const double ex = ecx / r;
         fe[k] = ex;
         ff[k] = (ex + c) / u;
     }
     for (int which = 0; which < 2; ++which) {
-        double* f = which ? fe : ff;
+        const double* f = which ? fe : ff;
         // Newton divided differences
         double d[4] = {f[0], f[1], f[2], f[3]};
         for (int lev = 1; lev < 4; ++lev)
@@ -121,8 +124,17 @@ __global__ void __launch_bounds__(128) sr_table_kernel(float4* __restrict__ tf, 
         const double b2 = d[2] - d[3] * (t0 + t1 + t2);
         const double b3 = d[3];
         const float4 o = make_float4((float)b0, (float)(b1 / h), (float)(b2 / (h * h)), (float)(b3 / (h * h * h)));
-        if (which) te[i] = o; else tf[i] = o;
+        if (which) te = o; else tf = o;
     }
+}
+
+__global__ void __launch_bounds__(128) sr_table_kernel(float4* __restrict__ tf, float4* __restrict__ te, int n, double alpha) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    float4 f, e;
+    sr_table_entry(i, alpha, f, e);
+    tf[i] = f;
+    te[i] = e;
 }
 
 // dynamic shared memory of the pair kernel: the table(s), when that variant runs (rbe_set_pair_table)

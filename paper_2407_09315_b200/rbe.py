@@ -64,6 +64,8 @@ def lib():
         L.rbe_set_pair_table.argtypes = [vp, i32]
         L.rbe_set_pair_kernel.restype = ctypes.c_int
         L.rbe_set_pair_kernel.argtypes = [vp, i32]
+        L.rbe_pair_table_host.restype = ctypes.c_int
+        L.rbe_pair_table_host.argtypes = [vp, dbl, vp, vp, i32, ctypes.POINTER(i32)]
         L.rbe_get_launch_info.restype = ctypes.c_int
         L.rbe_get_launch_info.argtypes = [vp, ctypes.POINTER(LaunchInfo)]
         L.rbe_set_kvectors.restype = ctypes.c_int
@@ -220,6 +222,17 @@ class Rbe:
 
     def rbe_set_pair_kernel(self, kind: int):
         self._check(lib().rbe_set_pair_kernel(self._h, int(kind)))
+
+    def rbe_pair_table_host(self, rs: float):
+        """(tf, te): float32 [n, 4] cubic coefficients of the pair-term tables, computed on the host (needs no GPU)."""
+        import numpy as np
+        n = ctypes.c_int32(0)
+        self._check(lib().rbe_pair_table_host(self._h, float(rs), None, None, 0, ctypes.byref(n)))
+        tf = np.zeros((n.value, 4), dtype=np.float32)
+        te = np.zeros((n.value, 4), dtype=np.float32)
+        self._check(lib().rbe_pair_table_host(self._h, float(rs), ctypes.c_void_p(tf.ctypes.data), ctypes.c_void_p(te.ctypes.data),
+                                              n.value, ctypes.byref(n)))
+        return tf, te
 
     def rbe_set_pair_table(self, on: bool):
         self._check(lib().rbe_set_pair_table(self._h, int(bool(on))))

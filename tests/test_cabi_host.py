@@ -144,3 +144,37 @@ def test_product_does_not_import_oracle():
             src = open(os.path.join(ROOT, "oracle", f)).read()
             assert not re.search(r"^\s*(import|from)\s+paper_2407_09315_b200\b", src, flags=re.M), f
             assert "librbe" not in src and "#include \"rbe" not in src, f
+
+
+@pytest.mark.parametrize("alpha,rs", [(0.09, 10.0), (0.35, 6.0), (0.02, 11.3), (0.1156, 30.0), (1.0, 30.0)])
+def test_pair_table_matches_the_closed_forms(alpha, rs):
+    """rbe_pair_table_host (the same function the device kernel runs): the tabulated pair term of P:196 as built here
+    (reading Q23).  Evaluated the way the kernels do -- index and origin from the fp32 bit pattern of u = r^2, cubic
+    in fp32 -- it must reproduce T_f(u) = e^{alpha u} [erfc(x)/r + 2 sqrt(alpha/pi) e^{-x^2}] / u and
+    T_e(u) = e^{alpha u} erfc(x)/r (x = sqrt(alpha) r; written out with scipy) to 1e-6 relative everywhere on
+    [2^-6, r_s^2), i.e. the pair force and energy of Eq. (2.10) / Eq. (2.8) once multiplied by e^{-alpha u}."""
+    from scipy.special import erfcx
+
+    from paper_2407_09315_b200 import rbe
+    ctx = rbe.Rbe(8, 100.0, alpha, 4, allocate=False)
+    tf, te = ctx.rbe_pair_table_host(rs)
+    n = tf.shape[0]
+    assert n == (int(np.floor(np.log2(rs * rs))) + 1 + 6) * 32 and te.shape == (n, 4)
+    rng = np.random.default_rng(3)
+    u = np.concatenate([np.exp(rng.uniform(np.log(2.0 ** -6), np.log(rs * rs), 200_000)),
+                        2.0 ** -6 * (1 + np.arange(64) / 32.0), [np.nextafter(np.float32(rs * rs), np.float32(0))]]).astype(np.float32)
+    u = u[(u >= 2.0 ** -6) & (u < rs * rs)]
+    bits = u.view(np.uint32)
+    idx = (bits >> 18).astype(np.int64) - ((127 - 6) << 5)
+    assert idx.min() == 0 and idx.max() < n
+    d = u - (bits & np.uint32(0xFFFC0000)).view(np.float32)                          # exact in fp32
+    def cubic(t):
+        c = t[idx]
+        return ((c[:, 3] * d + c[:, 2]) * d + c[:, 1]) * d + c[:, 0]                 # fp32 Horner, as the kernels
+    ud = u.astype(np.float64)
+    r = np.sqrt(ud)
+    x = np.sqrt(alpha) * r
+    Te = erfcx(x) / r
+    Tf = (Te + 2.0 * np.sqrt(alpha / np.pi)) / ud
+    assert np.abs(cubic(tf) / Tf - 1).max() <= 1e-6
+    assert np.abs(cubic(te) / Te - 1).max() <= 1e-6
