@@ -102,12 +102,14 @@ __device__ __forceinline__ void sr_cell_pair(const SrCellParams& p, const float4
     } else {                                                 // polynomial erfc; with TABLE: the closest pairs ("below r_0")
         const float inv_r = sr_rsqrt(r2);
         const float x = p.sqrt_alpha * (r2 * inv_r);
-        const float E = sr_ex2(-1.4426950408889634f * x * x);
+        const float E = sr_ex2(p.nalpha_log2e * r2);           // x^2 = alpha r^2: off the rsqrt chain
         const float ec = sr_erfc_from_exp(x, E);
-        s = fmaf(ec, inv_r, two_sa_over_sqrtpi * E) * inv_r * inv_r;
+        s = fmaf(ec, inv_r, two_sa_over_sqrtpi * E) * (inv_r * inv_r);
         u = ec * inv_r;
     }
-    if (!(r2 < p.rs2 && r2 > 0.f)) { s = 0.f; u = 0.f; }   // the exact cutoff test; the atom itself and coincident atoms are skipped (Q18)
+    const bool inside = r2 < p.rs2 && r2 > 0.f;            // the exact cutoff test; the atom itself and coincident atoms are skipped (Q18)
+    s = inside ? s : 0.f;
+    if (ENERGY) u = inside ? u : 0.f;
     const float sj = o.w * s;
     acc.x = fmaf(sj, dx, acc.x); acc.y = fmaf(sj, dy, acc.y); acc.z = fmaf(sj, dz, acc.z);
     if (ENERGY) acc.w = fmaf(o.w, u, acc.w);
