@@ -253,6 +253,54 @@ rbe_status rbe_forces(rbe_ctx* ctx, const void* d_xyzq, void* d_force, int32_t w
 rbe_status rbe_step(rbe_ctx* ctx, const int32_t* h_m, const double* h_w, const void* d_xyzq, void* d_force,
                     int32_t with_energy, void* d_rho, void* stream);
 
+/* rbe_step for a caller that has no device memory to give, and no way to get any.
+ *
+ * Everywhere else in this header the scratch a kernel needs (per-CTA partial sums, the reduced rho, the per-k
+ * force records, the grid-barrier counter) sits in a workspace the CALLER allocates and hands over with
+ * rbe_set_workspace.  That does not suit every host program.  A force plug-in loaded into an MD engine, or into
+ * any application whose own pool has already claimed the GPU's memory, may be given the position and force
+ * arrays and nothing else: cudaMalloc there either fails outright or takes memory the host program counted on.
+ * Code in a time-step loop with a latency budget cannot afford it either, because cudaMalloc and cudaFree
+ * stall the whole device while they run.  For such callers this one call computes the same k-space step --
+ * Algorithm 1 steps 2-4, Eq. (2.9) P:117 then Eq. (2.12), one cooperative launch of the same
+ * kernel as rbe_step -- with its scratch in an array that is part of the library image (a file-scope
+ * `static __device__` array in rbe_api.cu).  The call itself, and everything it calls, uses no cudaMalloc,
+ * cudaFree, cudaMallocHost or other allocating routine; it needs a context from rbe_create (host memory only,
+ * no CUDA call) but NO rbe_set_workspace, and it neither reads nor changes the context's workspace or k-set state
+ * (rbe_kspace_energy, rbe_forces etc. do not see this step).
+ *
+ *   h_m        int32 [P][3], host: the batch of wavevectors, as rbe_set_kvectors (uniform weights S / P only);
+ *              they travel in the kernel parameters, so there is no host-to-device copy to stage
+ *   d_xyzq     float4 [N] device (caller-owned input);  d_force  float4 [N] device (caller-owned output, as
+ *              rbe_forces; .w = e_i if with_energy != 0, else 0);  d_rho  double2 [P] device or NULL (output)
+ *
+ * Limits.  The array is RBE_STATIC_SCRATCH_BYTES = 1 605 888 bytes (about 1.5 MiB): room for
+ * P <= RBE_STATIC_MAX_P = 512 wavevectors and a grid of at most RBE_STATIC_MAX_CTAS = 192 CTAs (the kernel runs
+ * one CTA per SM: 148 on B200).  N is not limited by it (the scratch does not grow with N).  A larger P, or a
+ * device with more SMs than that, is refused with RBE_ERR_WORKSPACE and a message naming the limit; nothing is
+ * launched.  Every GPU on which a process has loaded librbe.so holds one copy of the array, from the moment the
+ * library's code is loaded onto it until the process exits, whether or not this call is ever made.
+ *
+ * First call on a device.  The first rbe_step_static on each device (with that device current) also does a
+ * one-time set-up on the host: it looks up the array's device address (cudaGetSymbolAddress) and raises the
+ * kernel's shared-memory limit.  Make that first call outside any stream capture; later calls only enqueue a
+ * 8-byte memset (the barrier counter must start at zero, and the array keeps whatever the previous call left
+ * in it) and the kernel on `stream`.
+ *
+ * Sharing.  There is ONE array per device, shared by every context, host thread and stream of the process.  Calls
+ * that follow one another on one stream are safe.  Two rbe_step_static calls whose kernels could run at the same
+ * time on one device -- different streams without an event between them, or two host threads -- race on it: wrong
+ * forces, or a grid barrier that never opens.  Serialise them.  It is independent of every workspace, so it may
+ * overlap with the other calls of this header.
+ * Results: the same arithmetic, launch geometry and summation order as the one-launch form of rbe_step with h_m given.
+ * Errors: RBE_ERR_INVALID_ARG (null / misaligned pointer, or the context was first used on another device),
+ *         RBE_ERR_BAD_KVECTOR, RBE_ERR_WORKSPACE (beyond the limits above), RBE_ERR_NO_DEVICE, RBE_ERR_CUDA. */
+#define RBE_STATIC_MAX_P 512
+#define RBE_STATIC_MAX_CTAS 192
+#define RBE_STATIC_SCRATCH_BYTES 1605888
+rbe_status rbe_step_static(rbe_ctx* ctx, const int32_t* h_m, const void* d_xyzq, void* d_force, int32_t with_energy,
+                           void* d_rho, void* stream);
+
 /* Real-space partner of the RBE force: the short-range part of the Ewald-split Coulomb force,
  * Eq. (2.10), truncated at the cutoff radius r_s, over a linked-cell list of cubic
  * cells of side >= r_s (a one-shot cell list; Algorithm 2's own list has cells of side r_c):

@@ -6,6 +6,7 @@
 #include <cmath>
 #include <cstdio>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <string>
 #include <vector>
@@ -1344,3 +1345,146 @@ const char* rbe_status_string(rbe_status s) {
 int32_t rbe_version(void) { return 100; }
 
 }  // extern "C"
+
+// ------------------------------------------------------------------------------------------------------------
+// rbe_step_static: the k-space step without a caller-provided workspace (include/rbe.h gives the reasons: a
+// plug-in inside a host program that owns all device memory, or a loop that cannot take cudaMalloc's stall).
+// The scratch of step_kernel -- per-CTA fp64 rows, k-set copy, rho, the per-k force records, the barrier
+// counter -- is carved from ONE array that is part of this library's device image.  Nothing on this path
+// allocates; the array holds its contents from call to call and is shared by every caller on the device.
+namespace {
+
+constexpr size_t ST_OFF_PART = 0;                                                                         // double2 [rows][P]
+constexpr size_t ST_OFF_KVEC = ST_OFF_PART + (size_t)RBE_STATIC_MAX_CTAS * RBE_STATIC_MAX_P * sizeof(double2);   // int4 [P]
+constexpr size_t ST_OFF_RHO = ST_OFF_KVEC + (size_t)RBE_STATIC_MAX_P * sizeof(int4);                      // double2 [P]
+constexpr size_t ST_OFF_KA = ST_OFF_RHO + (size_t)RBE_STATIC_MAX_P * sizeof(double2);                     // int4 [P]
+constexpr size_t ST_OFF_KB = ST_OFF_KA + (size_t)RBE_STATIC_MAX_P * sizeof(int4);                         // float4 [P]
+constexpr size_t ST_OFF_BAR = ST_OFF_KB + (size_t)RBE_STATIC_MAX_P * sizeof(float4);                      // u64, on a line of its own
+constexpr size_t ST_BYTES = ST_OFF_BAR + 256;
+static_assert(ST_BYTES == RBE_STATIC_SCRATCH_BYTES, "rbe.h states the size of the built-in scratch");
+static_assert(RBE_STATIC_MAX_P <= rbe::STEP_KPARAM_MAX, "the wavevectors must fit the kernel parameters");
+static_assert(ST_OFF_KVEC % 256 == 0 && ST_OFF_BAR % 256 == 0, "sub-arrays stay 256-byte aligned");
+
+}  // namespace
+
+// In HOST code this name is only a handle for cudaGetSymbolAddress: it is not a device address, and a kernel
+// handed `g_static_scratch` itself would fault (or scribble over host memory where the GPU can reach it).
+static __device__ __align__(256) unsigned char g_static_scratch[ST_BYTES];
+
+namespace {
+
+constexpr int STATIC_MAX_DEVICES = 64;
+struct StaticDevice {
+    unsigned char* base = nullptr;   // device address of g_static_scratch on this device (nullptr: set-up not done)
+    int smem_max = 0;                // dynamic shared memory the step kernels may use there
+    int coop = 0;
+};
+StaticDevice g_static_dev[STATIC_MAX_DEVICES];
+std::mutex g_static_mu;
+
+// Once per device, with that device current: the address of the array as the GPU sees it, and the kernel
+// attributes rbe_step would have set through the context.  No allocation; not to be run under stream capture.
+rbe_status static_setup(rbe_ctx* c, int dev, StaticDevice* out) {
+    std::lock_guard<std::mutex> lock(g_static_mu);
+    StaticDevice& d = g_static_dev[dev];
+    if (!d.base) {
+        void* ptr = nullptr;
+        RBE_CUDA(c, cudaGetSymbolAddress(&ptr, g_static_scratch));
+        if (!ptr || (reinterpret_cast<uintptr_t>(ptr) & 255u))
+            return fail(c, RBE_ERR_CUDA, "rbe_step_static: cudaGetSymbolAddress returned a null or misaligned address");
+        int optin = 0, coop = 0;
+        RBE_CUDA(c, cudaDeviceGetAttribute(&optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev));
+        RBE_CUDA(c, cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev));
+        const int smem_max = optin - 4 * 1024;   // as init_device: the kernels' static shared memory stays under 4 KB
+        RBE_CUDA(c, cudaFuncSetAttribute(rbe::step_kernel<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_max));
+        RBE_CUDA(c, cudaFuncSetAttribute(rbe::step_kernel<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_max));
+        RBE_CUDA(c, cudaFuncSetAttribute(rbe::step_kernel<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_max));
+        RBE_CUDA(c, cudaFuncSetAttribute(rbe::step_kernel<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_max));
+        d.smem_max = smem_max;
+        d.coop = coop;
+        d.base = static_cast<unsigned char*>(ptr);   // last: marks the set-up as done
+    }
+    *out = d;
+    return RBE_OK;
+}
+
+}  // namespace
+
+extern "C" rbe_status rbe_step_static(rbe_ctx* c, const int32_t* h_m, const void* d_xyzq, void* d_force, int32_t with_energy,
+                                      void* d_rho, void* stream) {
+    if (!c) return RBE_ERR_INVALID_ARG;
+    if (!h_m) return fail(c, RBE_ERR_INVALID_ARG, "rbe_step_static: h_m is null (the wavevectors travel with the call)");
+    if ((c->N > 0 && (!d_xyzq || !d_force)) || (reinterpret_cast<uintptr_t>(d_xyzq) & 15u) || (reinterpret_cast<uintptr_t>(d_force) & 15u) ||
+        (reinterpret_cast<uintptr_t>(d_rho) & 15u))
+        return fail(c, RBE_ERR_INVALID_ARG, "rbe_step_static: null or misaligned pointer");
+    // the limits of the built-in array come first: they do not depend on the device
+    if (c->P > RBE_STATIC_MAX_P)
+        return fail(c, RBE_ERR_WORKSPACE, "rbe_step_static: P = " + std::to_string(c->P) + " exceeds the built-in scratch (P <= " +
+                                              std::to_string(RBE_STATIC_MAX_P) + "); use rbe_step with a caller-allocated workspace");
+    rbe_status s = check_kvectors(c, h_m, nullptr);
+    if (s != RBE_OK) return s;
+    s = init_device(c);   // launch geometry for this (N, P) on the current device: queries only
+    if (s != RBE_OK) return s;
+    int dev = -1;
+    RBE_CUDA(c, cudaGetDevice(&dev));
+    if (dev != c->device) return fail(c, RBE_ERR_INVALID_ARG, "rbe_step_static: the context was first used on another device");
+    if (dev < 0 || dev >= STATIC_MAX_DEVICES) return fail(c, RBE_ERR_NO_DEVICE, "rbe_step_static: device ordinal beyond 63");
+    StaticDevice sd;
+    s = static_setup(c, dev, &sd);
+    if (s != RBE_OK) return s;
+    const int G = c->li.sf_grid_x;
+    if (G > RBE_STATIC_MAX_CTAS || G > c->li.num_sms)
+        return fail(c, RBE_ERR_WORKSPACE, "rbe_step_static: a grid of " + std::to_string(G) + " CTAs exceeds the built-in scratch (<= " +
+                                              std::to_string(RBE_STATIC_MAX_CTAS) + " rows)");
+    if (!sd.coop || c->li.sf_grid_y != 1 || c->step_smem > (size_t)sd.smem_max)
+        return fail(c, RBE_ERR_CUDA, "rbe_step_static: the device cannot run the one-launch step kernel for this P");
+
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    unsigned char* base = sd.base;
+    // The array still holds the previous call's contents.  Only the barrier counter has to start from a known
+    // value (a multiple of this call's grid size; zero is one): rows, rho and records are rewritten before use.
+    RBE_CUDA(c, cudaMemsetAsync(base + ST_OFF_BAR, 0, sizeof(unsigned long long), st));
+
+    rbe::StepParams sp;
+    sp.sf.xyzq = static_cast<const float4*>(d_xyzq);
+    sp.sf.N = c->N;
+    sp.sf.part = reinterpret_cast<double2*>(base + ST_OFF_PART);
+    sp.sf.two32_over_L = rbe::TWO32 / c->L;
+    sp.sf.P = c->P; sp.sf.gs = c->sf_gs; sp.sf.ng = c->sf_ng;
+    sp.sf.pairing = c->sf_pairing;
+    sp.sf.accumulate = 0;
+    sp.f.xyzq = static_cast<const float4*>(d_xyzq);
+    sp.f.force = static_cast<float4*>(d_force);
+    sp.f.N = c->N;
+    sp.f.two32_over_L = rbe::TWO32 / c->L;
+    sp.kvec = reinterpret_cast<const int4*>(base + ST_OFF_KVEC);
+    sp.w = nullptr;
+    sp.w_uniform = c->S / (double)c->P;
+    sp.L = c->L;
+    sp.rho = reinterpret_cast<double2*>(base + ST_OFF_RHO);
+    sp.rho_user = static_cast<double2*>(d_rho);
+    sp.ka = reinterpret_cast<int4*>(base + ST_OFF_KA);
+    sp.kb = reinterpret_cast<float4*>(base + ST_OFF_KB);
+    sp.bar = reinterpret_cast<unsigned long long*>(base + ST_OFF_BAR);
+    sp.kparam = 1;
+    for (int32_t i = 0; i < 3 * c->P; ++i) sp.km[i] = (int16_t)h_m[i];   // validated above: |m_d| < 2^15
+
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((unsigned)G);
+    cfg.blockDim = dim3((unsigned)c->li.sf_threads);
+    cfg.dynamicSmemBytes = c->step_smem;
+    cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeCooperative;
+    attr[0].val.cooperative = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    if (c->sf_deep) {
+        if (with_energy) RBE_CUDA(c, cudaLaunchKernelEx(&cfg, rbe::step_kernel<true, true>, sp));
+        else RBE_CUDA(c, cudaLaunchKernelEx(&cfg, rbe::step_kernel<true, false>, sp));
+    } else {
+        if (with_energy) RBE_CUDA(c, cudaLaunchKernelEx(&cfg, rbe::step_kernel<false, true>, sp));
+        else RBE_CUDA(c, cudaLaunchKernelEx(&cfg, rbe::step_kernel<false, false>, sp));
+    }
+    return RBE_OK;
+}

@@ -101,6 +101,8 @@ def lib():
         L.rbe_forces.argtypes = [vp, vp, vp, i32, vp]
         L.rbe_step.restype = ctypes.c_int
         L.rbe_step.argtypes = [vp, vp, vp, vp, vp, i32, vp, vp]
+        L.rbe_step_static.restype = ctypes.c_int
+        L.rbe_step_static.argtypes = [vp, vp, vp, vp, i32, vp, vp]
         L.rbe_step_host_bytes.restype = sz
         L.rbe_step_host_bytes.argtypes = [vp, i32]
         L.rbe_probe_pipe_rates.restype = ctypes.c_int
@@ -324,6 +326,24 @@ class Rbe:
         self._check(lib().rbe_step(self._h, _np_ptr(mm), _np_ptr(ww), ctypes.c_void_p(xyzq.data_ptr()),
                                    ctypes.c_void_p(force.data_ptr()), int(bool(with_energy)),
                                    None if rho is None else ctypes.c_void_p(rho.data_ptr()), _stream_ptr(stream)))
+
+    def rbe_step_static(self, m, xyzq, force, with_energy: bool = False, rho=None, stream=None):
+        """rbe_step for callers that cannot allocate device memory (a plug-in inside a program whose pool owns the
+        GPU's memory; a loop that cannot take cudaMalloc's device-wide stall): the kernel's scratch is an array built
+        into librbe.so, so the context needs no workspace (`Rbe(..., allocate=False)` works).  m: numpy int32 [P,3]
+        (host, required); xyzq, force: cuda float32 [N,4]; rho: cuda float64 [P,2] or None.  P <= 512.  One array per
+        device, shared by all callers: keep calls on one stream, or order them with events.  The first call on a
+        device does a one-time set-up and should be made outside stream capture.  See include/rbe.h."""
+        import numpy as np
+        _check_tensor(xyzq, (self.N, 4), "float32")
+        _check_tensor(force, (self.N, 4), "float32")
+        if rho is not None:
+            _check_tensor(rho, (self.P, 2), "float64")
+        mm = np.ascontiguousarray(m, dtype=np.int32)
+        assert mm.shape == (self.P, 3), mm.shape
+        self._check(lib().rbe_step_static(self._h, _np_ptr(mm), ctypes.c_void_p(xyzq.data_ptr()),
+                                          ctypes.c_void_p(force.data_ptr()), int(bool(with_energy)),
+                                          None if rho is None else ctypes.c_void_p(rho.data_ptr()), _stream_ptr(stream)))
 
     def rbe_step_bound(self, xyzq, force, with_energy: bool = False, rho=None, stream=None):
         """rbe_step with everything but the k-set marshalled ONCE: returns call(m) for m a C-contiguous numpy int32
