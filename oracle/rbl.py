@@ -35,7 +35,8 @@ Plain numpy, fp64, one atom at a time: O(N^2).  Pins (tests/test_oracle_rbl.py):
 reproduces oracle.short_range exactly; sum_i F_i = 0 after the correction; the mean over steps
 converges to oracle.short_range (unbiasedness) with the 1/sqrt(T) law; the keys: bijectivity of
 fmix32 (inverted with the modular inverses of its multipliers), avalanche, and a chi-square test that every
-shell member is picked with probability p / N_s; Philox itself by the Random123 vectors
+shell member is picked with probability p / N_s, and correlation tests that the batches of different atoms, of the two
+directions of a pair and of consecutive steps are independent; Philox itself by the Random123 vectors
 (tests/test_oracle_sampler.py).
 """
 from __future__ import annotations

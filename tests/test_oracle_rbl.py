@@ -120,3 +120,51 @@ def test_batch_is_a_uniform_p_subset_of_the_shell():
         q2 = p * (p - 1) / (n * (n - 1))
         assert abs(off.mean() - T * q2) <= 1e-9 * T          # exact: every batch has p (p - 1) ordered pairs
         assert off.std() <= 1.6 * np.sqrt(T * q2 * (1 - q2)), (off.std(), np.sqrt(T * q2))
+
+
+def test_batches_are_independent_across_atoms_and_across_steps():
+    """Eq. (2.15)'s variance and the unbiasedness of the corrected sum need more than the right marginal
+    p / N_s: the batches of different atoms, and of one atom at different steps, must not move together.  With
+    salted hash keys only 64 bits of salt change from step to step, so this is checked, not assumed: over T steps the
+    inclusion indicators X_t(i, j) = [j in B(i)] of (a) two atoms i != i' looking at the same neighbour j, (b) the
+    two directions of one pair, X(i, j) and X(j, i), and (c) the same pair at consecutive steps, are uncorrelated --
+    sample correlations behave as N(0, 1/T), so the sum of T r^2 over K such combinations is chi-square with about K
+    degrees of freedom.  A key that ignored i (every atom picks the same neighbours), a symmetric key (u_ij = u_ji),
+    or a salt that moved only a few key bits per step fails by a wide margin (r = 1 gives T per term)."""
+    n_atoms, n_i, p, T = 40, 8, 6, 2000
+    X = np.zeros((T, n_i, n_atoms), dtype=np.float64)
+    for t in range(T):
+        for i in range(n_i):
+            shell = np.array([j for j in range(n_atoms) if j != i])
+            keys = rbl.pair_keys(i, shell, 2024, t).astype(np.uint64)
+            X[t, i, shell[np.lexsort((shell, keys))[:p]]] = 1.0
+    q = p / (n_atoms - 1)
+    assert abs(X.sum() - T * n_i * p) == 0
+    Xc = X - q                              # the exact mean of every indicator that is not structurally zero
+    var = q * (1 - q)
+
+    def chi2(a, b):
+        """sum over the trailing axes of T r^2, r = sample correlation over the step axis (known mean and variance)"""
+        r = (a * b).mean(0) / var
+        return float((T * r ** 2).sum()), r.size
+
+    # (a) same neighbour j, two different atoms: j runs over the atoms outside 0 .. n_i - 1 (in every shell)
+    tot, dof = 0.0, 0
+    for i in range(n_i):
+        for k in range(i + 1, n_i):
+            c, d = chi2(Xc[:, i, n_i:], Xc[:, k, n_i:])
+            tot, dof = tot + c, dof + d
+    assert dof == 28 * 32 and tot <= dof + 5 * np.sqrt(2 * dof), (tot, dof)
+    assert tot >= dof - 5 * np.sqrt(2 * dof), (tot, dof)          # neither correlated nor suspiciously regular
+    # (b) the two directions of a pair
+    a = np.stack([X[:, i, k] for i in range(n_i) for k in range(i + 1, n_i)], 1) - q
+    b = np.stack([X[:, k, i] for i in range(n_i) for k in range(i + 1, n_i)], 1) - q
+    tot, dof = chi2(a, b)
+    assert dof == 28 and tot <= dof + 5 * np.sqrt(2 * dof), (tot, dof)
+    # (c) consecutive steps, same ordered pair
+    tot, dof = chi2(Xc[:-1, :, n_i:], Xc[1:, :, n_i:])
+    tot *= (T - 1) / T
+    assert dof == n_i * 32 and tot <= dof + 5 * np.sqrt(2 * dof), (tot, dof)
+    # and a lag of two steps, in case consecutive salts were related pairwise
+    tot, dof = chi2(Xc[:-2, :, n_i:], Xc[2:, :, n_i:])
+    assert tot <= dof + 5 * np.sqrt(2 * dof), (tot, dof)
