@@ -397,7 +397,11 @@ rbe_status rbe_step_host_xyz(rbe_ctx* ctx, const float* h_xyz, const int32_t* h_
  * rbe_nve_kick:  v += half_dt * F / m  from d_force float4 [N] (.w ignored); then, if d_pos != NULL, the drift
  *   x += dt * v and d_xyzq[i].xyz = (float) x[i] (d_xyzq[i].w, the charge, is kept).  One step of the scheme is
  *   kick(dt/2, drift dt) -> forces at the new positions -> kick(dt/2, no drift).  Enqueues one kernel.
- * rbe_nve_energies:  h_out double [2] (host) = { sum_i 1/2 m_i v_i^2 (0 if d_vel == NULL), sum_i d_force[i].w
+ *   An inverse mass of 0 freezes an atom's velocity.  Positions are NOT wrapped into the box: the fp64 positions stay
+ *   continuous (handy for displacements), and the force kernels are exactly periodic, but the fp32 copy in d_xyzq
+ *   loses resolution as |x| grows (ulp(x) = 2^-23 |x|), so in runs where atoms diffuse over many box lengths the caller
+ *   should subtract whole box vectors from d_pos now and then.
+ * rbe_nve_energies:  h_out double [2] (host) = { sum_i 1/2 m_i v_i^2 over the atoms with inverse mass > 0 (0 if d_vel == NULL), sum_i d_force[i].w
  *   (0 if d_force == NULL: with_energy forces carry the per-atom potential energies there) }, fp64, fixed order;
  *   synchronises `stream`; needs the workspace.
  * rbe_md_capture:  one whole MD step -- kick + drift, [a fresh batch from the device sampler if sampled != 0:

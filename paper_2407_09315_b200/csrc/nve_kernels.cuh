@@ -39,7 +39,10 @@ __global__ void __launch_bounds__(256) nve_energy_partial_kernel(const double* _
     for (int64_t i = (int64_t)blockIdx.x * 256 + threadIdx.x; i < N; i += (int64_t)gridDim.x * 256) {
         if (vel) {
             const double vx = vel[3 * i], vy = vel[3 * i + 1], vz = vel[3 * i + 2];
-            ke += 0.5 * (vx * vx + vy * vy + vz * vz) / inv_mass[i];
+            // a frozen atom (inverse mass 0: the kick never moves it) has no finite kinetic energy to report and is
+            // left out of the sum; dividing by its inverse mass would turn the whole sum into NaN (0 / 0) or inf
+            const double im = inv_mass[i];
+            if (im > 0.0) ke += 0.5 * (vx * vx + vy * vy + vz * vz) / im;
         }
         if (force) sw += (double)force[i].w;
     }

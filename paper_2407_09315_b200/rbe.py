@@ -412,14 +412,17 @@ class Rbe:
         n = self.rbe_short_range_bytes(rs)
         if n == 0:
             raise RbeError(1, "rbe_md_capture: need 0 < r_s <= L/3")
-        if getattr(self, "_sr_ws", None) is None or self._sr_ws.numel() < n:
-            self._sr_ws = torch.empty(n, dtype=torch.uint8, device="cuda")
-        self._graph_buffers = (pos, vel, inv_mass, xyzq, force)
+        # The graph records the ADDRESS of its short-range scratch, so it gets a tensor of its own, kept alive beside
+        # the other arrays the graph is bound to and never rebound: rbe_short_range / rbe_rbl_forces may replace the
+        # shared self._sr_ws by a larger one at any time (the RBL cell list can need more bytes), which would leave a
+        # graph that used it replaying into freed memory.
+        graph_sr_ws = torch.empty(n, dtype=torch.uint8, device="cuda")
         self._check(lib().rbe_md_capture(self._h, ctypes.c_void_p(pos.data_ptr()), ctypes.c_void_p(vel.data_ptr()),
                                          ctypes.c_void_p(inv_mass.data_ptr()), ctypes.c_void_p(xyzq.data_ptr()),
                                          ctypes.c_void_p(force.data_ptr()), float(rs), float(dt),
-                                         ctypes.c_void_p(self._sr_ws.data_ptr()), self._sr_ws.numel(), int(bool(sampled)),
+                                         ctypes.c_void_p(graph_sr_ws.data_ptr()), graph_sr_ws.numel(), int(bool(sampled)),
                                          int(seed), int(first_step), int(bool(with_energy))))
+        self._graph_buffers = (pos, vel, inv_mass, xyzq, force, graph_sr_ws)   # replaced only after the new graph exists
 
     def rbe_short_range_bytes(self, rs: float) -> int:
         return int(lib().rbe_short_range_bytes(self._h, float(rs)))

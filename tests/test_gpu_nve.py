@@ -130,7 +130,50 @@ def test_energy_sums_and_argument_checks():
     assert abs(ke - 0.5 * (mass[:, None] * v * v).sum()) <= 1e-13 * ke
     assert sw == 0.25 * x.shape[0] * (x.shape[0] - 1) / 2
     assert ctx.rbe_nve_energies(None, None, force)[0] == 0.0
+    # frozen atoms (inverse mass 0) are left out of the kinetic energy instead of turning it into NaN (0 / 0)
+    inv_f, vel_f = inv_m.clone(), vel.clone()
+    inv_f[:5] = 0.0
+    vel_f[:3] = 0.0
+    ke_f = ctx.rbe_nve_energies(vel_f, inv_f, force)[0]
+    assert abs(ke_f - 0.5 * (mass[5:, None] * v[5:] * v[5:]).sum()) <= 1e-13 * ke
+    ctx.rbe_nve_kick(vel_f, inv_f, force, 0.5 * DT)
+    assert torch.equal(vel_f[:5], torch.cat([torch.zeros_like(vel[:3]), vel[3:5]]))   # and the kick leaves them alone
     with pytest.raises(rbe.RbeError):
         ctx.rbe_md_capture(pos, vel, inv_m, xyzq, force, rs, DT, sampled=False)        # no k-set yet
     with pytest.raises(rbe.RbeError):
         ctx.rbe_md_capture(pos, vel, inv_m, xyzq, force, rs, -1.0, sampled=True, seed=1)
+
+
+def test_captured_graph_owns_its_short_range_scratch():
+    """The MD graph records the address of its short-range scratch.  The binding used to lend it the context's shared
+    scratch tensor, which rbe_short_range / rbe_rbl_forces replace by a larger one when they need more bytes: the graph
+    then replayed into freed memory.  Now the graph has a tensor of its own: calls that grow the shared scratch between
+    replays change nothing, bit for bit."""
+    x, v, q, mass, L, alpha, rs = _system()
+    P, seed = 64, 3
+    results = []
+    for disturb in (False, True):
+        ctx = rbe.Rbe(x.shape[0], L, alpha, P)
+        pos, vel, inv_m, xyzq, force = _gpu_state(x, v, q, mass)
+        ctx.rbe_sample_kvectors(seed, 0)
+        ctx.rbe_step(None, xyzq, force)
+        ctx.rbe_short_range(xyzq, 0.5 * rs, force, accumulate=True)     # a small shared scratch exists before the capture
+        force.zero_()
+        ctx.rbe_step(None, xyzq, force)
+        ctx.rbe_short_range(xyzq, rs, force, accumulate=True)
+        ctx.rbe_md_capture(pos, vel, inv_m, xyzq, force, rs, DT, sampled=True, seed=seed, first_step=1)
+        graph_ws = ctx._graph_buffers[-1]
+        assert graph_ws.data_ptr() != ctx._sr_ws.data_ptr()
+        other = torch.empty_like(force)
+        for n in range(20):
+            ctx.rbe_graph_launch()
+            if disturb and n % 5 == 0:
+                ctx._sr_ws = None                                        # the shared scratch is dropped and rebuilt ...
+                junk = torch.full((1 << 20,), 0xFF, dtype=torch.uint8, device="cuda")   # ... and its memory reused
+                ctx.rbe_rbl_forces(xyzq.clone(), 0.5 * rs, rs, 8, seed, n, other)
+                del junk
+        torch.cuda.synchronize()
+        assert ctx._graph_buffers[-1] is graph_ws
+        results.append((pos.clone(), vel.clone(), force.clone()))
+    for a, b in zip(*results):
+        assert torch.equal(a, b)
