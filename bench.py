@@ -138,9 +138,11 @@ class ClockSampler:
         return out
 
 
-def time_oracle(cfg_name, n_sample, steps, warmup, threads=None):
+def time_oracle(cfg_name, n_sample, steps, warmup, threads=None, last_kset=None):
     """The oracle as it stands, timed on the host cores, on the first n_sample atoms of the
-    workload (cost is linear in atoms) with the workload's full batch of P wavevectors."""
+    workload (cost is linear in atoms) with the workload's full batch of P wavevectors.
+    last_kset: the k-set index of the LAST timed oracle step (the others keep 0, 1, ...), so that its result can be
+    compared with what the GPU computed for that same k-set; the last (rho, F) are returned in `keep`."""
     import oracle
     from paper_2407_09315_b200 import inputs
     cfg = workload_config(cfg_name, 1)
@@ -149,19 +151,21 @@ def time_oracle(cfg_name, n_sample, steps, warmup, threads=None):
     if threads:
         oracle.set_threads(threads)
     S = oracle.S(cfg.L, cfg.alpha)
-    ts = []
+    ts, keep = [], None
     for it in range(warmup + steps):
-        m = inputs.sample_kset(cfg.L, cfg.alpha, cfg.P, cfg.seed, it)
+        k_idx = last_kset if (last_kset is not None and it == warmup + steps - 1) else it
+        m = inputs.sample_kset(cfg.L, cfg.alpha, cfg.P, cfg.seed, k_idx)
         t0 = time.perf_counter()
         rho = oracle.rho(atoms, cfg.L, m)
-        oracle.force(atoms, cfg.L, m, S, rho)
+        F = oracle.force(atoms, cfg.L, m, S, rho)
         dt = time.perf_counter() - t0
         if it >= warmup:
             ts.append(dt)
+        keep = (k_idx, rho, F)
     per_step = sum(ts) / len(ts)
     used = oracle.max_threads()
     oracle.set_threads(all_threads)
-    return per_step, per_step / n_sample * 1e9, used, cfg
+    return per_step, per_step / n_sample * 1e9, used, cfg, keep
 
 
 def workload_config(name, world):
@@ -178,18 +182,26 @@ def run_reference(args):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
-    n_sample = args.ref_atoms
     steps, warmup = max(1, args.steps), max(0, args.warmup)
-    # keep the whole run within a few minutes whatever --steps says
-    budget_s, est_per_atom = 150.0, 200 * 100e-9
-    n_sample = int(min(n_sample, max(1000, budget_s / ((steps + warmup) * est_per_atom))))
-    per_step, ns_atom, cores, cfg = time_oracle(args.config, n_sample, steps, warmup)
-    sample = f"first {n_sample} atoms of {cfg.name} (N={cfg.N}), all P={cfg.P} wavevectors, oracle.rho + oracle.force"
+    cfg0 = workload_config(args.config, 1)
+    # The whole workload if the host cores manage it within the budget (N = 999 999, P = 200: ~0.7 s per step on 16
+    # threads), else a prefix of the atoms (the cost is linear in atoms): sized from a probe on 20 000 atoms.
+    n_probe = min(20_000, cfg0.N)
+    t_probe, _, _, _, _ = time_oracle(args.config, n_probe, 1, 1)
+    budget_s = 150.0
+    n_fit = int(budget_s / ((steps + warmup) * max(t_probe / n_probe, 1e-12)))
+    n_sample = cfg0.N if args.ref_atoms <= 0 else min(args.ref_atoms, cfg0.N)
+    n_sample = max(min(n_sample, n_fit), min(1000, cfg0.N))
+    per_step, ns_atom, cores, cfg, _ = time_oracle(args.config, n_sample, steps, warmup)
+    what = "all" if n_sample == cfg.N else "first"
+    sample = f"{what} {n_sample} atoms of {cfg.name} (N={cfg.N}), all P={cfg.P} wavevectors, oracle.rho + oracle.force"
     print(json.dumps({
         "impl": "reference", "metric": METRIC, "value": ns_atom, "unit": UNIT, "n_gpus": args.gpus,
         "steps": steps, "warmup": warmup, "ms_per_step": per_step * 1e3, "higher_is_better": False,
         "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": cfg.name, "N": cfg.N, "P": cfg.P, "L": cfg.L, "alpha": cfg.alpha},
+        # the same keys the GPU arm prints for the workload (one rank runs the oracle: N_total = N_per_gpu = the config's N)
+        "config": {"workload": cfg.name, "N_per_gpu": cfg.N, "N_total": cfg.N, "P": cfg.P, "L": cfg.L, "alpha": cfg.alpha,
+                   "sample_atoms": n_sample},
         "cpu_baseline": {"value": ns_atom, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
         "e2e": {"value": ns_atom, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
@@ -203,7 +215,9 @@ def main():
     ap.add_argument("--warmup", type=int, default=20)
     ap.add_argument("--config", default="water_nacl_1m")
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
-    ap.add_argument("--ref-atoms", type=int, default=100_000)
+    ap.add_argument("--ref-atoms", type=int, default=0, help="--impl reference: atoms per oracle step (0 = the whole workload, "
+                    "cut down only if the host cores cannot finish it within ~150 s)")
+    ap.add_argument("--no-md", action="store_true")
     ap.add_argument("--cpu-baseline-atoms", type=int, default=1_000_000)
     ap.add_argument("--cpu-baseline-steps", type=int, default=15)
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -342,6 +356,20 @@ def main():
     e1.record()
     sync()
     ms_total = e0.elapsed_time(e1)
+    # the forces the LAST timed step left in its buffer, for parity_in_run (compared with the oracle in the cpu_baseline leg)
+    i_last = args.warmup + args.steps - 1
+    F_last = fs[i_last % n_rot].cpu().numpy() if world == 1 else None
+    rho_last, rerun_equal = None, None
+    if world == 1:
+        # the same step once more, untimed, into fresh buffers and with the structure factors returned: it must
+        # reproduce the timed step's forces bit for bit (a timed step that skipped work would not)
+        f_chk = torch.full((n_local, 4), float("nan"), dtype=torch.float32, device="cuda")
+        rho_chk = torch.full((P, 2), float("nan"), dtype=torch.float64, device="cuda")
+        ctx.rbe_step(ksets[i_last % n_k], xs[i_last % n_rot], f_chk, with_energy=args.with_energy, rho=rho_chk)
+        sync()
+        rerun_equal = bool(np.array_equal(f_chk.cpu().numpy(), F_last))
+        rho_last = rho_chk.cpu().numpy()
+        del f_chk, rho_chk
 
     # ---- region A2: the same K steps with CUDA events around every step, for the median and the minimum;
     # the headline stays region A's mean, which carries no per-step event
@@ -352,6 +380,23 @@ def main():
         evs_a[i][1].record()
     sync()
     t_step = sorted(e[0].elapsed_time(e[1]) for e in evs_a)
+
+    # ---- region A3: the same K steps with the charge pairing of the structure-factor phase switched off
+    # (rbe_set_pairing(0)): what a system whose atoms all carry different |q| would see -- 2 special-function
+    # evaluations per pair there instead of the 1.5 that water's equal charges allow
+    ms_unpaired = None
+    if world == 1:
+        ctx.rbe_set_pairing(0)
+        for i in range(3):
+            step(i)
+        sync()
+        e0.record()
+        for i in range(args.steps):
+            step(args.warmup + i)
+        e1.record()
+        sync()
+        ms_unpaired = e0.elapsed_time(e1) / args.steps
+        ctx.rbe_set_pairing(3)
 
     # ---- timed region B: the same K steps in the two-launch form with CUDA events around each call, for the
     # per-kernel durations of sf_kernel and f_kernel
@@ -455,6 +500,46 @@ def main():
                               "than the deterministic sum on B200 (instruction budget: profiles/r02_rbl_README.md)"},
               "note": "rbe_short_range: bin + scan + scatter + sort + group boxes + pair kernel (every unordered pair "
                       "once, fixed-point integer atomics across warps) + finalise; not part of `value`"}
+
+    # ---- one whole MD step (velocity Verlet P:78, NVE P:86): rbe_md_capture's graph -- kick +
+    # drift, device sampler, k-space step, rbe_short_range (accumulate), kick -- replayed on ~1e6 ions at the
+    # workload's density
+    md = None
+    if world == 1 and not args.no_md:
+        cells = max(2, int(round((n_local / 2.0) ** (1.0 / 3.0))))
+        a_cell = (2.0 / inputs.DENSITY) ** (1.0 / 3.0)                     # bcc cell side for 0.1 ions per A^3
+        x_m, v_m, q_m, mass_m, L_m = inputs.plasma(cells, a=a_cell, seed=11, jitter=0.05, v_rms=0.04)
+        n_m = x_m.shape[0]
+        if L_m >= 3 * args.rs:
+            mctx = rbe.Rbe(n_m, L_m, alpha, P)
+            pos_m = torch.from_numpy(x_m).cuda()
+            vel_m = torch.from_numpy(v_m).cuda()
+            inv_m = torch.from_numpy(1.0 / mass_m).cuda()
+            xyzq_m = torch.from_numpy(np.concatenate([x_m.astype(np.float32), q_m[:, None]], axis=1)).cuda().contiguous()
+            force_m = torch.zeros((n_m, 4), dtype=torch.float32, device="cuda")
+            mctx.rbe_sample_kvectors(base.seed, 0)
+            mctx.rbe_step(None, xyzq_m, force_m)
+            mctx.rbe_short_range(xyzq_m, args.rs, force_m, accumulate=True)
+            mctx.rbe_md_capture(pos_m, vel_m, inv_m, xyzq_m, force_m, args.rs, 0.2, sampled=True, seed=base.seed, first_step=1)
+            k_md = max(3, min(args.steps, 20))
+            for i in range(3):
+                mctx.rbe_graph_launch()
+            sync()
+            e0.record()
+            for i in range(k_md):
+                mctx.rbe_graph_launch()
+            e1.record()
+            sync()
+            ms_md = e0.elapsed_time(e1) / k_md
+            finite = bool(torch.isfinite(pos_m).all().item() and torch.isfinite(force_m).all().item())
+            k_launch = 2 if bool(mctx.rbe_get_launch_info()["step_fused"]) else 3      # sampler + step (or + sf + f)
+            md = {"ms_per_step": ms_md, "value": ms_md * 1e6 / n_m, "unit": UNIT, "N": n_m, "L": L_m, "r_s": args.rs, "dt_tau": 0.2,
+                  "steps": k_md, "graph_launches_per_step": 1, "kernels_per_step": 2 + k_launch + 7, "memsets_per_step": 2,
+                  "finite": finite,
+                  "note": "rbe_md_capture replayed by rbe_graph_launch: kick+drift, sample_kernel, k-space step, rbe_short_range "
+                          "(7 kernels, 2 memsets, accumulate), kick; one-component plasma (bcc, +1 e, implied background) at 0.1 ions/A^3, "
+                          "positions and velocities fp64 resident on the device; not part of `value`"}
+            del mctx, pos_m, vel_m, inv_m, xyzq_m, force_m
 
     if world > 1:
         t = torch.tensor([ms_total, ms_sf, ms_f, ms_two], dtype=torch.float64, device="cuda")
@@ -601,27 +686,57 @@ def main():
             "note": "rbe_graph_launch: device sampler (Philox) + the k-space step replayed as one CUDA graph, "
                     "no per-step H2D; not the headline (the k-set there comes from the host each step)"},
         "short_range": sr,
+        "md_step": md,
         "clocks": clocks,
         "gpu_launches": (1 if one_launch else 2) * args.steps,
         "paper_context": "8.20 ms/step, 1e6 atoms, A100, RBL+RBE nonbonded total, P=100 (PAPER.md P:284); 2.89 ms k-space at 1e5 atoms, P=200 (P:266)",
     }
+    if ms_unpaired is not None:
+        out["roofline"]["unpaired"] = {
+            "ms_per_step": ms_unpaired, "value": ms_unpaired * 1e6 / n_total,
+            "frac": 2 * SFU_PER_PAIR_PER_KERNEL * pairs / (ms_unpaired * 1e-3) / mufu_rate,   # of the whole step (both phases)
+            "executed_mufu_per_pair": 2.0 + MUFU_EXECUTED_PER_PAIR["f"],
+            "note": "the timed steps again with rbe_set_pairing(0): no two atoms share a special-function evaluation in the structure-"
+                    "factor phase -- the figure a system with all-distinct |q| would see; `frac` as roofline.frac (algorithmic count)"}
     if e2e:
         out["e2e"] = e2e
     if not args.no_cpu_baseline and world == 1:
         n_s = min(args.cpu_baseline_atoms, base.N)
         k_cpu = max(1, args.cpu_baseline_steps)
-        per_step, ns_cpu, cores, _ = time_oracle(args.config, n_s, k_cpu, 1)
+        per_step, ns_cpu, cores, _, keep = time_oracle(args.config, n_s, k_cpu, 1, last_kset=i_last % n_k)
+        # parity inside this run: the oracle's last timed step used the k-set of the GPU's last timed step, so its
+        # output doubles as the check that the timed region did the work (no extra oracle time is spent)
+        if n_s == base.N and F_last is not None:
+            _, rho_o, F_o = keep
+            qsum = float(np.abs(atoms[:, 3].astype(np.float64)).sum())
+            d_f = F_last[:, :3].astype(np.float64) - F_o
+            parity = {"F_relL2": float(np.linalg.norm(d_f) / np.linalg.norm(F_o)),
+                      "rho_err": float(np.abs(rho_last - rho_o).max() / qsum),
+                      "tolerance": {"F_relL2": 2e-5, "rho_err": 1e-6}, "atoms": int(n_s), "kset_step": int(i_last % n_k),
+                      "timed_step_reproduced_bitwise": rerun_equal,
+                      "what": "forces left by the LAST timed step (all 3N components) and rho of the same step re-run, against "
+                              "oracle.rho / oracle.force on the same atoms and k-set (the cpu_baseline leg's last step)"}
+            parity["passed"] = bool(parity["F_relL2"] <= 2e-5 and parity["rho_err"] <= 1e-6 and rerun_equal)
+            out["parity_in_run"] = parity
+        else:
+            out["parity_in_run"] = {"passed": None, "timed_step_reproduced_bitwise": rerun_equal,
+                                    "what": "the cpu_baseline sample is smaller than the workload: no oracle comparison in this run"}
         # the same oracle on ONE thread, on a sample sized for ~5 s: a bare core count would mislead
         n_1 = max(1000, min(n_s, 25_000))
-        per_step1, ns_cpu1, _, _ = time_oracle(args.config, n_1, 1, 1, threads=1)
+        per_step1, ns_cpu1, _, _, _ = time_oracle(args.config, n_1, 1, 1, threads=1)
         out["cpu_baseline"] = {"value": ns_cpu, "unit": UNIT, "cores": cores, "kind": "oracle",
                                "one_thread": {"value": ns_cpu1, "unit": UNIT, "sample_atoms": n_1},
                                "speedup_all_threads_vs_one": ns_cpu1 / ns_cpu,
                                "sample": f"first {n_s} atoms of {base.name} (N={base.N}), all P={P} wavevectors, oracle.rho + "
                                          f"oracle.force, {k_cpu} steps after 1 warm-up ({per_step * k_cpu:.1f} s of CPU work)"}
+    if "parity_in_run" not in out:
+        out["parity_in_run"] = {"passed": None, "timed_step_reproduced_bitwise": rerun_equal, "what": "no cpu_baseline leg in this run"}
     print(json.dumps(out))
     if world > 1:
         dist.destroy_process_group()
+    if out["parity_in_run"]["passed"] is False or rerun_equal is False:
+        print("bench: the timed step's output FAILED its in-run check: " + json.dumps(out["parity_in_run"]), file=sys.stderr)
+        raise SystemExit(1)
 
 
 if __name__ == "__main__":

@@ -13,7 +13,7 @@ ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 
 def test_bench_json_line_contract():
     cmd = [sys.executable, os.path.join(ROOT, "bench.py"), "--config", "water_96k", "--steps", "5", "--warmup", "3",
-           "--cpu-baseline-atoms", "20000", "--cpu-baseline-steps", "1"]
+           "--cpu-baseline-atoms", "96000", "--cpu-baseline-steps", "1"]
     res = subprocess.run(cmd, capture_output=True, text=True, timeout=600, cwd=ROOT)
     assert res.returncode == 0, res.stderr[-2000:]
     lines = [l for l in res.stdout.splitlines() if l.startswith("{")]
@@ -41,3 +41,13 @@ def test_bench_json_line_contract():
     assert [k["kernel"] for k in d["roofline_kernels"]] == ["sf_kernel", "f_kernel"]
     assert c["one_thread"]["value"] > 0 and c["speedup_all_threads_vs_one"] > 0
     assert d["kernels_ms"]["two_launch_step"] > 0 and d["kernels_ms"]["step_call"] == d["ms_per_step"]
+    # honesty keys of round 3: the timed step checked against the oracle inside the run, the step without charge pairing,
+    # one whole MD step
+    pr = d["parity_in_run"]
+    assert pr["passed"] is True and pr["timed_step_reproduced_bitwise"] is True and pr["atoms"] == 96000
+    assert pr["F_relL2"] <= 2e-5 and pr["rho_err"] <= 1e-6
+    un = r["unpaired"]
+    assert un["ms_per_step"] > 0 and un["executed_mufu_per_pair"] == 3.0 and abs(un["value"] - un["ms_per_step"] * 1e6 / 96000) < 1e-9
+    md = d["md_step"]
+    assert md["ms_per_step"] > d["short_range"]["ms_per_call"] * 0.2 and md["graph_launches_per_step"] == 1 and md["finite"] is True
+    assert md["kernels_per_step"] == 11 and 90_000 <= md["N"] <= 100_000
