@@ -115,12 +115,10 @@ __device__ __forceinline__ void sr_cell_pair(const SrCellParams& p, const float4
     if (ENERGY) acc.w = fmaf(o.w, u, acc.w);
 }
 
-#ifndef RBE_SR_CELL_CTAS
-#define RBE_SR_CELL_CTAS 6
-#endif
+constexpr int SR_CELL_CTAS = 6;   // resident CTAs per SM asked of the compiler (80 registers); sweep: profiles/r02_sr_designs.md
 
 template <bool ENERGY, bool TABLE>
-__global__ void __launch_bounds__(32 * SR_W, RBE_SR_CELL_CTAS) sr_cell_kernel(const SrCellParams p) {
+__global__ void __launch_bounds__(32 * SR_W, SR_CELL_CTAS) sr_cell_kernel(const SrCellParams p) {
     extern __shared__ __align__(16) unsigned char sr_dyn_smem[];      // the pair-term table(s), then the candidate list
     __shared__ float4 cposw[SR_W][4 * 33];                 // per warp: its slice's candidates, word-major [word][bit], one slot of padding per word
     __shared__ __align__(16) float fa[SR_W][SR_SLICE * 4]; // candidate nl: {x^hi, y^hi, z^hi, x^lo}

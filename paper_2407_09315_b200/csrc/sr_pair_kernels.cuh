@@ -142,13 +142,8 @@ __host__ __device__ constexpr size_t sr_pair_smem_bytes(int ntab, bool table, bo
     return table ? (size_t)ntab * sizeof(float4) * (energy ? 2 : 1) : 0;
 }
 
-#ifndef RBE_SR_PAIR_WARPS
-#define RBE_SR_PAIR_WARPS 4
-#endif
-#ifndef RBE_SR_PAIR_CTAS
-#define RBE_SR_PAIR_CTAS 9
-#endif
-constexpr int SR_PAIR_WARPS = RBE_SR_PAIR_WARPS;
+constexpr int SR_PAIR_WARPS = 4;   // warps per CTA
+constexpr int SR_PAIR_CTAS = 9;    // resident CTAs per SM asked of the compiler
 
 // the own cell, then the 13 forward neighbours: (dz > 0) or (dz == 0 and dy > 0) or (dz == dy == 0 and dx > 0)
 __constant__ int8_t SR_HALF_STENCIL[14][3] = {
@@ -157,7 +152,7 @@ __constant__ int8_t SR_HALF_STENCIL[14][3] = {
 
 // TABLE: pair terms from the table (the paper's method); else erfc by the polynomial (sr_erfc_from_exp)
 template <bool ENERGY, bool TABLE>
-__global__ void __launch_bounds__(32 * SR_PAIR_WARPS, RBE_SR_PAIR_CTAS) sr_pair_kernel(const SrPairParams p) {
+__global__ void __launch_bounds__(32 * SR_PAIR_WARPS, SR_PAIR_CTAS) sr_pair_kernel(const SrPairParams p) {
     __shared__ float4 vpos[SR_PAIR_WARPS][32];   // the visiting group: positions relative to THIS cell's centre, charge
     __shared__ float4 vacc[SR_PAIR_WARPS][32];   // ... and what this warp adds to its atoms
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
