@@ -92,7 +92,10 @@ size_t rbe_workspace_bytes(const rbe_ctx* ctx);
  * allocated on the current CUDA device.  Caller keeps ownership and must keep it alive.  The buffer belongs to
  * THIS context alone for as long as it is set (it holds state that survives from launch to launch: the k-set,
  * rho, the step counter of the device sampler, the arrival counter of rbe_step's grid barrier, which the call
- * zeroes and which must stay a multiple of the context's grid size): never share it between contexts.
+ * zeroes and which must stay a multiple of the context's grid size): never share it between contexts.  The library keeps
+ * a list of the buffers its live contexts hold and refuses (RBE_ERR_WORKSPACE) a buffer whose first
+ * rbe_workspace_bytes bytes overlap another live context's; rbe_destroy, or giving that context another buffer, frees
+ * the claim.  Several workspaces may be carved out of one allocation as long as they do not overlap.
  * Errors: RBE_ERR_WORKSPACE, RBE_ERR_NO_DEVICE, RBE_ERR_CUDA. */
 rbe_status rbe_set_workspace(rbe_ctx* ctx, void* d_ws, size_t bytes);
 

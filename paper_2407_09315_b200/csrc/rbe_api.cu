@@ -107,6 +107,31 @@ rbe_status cuda_fail(rbe_ctx* c, const char* what, cudaError_t e) {
         if (e__ != cudaSuccess) return cuda_fail(ctx, #call, e__); \
     } while (0)
 
+// Which live context owns which workspace buffer.  A workspace carries state from launch to launch (the k-set, rho, the
+// sampler's step counter, the arrival counter of step_kernel's grid barrier, which must stay a multiple of ONE grid size):
+// two contexts on one buffer corrupt each other silently or leave a grid barrier waiting for arrivals that never come.
+// No sanitizer run can vouch for the callers on this pool, so rbe_set_workspace refuses the overlap instead.
+struct WsClaim { const rbe_ctx* owner; int device; uintptr_t lo, hi; };
+std::mutex g_ws_mu;
+std::vector<WsClaim> g_ws_claims;
+
+void ws_release(const rbe_ctx* c) {
+    std::lock_guard<std::mutex> lock(g_ws_mu);
+    for (size_t i = 0; i < g_ws_claims.size();)
+        if (g_ws_claims[i].owner == c) { g_ws_claims[i] = g_ws_claims.back(); g_ws_claims.pop_back(); } else ++i;
+}
+
+// true if [lo, hi) on `device` is free of every other context's claim; then it becomes c's (replacing c's previous one)
+bool ws_claim(const rbe_ctx* c, int device, uintptr_t lo, uintptr_t hi) {
+    std::lock_guard<std::mutex> lock(g_ws_mu);
+    for (const WsClaim& w : g_ws_claims)
+        if (w.owner != c && w.device == device && lo < w.hi && w.lo < hi) return false;
+    for (size_t i = 0; i < g_ws_claims.size();)
+        if (g_ws_claims[i].owner == c) { g_ws_claims[i] = g_ws_claims.back(); g_ws_claims.pop_back(); } else ++i;
+    g_ws_claims.push_back({c, device, lo, hi});
+    return true;
+}
+
 // Philox4x32-10 (Salmon et al., SC'11) on the host, for the one call per step that salts the RBL pair keys
 void philox4x32_10_host(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3, uint32_t k0, uint32_t k1, uint32_t out[4]) {
     for (int r = 0; r < 10; ++r) {
@@ -476,6 +501,7 @@ rbe_status rbe_create(rbe_ctx** out, int64_t N, double L, double alpha, int32_t 
 
 rbe_status rbe_destroy(rbe_ctx* c) {
     if (!c) return RBE_OK;
+    ws_release(c);
     for (int i = 0; i < NSTAGE; ++i) {
         if (c->stage_ev[i]) cudaEventDestroy(c->stage_ev[i]);
         if (c->stage[i]) cudaFreeHost(c->stage[i]);
@@ -511,6 +537,10 @@ rbe_status rbe_set_workspace(rbe_ctx* c, void* d_ws, size_t bytes) {
     if (s != RBE_OK) return s;
     if (!d_ws || bytes < c->ws_bytes || (reinterpret_cast<uintptr_t>(d_ws) & 255u))
         return fail(c, RBE_ERR_WORKSPACE, "workspace must be non-null, 256-byte aligned and >= rbe_workspace_bytes");
+    // only the bytes this context uses are claimed: a caller may carve several workspaces out of one allocation
+    if (!ws_claim(c, c->device, reinterpret_cast<uintptr_t>(d_ws), reinterpret_cast<uintptr_t>(d_ws) + c->ws_bytes))
+        return fail(c, RBE_ERR_WORKSPACE, "rbe_set_workspace: the buffer overlaps the workspace of another live context "
+                                          "(a workspace belongs to one context until that context is destroyed or given another buffer)");
     c->ws = static_cast<unsigned char*>(d_ws);
     c->have_k = c->have_w = c->have_rho = false;
     // the structure-factor kernel's completion ticket starts at zero and resets itself

@@ -843,7 +843,13 @@ __device__ __forceinline__ unsigned long long grid_barrier_base(const unsigned l
     return v - v % gridDim.x;
 }
 // All threads of all CTAs.  Release: barrier + red.release by thread 0; acquire: its polling load before the barrier
-// that lets the CTA continue.
+// that lets the CTA continue.  No timeout on the wait: the CTAs of a cooperative launch are co-resident by construction, a
+// kernel that faults leaves a sticky error that ends the process's use of the device anyway, and the one way to put the
+// counter out of step from outside -- two contexts on one workspace -- is refused by rbe_set_workspace.
+// (The base stays in thread 0's registers on purpose: parked in shared memory it frees two registers and removes 8 of
+// the 28 spilled bytes, and the step gets 7 us SLOWER at N = 1e6 -- 176.9 against 170.0 us, measured in round 3; the same
+// happened when the CTA's atom range was parked there, which brings the stack frame to 0 bytes: 176.5 us.  The spills
+// sit at tile boundaries, outside the special-function loops, and the allocation ptxas finds with them is the faster one.)
 __device__ __forceinline__ void grid_barrier(unsigned long long* ctr, unsigned long long target) {
     __syncthreads();
     if (threadIdx.x == 0) {
