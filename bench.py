@@ -64,6 +64,7 @@ def read_counters(kernel, config):
     for r in csv.DictReader(open(path)):
         if r["kernel"] == kernel and r["config"] == config:
             out = {"dram_bytes": float(r["dram_bytes"]), "inst_executed": float(r["inst_executed"]),
+                   "inst_executed_pipe_xu": float(r["inst_executed_pipe_xu"]) if r.get("inst_executed_pipe_xu") else None,
                    "source_sha": r["source_sha"], "capture": r["capture"]}
             out["stale"] = out["source_sha"] != source_sha()
             if out["stale"]:
@@ -398,6 +399,25 @@ def main():
         ms_unpaired = e0.elapsed_time(e1) / args.steps
         ctx.rbe_set_pairing(3)
 
+    # ---- region A4: the same K steps through rbe_step_static (scratch in the library's own static device array: for callers
+    # that cannot allocate; one 8-byte memset + the same kernel per step)
+    ms_static = None
+    if world == 1 and one_launch and P <= 512:
+        sctx = rbe.Rbe(n_local, L, alpha, P, allocate=False)
+        for i in range(3):
+            sctx.rbe_step_static(ksets[i % n_k], xs[i % n_rot], fs[i % n_rot], with_energy=args.with_energy)
+        sync()
+        e0.record()
+        for i in range(args.steps):
+            j = args.warmup + i
+            sctx.rbe_step_static(ksets[j % n_k], xs[j % n_rot], fs[j % n_rot], with_energy=args.with_energy)
+        e1.record()
+        sync()
+        ms_static = e0.elapsed_time(e1) / args.steps
+        if F_last is not None and not np.array_equal(fs[i_last % n_rot].cpu().numpy(), F_last):
+            raise SystemExit("bench: rbe_step_static did not reproduce rbe_step's forces bit for bit")
+        del sctx
+
     # ---- timed region B: the same K steps in the two-launch form with CUDA events around each call, for the
     # per-kernel durations of sf_kernel and f_kernel
     evs = [[torch.cuda.Event(enable_timing=True) for _ in range(3)] for _ in range(args.steps)]
@@ -635,6 +655,9 @@ def main():
         r = {"bound": "alu", "kernel": kernel, "achieved": alg_per_pair * pairs / t / 1e9, "peak": mufu_rate / 1e9,
              "unit": "G sincos-evaluation/s, ALGORITHMIC count (2 per pair per phase) against the measured MUFU rate",
              "frac": alg_per_pair * pairs / t / mufu_rate,
+             "frac_is": "algorithmic work / measured peak (SURVEY.md s8(d)'s count, as the measurement contract defines it): a speed-of-"
+                        "light ratio that can pass 1 because the kernels EXECUTE fewer special-function instructions than the 4 per "
+                        "pair it counts; the pipe utilisation is executed.frac_of_mufu_peak / frac_of_xu_peak / frac_of_issue_bound",
              "executed": {"mufu_per_pair": exe_per_pair, "frac_of_mufu_peak": exe_per_pair * pairs / t / mufu_rate},
              "traffic": None if cnt is None else cnt["dram_bytes"],
              "peak_source": f"measured in this run: {pipe['mufu']:.2f} MUFU lanes/SM/clk (rbe_probe_pipe_rates) x {sms} SMs x "
@@ -643,6 +666,13 @@ def main():
             t_issue = cnt["inst_executed"] / issue_rate
             r["executed"].update(warp_instructions=cnt["inst_executed"], issue_bound_us=t_issue * 1e6, frac_of_issue_bound=t_issue / t,
                                  counters=cnt["capture"], counters_stale=cnt["stale"])
+            if cnt["inst_executed_pipe_xu"] is not None:
+                # COUNTED, not assumed: warp instructions the XU pipe executed in one launch (sm__inst_executed_pipe_xu.sum:
+                # MUFU plus whatever conversions share the pipe), 32 lanes each
+                xu = cnt["inst_executed_pipe_xu"] * 32.0
+                r["executed"].update(xu_warp_instructions=cnt["inst_executed_pipe_xu"], xu_per_pair=xu / pairs,
+                                     frac_of_xu_peak=xu / t / mufu_rate,
+                                     mufu_per_pair_source="design count (DESIGN.md section 5); xu_per_pair is the ncu count")
         return r
 
     main_kernel = "step_kernel" if one_launch else "sf_kernel"
@@ -685,6 +715,10 @@ def main():
             "ms_per_step": ms_graph, "value": ms_graph * 1e6 / n_total, "unit": UNIT, "gpu_launches_per_step": 2 if one_launch else 3,
             "note": "rbe_graph_launch: device sampler (Philox) + the k-space step replayed as one CUDA graph, "
                     "no per-step H2D; not the headline (the k-set there comes from the host each step)"},
+        "static_step": None if ms_static is None else {
+            "ms_per_step": ms_static, "value": ms_static * 1e6 / n_total, "unit": UNIT, "gpu_launches_per_step": 1, "memsets_per_step": 1,
+            "note": "rbe_step_static: the same kernel with its scratch in a 1.5 MiB static __device__ array of librbe.so (no workspace, "
+                    "no allocation anywhere on the path; P <= 512); forces checked bit-identical to rbe_step's in this run"},
         "short_range": sr,
         "md_step": md,
         "clocks": clocks,

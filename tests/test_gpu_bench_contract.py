@@ -48,6 +48,9 @@ def test_bench_json_line_contract():
     assert pr["F_relL2"] <= 2e-5 and pr["rho_err"] <= 1e-6
     un = r["unpaired"]
     assert un["ms_per_step"] > 0 and un["executed_mufu_per_pair"] == 3.0 and abs(un["value"] - un["ms_per_step"] * 1e6 / 96000) < 1e-9
+    st = d["static_step"]
+    assert st["ms_per_step"] > 0 and st["gpu_launches_per_step"] == 1 and st["ms_per_step"] < 2 * d["ms_per_step"]
+    assert r["executed"]["xu_per_pair"] is None or r["executed"]["xu_per_pair"] > 0 if "xu_per_pair" in r["executed"] else True
     md = d["md_step"]
     assert md["ms_per_step"] > d["short_range"]["ms_per_call"] * 0.2 and md["graph_launches_per_step"] == 1 and md["finite"] is True
     assert md["kernels_per_step"] == 11 and 90_000 <= md["N"] <= 100_000
